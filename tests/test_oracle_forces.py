@@ -1,0 +1,165 @@
+"""Pins for the oracle's geometry, energy and forces (PAPER.md:39 Eq. 1, :154-169 Eq. A1-A5).
+
+Nothing here compares the oracle with itself: closed forms for regular hexagons, central finite
+differences of Eq. A1 (the energy is a different code path from the force), conservation laws,
+and an independent numpy shoelace / scipy cross-check."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1702_02939_b200 import workloads as w
+from tests import helpers as h
+
+PARAMS = dict(KA=1.0, KP=1.0, A0=1.0, P0=3.8)
+
+
+def test_hexagon_closed_forms_and_zero_force():
+    """Regular hexagons of side a: A = (3 sqrt3 / 2) a^2, P = 6a, and F = 0 on every vertex for
+    any (A0, P0): three identical cells meet at 120 degrees (SURVEY 8(c) pins)."""
+    for a, A0, P0 in [(1.0, 1.0, 3.8), (0.62, 1.0, 3.6), (0.9, 2.5, 1.0)]:
+        t = w.hex_tiling(6, 4, a=a)
+        sim = oracle.from_tiling(t, KA=1.3, KP=0.7, A0=A0, P0=P0)
+        F, ap = sim.compute_forces()
+        assert np.allclose(ap[:, 0], 1.5 * np.sqrt(3.0) * a * a, rtol=1e-13, atol=0)
+        assert np.allclose(ap[:, 1], 6.0 * a, rtol=1e-13, atol=0)
+        assert np.abs(F).max() <= 1e-12
+        E = sim.energy()
+        E_closed = t.N * (1.3 * (1.5 * np.sqrt(3.0) * a * a - A0) ** 2 + 0.7 * (6 * a - P0) ** 2)
+        assert abs(E - E_closed) <= 1e-12 * max(1.0, E_closed)
+
+
+def test_single_moved_vertex_in_hexagons_closed_form():
+    """Move one vertex of a hexagonal tiling outward along an edge direction: the perimeter and
+    area changes of the three cells have elementary closed forms (catches a wrong prev/next)."""
+    a = 1.0
+    t = w.hex_tiling(6, 4, a=a)
+    v = 5
+    nb = t.vertex_neighbors[v]
+    d = t.pos[nb[0]] - t.pos[v]
+    d[0] = h.min_image(d[0], t.Lx); d[1] = h.min_image(d[1], t.Ly)
+    eps = 0.1
+    pos = t.pos.copy()
+    pos[v] += eps * d / np.linalg.norm(d)        # slide along edge to neighbour 0
+    sim = oracle.from_tiling(t)
+    sim.set_positions(np.mod(pos, [t.Lx, t.Ly]))
+    ap = sim.geometry()
+    A_hex = 1.5 * np.sqrt(3.0)
+    cells = t.vertex_cell_neighbors[v]
+    # each of the two cells containing edge (v, n0) loses the triangle (v_old, v_new, its other
+    # neighbour of v); the cell opposite the edge gains both triangles; total area is conserved
+    assert abs(ap[:, 0].sum() - t.Lx * t.Ly) < 1e-12 * t.Lx * t.Ly
+    tri = 0.5 * eps * a * np.sin(2 * np.pi / 3)  # sides eps and a enclosing 120 degrees
+    dA = ap[cells, 0] - A_hex
+    assert np.allclose(sorted(dA), [-tri, -tri, 2 * tri], atol=1e-13)
+    # perimeters: edge (v,n0) shortens by eps; the other two edges become sqrt(a^2+eps^2+a*eps)
+    l2 = np.sqrt(a * a + eps * eps + a * eps)
+    dP = ap[cells, 1] - 6 * a
+    expect = sorted([(-eps) + (l2 - a), (-eps) + (l2 - a), 2 * (l2 - a)])
+    assert np.allclose(sorted(dP), expect, atol=1e-13)
+
+
+@pytest.mark.parametrize("N,L,seed", [(64, 8.0, 1), (100, 10.0, 3)])
+def test_forces_match_finite_differences_of_energy(N, L, seed):
+    """F = -dE/dh (Eq. A2) against central differences of Eq. A1, to 1e-6 relative."""
+    t = w.voronoi_tiling(N, L, seed)
+    sim = oracle.from_tiling(t, **PARAMS)
+    F, ap0 = sim.compute_forces()
+    rms = np.sqrt((F ** 2).sum(axis=1).mean())
+    worst = 0.0
+    others_checked = False
+    for v in range(t.V):
+        cells = t.vertex_cell_neighbors[v]
+        # step well below the shortest incident edge (the perimeter has derivatives ~ 1/l^k) and a
+        # 4th-order central stencil, so truncation stays far below the 1e-6 target
+        dn = t.pos[t.vertex_neighbors[v]] - t.pos[v]
+        lmin = np.hypot(h.min_image(dn[:, 0], t.Lx), h.min_image(dn[:, 1], t.Ly)).min()
+        delta = min(1e-5, 1e-2 * lmin)
+        g = np.zeros(2)
+        for ax in range(2):
+            e = {}
+            for m in (-2, -1, 1, 2):
+                pos = t.pos.copy()
+                pos[v, ax] += m * delta
+                pos[v, ax] %= (t.Lx, t.Ly)[ax]
+                sim.set_positions(pos)
+                ap = sim.geometry()
+                # only the three cells of v change: difference their energies alone (less round-off)
+                e[m] = np.sum(PARAMS["KA"] * (ap[cells, 0] - PARAMS["A0"]) ** 2 +
+                              PARAMS["KP"] * (ap[cells, 1] - PARAMS["P0"]) ** 2)
+                if not others_checked:
+                    others = np.setdiff1d(np.arange(N), cells)
+                    assert np.array_equal(ap[others], ap0[others])
+                    others_checked = True
+            g[ax] = (8 * (e[1] - e[-1]) - (e[2] - e[-2])) / (12 * delta)
+        err = np.linalg.norm(F[v] + g) / max(np.linalg.norm(F[v]), rms)
+        worst = max(worst, err)
+    assert worst < 1e-6, worst
+
+
+@pytest.mark.parametrize("k", [0, 1])
+def test_conservation_laws_on_configs(k):
+    t = w.config_tiling(k)
+    p = w.config_params(k)
+    sim = oracle.from_tiling(t, **p)
+    F, ap = sim.compute_forces()
+    L2 = t.Lx * t.Ly
+    assert abs(ap[:, 0].sum() - L2) <= 1e-12 * L2                      # areas tile the box
+    scale = np.abs(F).sum(axis=0)
+    assert (np.abs(F.sum(axis=0)) <= 1e-10 * np.maximum(scale, 1.0)).all()   # translation invariance
+    assert np.abs(F.sum(axis=0)).max() < 1e-10
+    # geometry against an independent numpy shoelace
+    ref = h.polygon_areas_numpy(t.pos, t.cell_vertex_num, t.cell_vertices, t.Lx, t.Ly)
+    assert np.allclose(ap, ref, rtol=1e-12, atol=1e-13)
+
+
+def test_forces_invariant_under_rigid_shift():
+    """Shifting all positions by a vector (with wrap) must not change A, P or F: tests the
+    minimum-image / wrap handling across the box boundary."""
+    t = w.config_tiling(0)
+    p = w.config_params(0)
+    sim = oracle.from_tiling(t, **p)
+    F0, ap0 = sim.compute_forces()
+    rng = np.random.default_rng(0)
+    for _ in range(5):
+        shift = rng.uniform(0, t.Lx, size=2)
+        sim.set_positions(np.mod(t.pos + shift, [t.Lx, t.Ly]))
+        F, ap = sim.compute_forces()
+        assert np.allclose(ap, ap0, rtol=1e-12, atol=1e-13)
+        assert np.allclose(F, F0, rtol=0, atol=1e-11)
+
+
+def test_force_of_area_and_perimeter_terms_separately():
+    """K_P = 0: force is the pressure term only; for a single inflated cell pressure pushes its
+    vertices outward.  K_A = 0 with P > P0: tension pulls neighbours together (sign pins)."""
+    t = w.hex_tiling(6, 4, a=1.0)
+    A_hex = 1.5 * np.sqrt(3.0)
+    # all cells at preferred area except that A0 is smaller than A: every cell wants to shrink,
+    # symmetric -> zero force; now enlarge one cell by moving one of its vertices outward
+    c = 9
+    v = t.cell_vertices[c, 0]
+    polys = h.unwrapped_polygons(t.pos, t.cell_vertex_num, t.cell_vertices, t.Lx, t.Ly)
+    centre = polys[c].mean(axis=0)
+    out = polys[c][0] - centre
+    out /= np.linalg.norm(out)
+    pos = t.pos.copy()
+    pos[v] = np.mod(pos[v] + 0.05 * out, [t.Lx, t.Ly])
+    sim = oracle.from_tiling(t, KA=1.0, KP=0.0, A0=A_hex, P0=0.0)
+    sim.set_positions(pos)
+    F, ap = sim.compute_forces()
+    assert ap[c, 0] > A_hex
+    assert F[v] @ out < 0          # restoring: pushed back toward the centre of the enlarged cell
+    sim2 = oracle.from_tiling(t, KA=0.0, KP=1.0, A0=0.0, P0=6.0)
+    sim2.set_positions(pos)
+    F2, ap2 = sim2.compute_forces()
+    assert ap2[c, 1] > 6.0
+    assert F2[v] @ out < 0         # line tension also restores
+
+
+def test_energy_definition_has_no_half():
+    """Eq. 1 has no 1/2: E for a single perturbed configuration recomputed from A, P in numpy."""
+    t = w.config_tiling(0)
+    p = w.config_params(0)
+    sim = oracle.from_tiling(t, **p)
+    ap = h.polygon_areas_numpy(t.pos, t.cell_vertex_num, t.cell_vertices, t.Lx, t.Ly)
+    E = np.sum(p["KA"] * (ap[:, 0] - p["A0"]) ** 2 + p["KP"] * (ap[:, 1] - p["P0"]) ** 2)
+    assert abs(sim.energy() - E) <= 1e-12 * E
