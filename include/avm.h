@@ -1,0 +1,175 @@
+/* avm.h — C ABI of the B200-native active-vertex-model (AVM) hot path.
+ *
+ * One overdamped timestep of a 3-coordinated polygonal tiling in a periodic box, as defined by
+ * arXiv:1702.02939 ("cellGPU", D. M. Sussman); citations below are lines of
+ * /root/reference/PAPER.md with the section/equation they fall in.  R-numbers refer to the
+ * readings of the paper listed in DESIGN.md.
+ *
+ *   state    : vertex positions h_v in [0,Lx)x[0,Ly); cell directors theta_c; the three flat
+ *              topology lists of PAPER.md:66 (§II.B): vertices around each cell in
+ *              counter-clockwise order, vertices each vertex is connected to, cells that border
+ *              each vertex.
+ *   one step : geometry of every cell -> force on every vertex -> move the vertices (Eq. 4) ->
+ *              rotate the directors -> one T1 pass on the moved positions
+ *              (PAPER.md:62-64 §II.B, :104-108 §II.D).
+ *
+ * Conventions common to every entry point
+ *   - Plain C, no exceptions cross the boundary.  Return 0 on success, a negative AVM_E* code
+ *     otherwise; avm_strerror() names it.
+ *   - "device pointer" = CUDA global memory on params.device; "host pointer" = ordinary (pageable
+ *     or pinned) host memory.  The *_host twins take host pointers and do the copies themselves.
+ *   - The library never allocates or frees device memory: the caller passes one workspace of
+ *     avm_workspace_bytes() bytes (256-byte aligned) that must outlive the avm_sim.  The avm_sim
+ *     object itself owns only host-side bookkeeping.
+ *   - All work is enqueued on the CUDA stream given at creation.  avm_step never synchronises the
+ *     host (the AVM loop has no host<->device traffic).
+ *   - Every user-visible array is in USER ORDER (the order given to avm_create), whatever the
+ *     internal Hilbert order is.  Index layout, all C-contiguous:
+ *       pos_xy                [V][2] double   vertex positions
+ *       cell_vertex_num       [N]    int32    number of vertices of each cell (3..S)
+ *       cell_vertices         [N][S] int32    CCW vertex list of each cell, unused slots = -1
+ *       vertex_neighbors      [V][3] int32    the three vertices joined to v, CCW around v
+ *       vertex_cell_neighbors [V][3] int32    slot k = the cell between edges (v,n_k), (v,n_k+1),
+ *                                             i.e. in that cell's row (n_k+1, v, n_k) are consecutive
+ *       theta                 [N]    double   director angle of each cell (not wrapped)
+ *     Any OUTPUT pointer may be NULL (that array is skipped).
+ */
+#ifndef AVM_H_
+#define AVM_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct avm_sim avm_sim; /* opaque */
+
+typedef struct avm_params {
+  int32_t n_cells;           /* N                                                               */
+  int32_t n_vertices;        /* V, must equal 2N (3-coordinated tiling of the torus)            */
+  int32_t max_cell_vertices; /* S: row stride of cell_vertices, 4..32, multiple of 4            */
+  int32_t sort_every;        /* 0 = never; k > 0 = Hilbert re-sort after every k-th step        */
+  double Lx, Ly;             /* periodic box (R13); every cell must stay narrower than L/2      */
+  double KA, KP, A0, P0;     /* Eq. A1: E = sum KA (A-A0)^2 + KP (P-P0)^2        */
+  double v0, Dr, mu, dt;     /* Eq. 4, director noise variance 2 Dr */
+  double l_c;                /* T1 threshold: edges with length < l_c are flipped (R9)          */
+  uint64_t seed;             /* Philox4x32-10 key (R16)                                         */
+  uint64_t step0;            /* step counter at creation; resume from a saved state is exact    */
+  int32_t device;            /* CUDA device ordinal                                             */
+  int32_t flags;             /* AVM_FLAG_*                                                      */
+} avm_params;
+
+enum {
+  AVM_FLAG_SORT_AT_CREATE = 1, /* Hilbert-order cells and vertices once inside avm_create       */
+  AVM_FLAG_NO_GRAPH = 2        /* launch kernels directly instead of through CUDA graphs        */
+};
+
+/* Counters since creation.  error is a sticky bit set: 1 = a non-finite position was produced,
+ * 2 = a flip was suppressed because a cell row would exceed S. */
+typedef struct avm_stats {
+  int64_t step;             /* current step counter (step0 + steps taken)                       */
+  int64_t t1_short;         /* edges found shorter than l_c                                      */
+  int64_t t1_candidates;    /* of those, eligible (R10)                                          */
+  int64_t t1_flips;         /* candidates that won the conflict rule (R11) and were flipped      */
+  int64_t t1_blocked;       /* candidates blocked by a smaller key sharing a cell                */
+  int64_t overflow_rejects; /* short edges rejected because an end cell is already at S          */
+  int64_t error;            /* sticky error bits                                                 */
+  int64_t n_sorts;          /* Hilbert re-sorts done                                             */
+  int64_t kernel_launches;  /* kernels this library has launched since creation                  */
+} avm_stats;
+
+enum {
+  AVM_OK = 0,
+  AVM_EINVAL = -1,        /* NULL / out-of-range argument, V != 2N, bad stride                   */
+  AVM_EWORKSPACE = -2,    /* workspace too small or misaligned                                   */
+  AVM_EINCONSISTENT = -3, /* the topology lists contradict each other or a row is out of range   */
+  AVM_ECUDA = -4,         /* a CUDA call failed; avm_last_cuda_error() has the text              */
+  AVM_ENOMEM = -5
+};
+
+/* Bytes of device workspace avm_create needs for these parameters (0 on invalid parameters). */
+size_t avm_workspace_bytes(const avm_params* params);
+
+/* Build a simulation from an initial state (PAPER.md:66 lists; theta: PAPER.md:50).
+ * Inputs are copied into the workspace; the caller keeps ownership of its arrays.  The lists are
+ * validated on the device (ranges, slot convention of vertex_cell_neighbors against the rows);
+ * avm_create synchronises the stream once to report AVM_EINCONSISTENT.
+ * avm_create: all array arguments are device pointers.  avm_create_host: host pointers. */
+int avm_create(const avm_params* params, const double* pos_xy, const int32_t* cell_vertex_num,
+               const int32_t* cell_vertices, const int32_t* vertex_neighbors,
+               const int32_t* vertex_cell_neighbors, const double* theta, void* workspace,
+               size_t workspace_bytes, void* cuda_stream, avm_sim** out);
+int avm_create_host(const avm_params* params, const double* pos_xy, const int32_t* cell_vertex_num,
+                    const int32_t* cell_vertices, const int32_t* vertex_neighbors,
+                    const int32_t* vertex_cell_neighbors, const double* theta, void* workspace,
+                    size_t workspace_bytes, void* cuda_stream, avm_sim** out);
+
+/* Advance n_steps timesteps (order R6).  Asynchronous: only enqueues
+ * kernels (and, every sort_every steps, the Hilbert re-sort) on the stream.
+ * Conditions arising inside a step set avm_stats.error; they do not stop the run. */
+int avm_step(avm_sim* sim, int64_t n_steps);
+
+/* Same steps as avm_step, but every kernel of the step is bracketed by CUDA events on the stream
+ * and the call synchronises after each step: ms_per_kernel (HOST pointer, [AVM_K_COUNT]) receives
+ * the summed device time of each kernel class over the n_steps.  Measurement aid for the roofline
+ * figures of bench.py; not the timed path. */
+enum { AVM_K_FORCE_MOVE = 0, AVM_K_CELL_UPDATE = 1, AVM_K_T1_MARK = 2, AVM_K_T1_FLIP = 3, AVM_K_T1_RESET = 4,
+       AVM_K_COUNT = 5 };
+int avm_step_profile(avm_sim* sim, int64_t n_steps, double* ms_per_kernel);
+
+/* Geometry + forces of the current state, nothing modified (App. A.1, Eq. A1-A5):
+ * force_xy [V][2] = -dE/dh_v, area_perim [N][2] = (A_c, P_c), user order.  Asynchronous for the
+ * device variant; the host variant returns after the copies have completed. */
+int avm_compute_forces(avm_sim* sim, double* force_xy, double* area_perim);
+int avm_compute_forces_host(avm_sim* sim, double* force_xy, double* area_perim);
+
+/* Total energy of the current state, Eq. 1 / A1, summed on the device in a
+ * fixed order (deterministic).  energy is a HOST pointer; synchronises the stream. */
+int avm_energy(avm_sim* sim, double* energy);
+
+/* Copy the current state out in user order.  stats (HOST pointer, may be NULL) receives the
+ * counters; when it is non-NULL, or for the host variant, the call synchronises the stream. */
+int avm_get_state(avm_sim* sim, double* pos_xy, int32_t* cell_vertex_num, int32_t* cell_vertices,
+                  int32_t* vertex_neighbors, int32_t* vertex_cell_neighbors, double* theta,
+                  avm_stats* stats);
+int avm_get_state_host(avm_sim* sim, double* pos_xy, int32_t* cell_vertex_num, int32_t* cell_vertices,
+                       int32_t* vertex_neighbors, int32_t* vertex_cell_neighbors, double* theta,
+                       avm_stats* stats);
+
+/* Test hooks, not on the timed path.
+ * avm_debug_t1: T1 detection + conflict resolution (R9-R11) on the current state WITHOUT
+ *   flipping.  Writes up to `capacity` (tag_min, tag_max) pairs of candidates and of winners to
+ *   the HOST arrays cand_pairs / winner_pairs ([capacity][2] int32, unsorted) and the full counts
+ *   to *n_cand / *n_win.  Synchronises.
+ * avm_t1_pass: one T1 pass (detect, resolve, flip) on the current state, no move.
+ * avm_set_positions: overwrite the vertex positions (device pointer, user order) and refresh
+ *   the cached cell geometry.
+ * avm_resort: force a Hilbert re-sort now. */
+int avm_debug_t1(avm_sim* sim, int32_t* cand_pairs, int64_t* n_cand, int32_t* winner_pairs,
+                 int64_t* n_win, int64_t capacity);
+int avm_t1_pass(avm_sim* sim);
+int avm_set_positions(avm_sim* sim, const double* pos_xy);
+int avm_resort(avm_sim* sim);
+
+/* Raw Philox4x32-10 words (R16) for (seed, step, cell0 .. cell0+n-1), computed by the same device
+ * function the director update uses: out_words is a DEVICE pointer to [n][4] uint32.  Test hook
+ * for the bit-exact comparison with the oracle and with cuRAND. */
+int avm_philox_words(avm_sim* sim, uint64_t seed, uint64_t step, uint64_t cell0, int64_t n,
+                     uint32_t* out_words);
+
+/* Hilbert index (R18) of grid cells (ix[i], iy[i]) on a 2^m x 2^m grid, 1 <= m <= 16, computed by
+ * the device function the re-sort uses (ix, iy, out: DEVICE pointers to [n] uint32), and the same
+ * function compiled for the host (scalar; needs no GPU).  Test hooks. */
+int avm_hilbert_index(avm_sim* sim, int32_t m, int64_t n, const uint32_t* ix, const uint32_t* iy, uint32_t* out);
+uint32_t avm_hilbert_index_host(int32_t m, uint32_t ix, uint32_t iy);
+
+void avm_destroy(avm_sim* sim);
+const char* avm_strerror(int code);
+const char* avm_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AVM_H_ */

@@ -1,0 +1,277 @@
+"""Thin Python binding of the C ABI in ``include/avm.h`` (argument marshalling only).
+
+Every step of the hot path runs inside ``libavm_b200.so``; this module only
+  * loads the library (and fails loudly if it has not been built — there is no fallback),
+  * allocates device memory with PyTorch and passes ``data_ptr()`` / the current CUDA stream,
+  * mirrors the entry points one to one: ``avm_create``, ``avm_step``, ``avm_get_state``,
+    ``avm_compute_forces`` (+ the ``*_host`` twins and the test hooks).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libavm_b200.so")
+
+# every symbol include/avm.h declares (tests check that the library exports all of them)
+ABI_SYMBOLS = [
+    "avm_workspace_bytes", "avm_create", "avm_create_host", "avm_step", "avm_step_profile", "avm_compute_forces",
+    "avm_compute_forces_host", "avm_energy", "avm_get_state", "avm_get_state_host", "avm_debug_t1",
+    "avm_t1_pass", "avm_set_positions", "avm_resort", "avm_philox_words", "avm_hilbert_index",
+    "avm_hilbert_index_host", "avm_destroy", "avm_strerror", "avm_last_cuda_error",
+]
+
+AVM_FLAG_SORT_AT_CREATE = 1
+AVM_FLAG_NO_GRAPH = 2
+
+
+class AvmParams(ctypes.Structure):
+    _fields_ = [("n_cells", ctypes.c_int32), ("n_vertices", ctypes.c_int32),
+                ("max_cell_vertices", ctypes.c_int32), ("sort_every", ctypes.c_int32),
+                ("Lx", ctypes.c_double), ("Ly", ctypes.c_double),
+                ("KA", ctypes.c_double), ("KP", ctypes.c_double), ("A0", ctypes.c_double), ("P0", ctypes.c_double),
+                ("v0", ctypes.c_double), ("Dr", ctypes.c_double), ("mu", ctypes.c_double), ("dt", ctypes.c_double),
+                ("l_c", ctypes.c_double),
+                ("seed", ctypes.c_uint64), ("step0", ctypes.c_uint64),
+                ("device", ctypes.c_int32), ("flags", ctypes.c_int32)]
+
+
+class AvmStats(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int64) for n in
+                ("step", "t1_short", "t1_candidates", "t1_flips", "t1_blocked", "overflow_rejects", "error",
+                 "n_sorts", "kernel_launches")]
+
+    def as_dict(self):
+        return {n: int(getattr(self, n)) for n, _ in self._fields_}
+
+
+class AvmError(RuntimeError):
+    pass
+
+
+def _load() -> ctypes.CDLL:
+    if not os.path.exists(LIB_PATH):
+        raise AvmError(
+            f"{LIB_PATH} is missing: build the CUDA library first (python -m paper_1702_02939_b200.build). "
+            "There is no CPU fallback.")
+    lib = ctypes.CDLL(LIB_PATH)
+    p, i64, u64, i32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_uint64, ctypes.c_int32
+    PP = ctypes.POINTER(AvmParams)
+    lib.avm_workspace_bytes.restype = ctypes.c_size_t
+    lib.avm_workspace_bytes.argtypes = [PP]
+    for name in ("avm_create", "avm_create_host"):
+        f = getattr(lib, name)
+        f.restype = ctypes.c_int
+        f.argtypes = [PP, p, p, p, p, p, p, p, ctypes.c_size_t, p, ctypes.POINTER(p)]
+    lib.avm_step.argtypes = [p, i64]
+    lib.avm_step_profile.argtypes = [p, i64, p]
+    lib.avm_compute_forces.argtypes = [p, p, p]
+    lib.avm_compute_forces_host.argtypes = [p, p, p]
+    lib.avm_energy.argtypes = [p, ctypes.POINTER(ctypes.c_double)]
+    for name in ("avm_get_state", "avm_get_state_host"):
+        getattr(lib, name).argtypes = [p, p, p, p, p, p, p, ctypes.POINTER(AvmStats)]
+    lib.avm_debug_t1.argtypes = [p, p, ctypes.POINTER(i64), p, ctypes.POINTER(i64), i64]
+    lib.avm_t1_pass.argtypes = [p]
+    lib.avm_set_positions.argtypes = [p, p]
+    lib.avm_resort.argtypes = [p]
+    lib.avm_philox_words.argtypes = [p, u64, u64, u64, i64, p]
+    lib.avm_hilbert_index.argtypes = [p, i32, i64, p, p, p]
+    lib.avm_hilbert_index_host.argtypes = [i32, ctypes.c_uint32, ctypes.c_uint32]
+    lib.avm_hilbert_index_host.restype = ctypes.c_uint32
+    lib.avm_destroy.argtypes = [p]
+    lib.avm_destroy.restype = None
+    lib.avm_strerror.argtypes = [ctypes.c_int]
+    lib.avm_strerror.restype = ctypes.c_char_p
+    lib.avm_last_cuda_error.restype = ctypes.c_char_p
+    return lib
+
+
+lib = _load()
+
+
+def _check(rc: int) -> None:
+    if rc != 0:
+        msg = lib.avm_strerror(rc).decode()
+        if rc == -4:
+            msg += ": " + lib.avm_last_cuda_error().decode()
+        raise AvmError(f"avm error {rc}: {msg}")
+
+
+def hilbert_index_host(m: int, ix: int, iy: int) -> int:
+    return int(lib.avm_hilbert_index_host(m, ix, iy))
+
+
+def make_params(N: int, S: int, *, Lx, Ly, KA=1.0, KP=1.0, A0=1.0, P0=3.8, v0=0.0, Dr=0.0, mu=1.0, dt=0.01,
+                l_c=0.0, seed=0, step0=0, sort_every=0, sort_at_create=False, device=0, flags=0,
+                **_ignored) -> AvmParams:
+    if sort_at_create:
+        flags |= AVM_FLAG_SORT_AT_CREATE
+    return AvmParams(N, 2 * N, S, sort_every, Lx, Ly, KA, KP, A0, P0, v0, Dr, mu, dt, l_c, seed, step0, device, flags)
+
+
+def _dptr(t) -> Optional[int]:
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def _hptr(a: Optional[np.ndarray]):
+    return None if a is None else ctypes.c_void_p(a.ctypes.data)
+
+
+class AvmSim:
+    """One simulation living on a CUDA device.  Tensors in/out are torch CUDA tensors (device
+    entry points) or numpy arrays (``*_host`` entry points), always in user order."""
+
+    def __init__(self, tiling, params: AvmParams, host: bool = False):
+        import torch
+        self.torch = torch
+        self.params = params
+        self.N, self.V, self.S = params.n_cells, params.n_vertices, params.max_cell_vertices
+        self.device = torch.device("cuda", params.device)
+        nbytes = lib.avm_workspace_bytes(ctypes.byref(params))
+        if nbytes == 0:
+            raise AvmError("avm_workspace_bytes rejected the parameters")
+        self.workspace_bytes = int(nbytes)
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        assert self.workspace.data_ptr() % 256 == 0
+        self.stream = torch.cuda.current_stream(self.device)
+        self._h = ctypes.c_void_p()
+        arrays = [np.ascontiguousarray(tiling.pos, dtype=np.float64),
+                  np.ascontiguousarray(tiling.cell_vertex_num, dtype=np.int32),
+                  np.ascontiguousarray(tiling.cell_vertices, dtype=np.int32),
+                  np.ascontiguousarray(tiling.vertex_neighbors, dtype=np.int32),
+                  np.ascontiguousarray(tiling.vertex_cell_neighbors, dtype=np.int32),
+                  np.ascontiguousarray(tiling.theta, dtype=np.float64)]
+        assert arrays[2].shape == (self.N, self.S) and arrays[0].shape == (self.V, 2)
+        if host:
+            self._inputs = arrays
+            ptrs = [_hptr(a) for a in arrays]
+            fn = lib.avm_create_host
+        else:
+            self._inputs = [torch.from_numpy(a).to(self.device) for a in arrays]
+            ptrs = [_dptr(t) for t in self._inputs]
+            fn = lib.avm_create
+        _check(fn(ctypes.byref(params), *ptrs, ctypes.c_void_p(self.workspace.data_ptr()),
+                  self.workspace_bytes, ctypes.c_void_p(self.stream.cuda_stream), ctypes.byref(self._h)))
+        self._inputs = None
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            self.torch.cuda.synchronize(self.device)
+            lib.avm_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- hot path ------------------------------------------------------------------------------
+    def step(self, n: int = 1) -> None:
+        _check(lib.avm_step(self._h, n))
+
+    KERNEL_NAMES = ("force_move", "cell_update", "t1_mark", "t1_flip", "t1_reset")
+
+    def step_profile(self, n: int) -> dict:
+        """n steps with every kernel bracketed by CUDA events; summed device ms per kernel class."""
+        ms = (ctypes.c_double * len(self.KERNEL_NAMES))()
+        _check(lib.avm_step_profile(self._h, n, ms))
+        return dict(zip(self.KERNEL_NAMES, list(ms)))
+
+    def compute_forces(self):
+        t = self.torch
+        F = t.empty((self.V, 2), dtype=t.float64, device=self.device)
+        ap = t.empty((self.N, 2), dtype=t.float64, device=self.device)
+        _check(lib.avm_compute_forces(self._h, _dptr(F), _dptr(ap)))
+        return F, ap
+
+    def compute_forces_host(self):
+        F = np.empty((self.V, 2), dtype=np.float64)
+        ap = np.empty((self.N, 2), dtype=np.float64)
+        _check(lib.avm_compute_forces_host(self._h, _hptr(F), _hptr(ap)))
+        return F, ap
+
+    def energy(self) -> float:
+        e = ctypes.c_double(0.0)
+        _check(lib.avm_energy(self._h, ctypes.byref(e)))
+        return e.value
+
+    def get_state(self, stats: bool = True) -> dict:
+        t = self.torch
+        pos = t.empty((self.V, 2), dtype=t.float64, device=self.device)
+        cvn = t.empty(self.N, dtype=t.int32, device=self.device)
+        cv = t.empty((self.N, self.S), dtype=t.int32, device=self.device)
+        vn = t.empty((self.V, 3), dtype=t.int32, device=self.device)
+        vc = t.empty((self.V, 3), dtype=t.int32, device=self.device)
+        th = t.empty(self.N, dtype=t.float64, device=self.device)
+        st = AvmStats()
+        _check(lib.avm_get_state(self._h, _dptr(pos), _dptr(cvn), _dptr(cv), _dptr(vn), _dptr(vc), _dptr(th),
+                                 ctypes.byref(st) if stats else None))
+        return dict(pos=pos, cell_vertex_num=cvn, cell_vertices=cv, vertex_neighbors=vn,
+                    vertex_cell_neighbors=vc, theta=th, stats=st.as_dict() if stats else None)
+
+    def get_state_host(self, out: Optional[dict] = None) -> dict:
+        if out is None:
+            out = dict(pos=np.empty((self.V, 2), dtype=np.float64), cell_vertex_num=np.empty(self.N, dtype=np.int32),
+                       cell_vertices=np.empty((self.N, self.S), dtype=np.int32),
+                       vertex_neighbors=np.empty((self.V, 3), dtype=np.int32),
+                       vertex_cell_neighbors=np.empty((self.V, 3), dtype=np.int32),
+                       theta=np.empty(self.N, dtype=np.float64))
+        st = AvmStats()
+        _check(lib.avm_get_state_host(self._h, _hptr(out.get("pos")), _hptr(out.get("cell_vertex_num")),
+                                      _hptr(out.get("cell_vertices")), _hptr(out.get("vertex_neighbors")),
+                                      _hptr(out.get("vertex_cell_neighbors")), _hptr(out.get("theta")),
+                                      ctypes.byref(st)))
+        out["stats"] = st.as_dict()
+        return out
+
+    def stats(self) -> dict:
+        st = AvmStats()
+        _check(lib.avm_get_state(self._h, None, None, None, None, None, None, ctypes.byref(st)))
+        return st.as_dict()
+
+    # ---- test hooks ----------------------------------------------------------------------------
+    def debug_t1(self):
+        cap = 3 * self.N
+        cand = np.empty((cap, 2), dtype=np.int32)
+        win = np.empty((cap, 2), dtype=np.int32)
+        nc, nw = ctypes.c_int64(0), ctypes.c_int64(0)
+        _check(lib.avm_debug_t1(self._h, _hptr(cand), ctypes.byref(nc), _hptr(win), ctypes.byref(nw), cap))
+        return cand[:nc.value].copy(), win[:nw.value].copy()
+
+    def t1_pass(self) -> None:
+        _check(lib.avm_t1_pass(self._h))
+
+    def set_positions(self, pos) -> None:
+        t = self.torch
+        if isinstance(pos, np.ndarray):
+            pos = t.from_numpy(np.ascontiguousarray(pos, dtype=np.float64)).to(self.device)
+        assert pos.shape == (self.V, 2) and pos.dtype == t.float64 and pos.is_contiguous()
+        _check(lib.avm_set_positions(self._h, _dptr(pos)))
+        t.cuda.current_stream(self.device).synchronize()   # keep `pos` alive until consumed
+
+    def resort(self) -> None:
+        _check(lib.avm_resort(self._h))
+
+    def philox_words(self, seed: int, step: int, cell0: int, n: int):
+        t = self.torch
+        out = t.empty((n, 4), dtype=t.int32, device=self.device)
+        _check(lib.avm_philox_words(self._h, seed, step, cell0, n, _dptr(out)))
+        return out.cpu().numpy().view(np.uint32)
+
+    def hilbert_index(self, m: int, ix: np.ndarray, iy: np.ndarray) -> np.ndarray:
+        t = self.torch
+        dx = t.from_numpy(ix.astype(np.int64)).to(self.device).to(t.int32)
+        dy = t.from_numpy(iy.astype(np.int64)).to(self.device).to(t.int32)
+        out = t.empty(ix.shape[0], dtype=t.int32, device=self.device)
+        _check(lib.avm_hilbert_index(self._h, m, ix.shape[0], _dptr(dx), _dptr(dy), _dptr(out)))
+        return out.cpu().numpy().view(np.uint32)
+
+
+def from_tiling(tiling, host: bool = False, **params) -> AvmSim:
+    p = make_params(tiling.N, tiling.S, **dict(params, Lx=tiling.Lx, Ly=tiling.Ly))
+    return AvmSim(tiling, p, host=host)

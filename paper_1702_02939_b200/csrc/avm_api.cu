@@ -1,0 +1,520 @@
+// avm_api.cu — the C ABI of include/avm.h: workspace carve-up, creation/validation, the step
+// loop, state export in user order.  Host logic only enqueues work; the arithmetic of the hot
+// path lives in avm_step.cu / avm_sort.cu.
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include "avm_internal.cuh"
+
+namespace avm {
+int launch_hilbert_index(int m, long long n, const unsigned int* ix, const unsigned int* iy, unsigned int* out, cudaStream_t s);
+int hilbert_bits(const Consts& k);
+unsigned int hilbert_index_host(unsigned int x, unsigned int y, int m);
+}
+
+using namespace avm;
+
+namespace {
+
+thread_local std::string g_cuda_error;
+
+#define AVM_CUDA(call)                                                                      \
+  do {                                                                                      \
+    cudaError_t e_ = (call);                                                                \
+    if (e_ != cudaSuccess) {                                                                \
+      g_cuda_error = std::string(#call) + ": " + cudaGetErrorString(e_);                    \
+      return AVM_ECUDA;                                                                     \
+    }                                                                                       \
+  } while (0)
+
+inline size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+struct BufferSet {
+  int *vn, *vc, *cv, *cvn, *vtag, *ctag;
+  double* theta;
+  CellRec* rec;
+};
+
+struct Layout {
+  size_t pos[2], vn[2], vc[2], cv[2], cvn[2], theta[2], rec[2], vtag[2], ctag[2];
+  size_t minkey, short_list, cand, ctr, ap, epart, key[2], val[2], hist, newidx_v, newidx_c, order_v, order_c;
+  size_t total;
+};
+
+Layout make_layout(const avm_params& p) {
+  Layout L;
+  const size_t N = (size_t)p.n_cells, V = (size_t)p.n_vertices, S = (size_t)p.max_cell_vertices;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
+  for (int i = 0; i < 2; ++i) L.pos[i] = take(16 * V);
+  for (int i = 0; i < 2; ++i) {
+    L.vn[i] = take(12 * V); L.vc[i] = take(12 * V); L.cv[i] = take(4 * N * S); L.cvn[i] = take(4 * N);
+    L.theta[i] = take(8 * N); L.rec[i] = take(32 * N); L.vtag[i] = take(4 * V); L.ctag[i] = take(4 * N);
+  }
+  L.minkey = take(8 * N);
+  L.short_list = take(8 * 3 * N);
+  L.cand = take(sizeof(Cand) * 3 * N);
+  L.ctr = take(sizeof(Counters));
+  L.ap = take(16 * N);
+  L.epart = take(8 * 1024);
+  for (int i = 0; i < 2; ++i) { L.key[i] = take(4 * V); L.val[i] = take(4 * V); }
+  L.hist = take(4 * sort_hist_entries((int)V));
+  L.newidx_v = take(4 * V); L.newidx_c = take(4 * N); L.order_v = take(4 * V); L.order_c = take(4 * N);
+  L.total = off;
+  return L;
+}
+
+bool params_ok(const avm_params* p) {
+  if (!p) return false;
+  if (p->n_cells < 4 || p->n_cells > (1 << 29)) return false;
+  if (p->n_vertices != 2 * p->n_cells) return false;
+  if (p->max_cell_vertices < 4 || p->max_cell_vertices > 32 || (p->max_cell_vertices & 3)) return false;
+  if (!(p->Lx > 0.0) || !(p->Ly > 0.0) || !(p->dt >= 0.0) || !(p->l_c >= 0.0) || !(p->Dr >= 0.0)) return false;
+  if (p->sort_every < 0) return false;
+  return true;
+}
+
+}  // namespace
+
+struct avm_sim {
+  avm_params p;
+  Consts k;
+  cudaStream_t stream;
+  char* ws;
+  Layout L;
+  double2* pos[2];
+  BufferSet set[2];
+  unsigned long long* minkey;
+  int2* short_list;
+  Cand* cand;
+  Counters* ctr;
+  double2* ap;
+  double* epart;
+  SortScratch sc;
+  int cur_pos, cur_set;
+  unsigned long long step;
+  long long n_sorts, launches;
+
+  Dev dev() const {
+    Dev d;
+    d.pos = pos[cur_pos]; d.pos_next = pos[1 - cur_pos];
+    const BufferSet& b = set[cur_set];
+    d.vn = b.vn; d.vc = b.vc; d.cv = b.cv; d.cvn = b.cvn; d.theta = b.theta; d.rec = b.rec;
+    d.vtag = b.vtag; d.ctag = b.ctag;
+    d.minkey = minkey; d.short_list = short_list; d.cand = cand; d.ctr = ctr;
+    return d;
+  }
+  Dev dev_alt() const {   // the other buffer set, target of a re-sort / staging area
+    Dev d = dev();
+    const BufferSet& b = set[1 - cur_set];
+    d.pos = pos[1 - cur_pos]; d.pos_next = pos[cur_pos];
+    d.vn = b.vn; d.vc = b.vc; d.cv = b.cv; d.cvn = b.cvn; d.theta = b.theta; d.rec = b.rec;
+    d.vtag = b.vtag; d.ctag = b.ctag;
+    return d;
+  }
+};
+
+namespace {
+
+// ---- creation-time kernels ---------------------------------------------------------------------
+__global__ void init_kernel(const Dev d, const Consts k) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < k.V) d.vtag[i] = i;
+  if (i < k.N) {
+    d.ctag[i] = i;
+    d.minkey[i] = ~0ull;
+    int n = d.cvn[i];
+    n = n < 0 ? 0 : (n > k.S ? k.S : n);
+    for (int j = n; j < k.S; ++j) d.cv[(size_t)i * k.S + j] = -1;   // normalise the padding
+  }
+}
+
+// error bit 4: lists out of range or mutually inconsistent (slot convention, R12)
+__global__ void validate_kernel(const Dev d, const Consts k) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  bool bad = false;
+  if (i < k.N) {
+    const int n = d.cvn[i];
+    if (n < 3 || n > k.S) bad = true;
+    else
+      for (int j = 0; j < n; ++j) {
+        const int v = d.cv[(size_t)i * k.S + j];
+        if (v < 0 || v >= k.V) { bad = true; break; }
+        const int c0 = d.vc[3 * v], c1 = d.vc[3 * v + 1], c2 = d.vc[3 * v + 2];
+        if (c0 != i && c1 != i && c2 != i) bad = true;
+      }
+  }
+  if (i < k.V) {
+    const double2 h = d.pos[i];
+    if (!(h.x >= 0.0 && h.x < k.Lx && h.y >= 0.0 && h.y < k.Ly)) bad = true;
+    for (int s = 0; s < 3 && !bad; ++s) {
+      const int w = d.vn[3 * i + s], c = d.vc[3 * i + s], wn = d.vn[3 * i + (s + 1) % 3];
+      if (w < 0 || w >= k.V || c < 0 || c >= k.N || w == i) { bad = true; break; }
+      const int n = d.cvn[c];
+      if (n < 3 || n > k.S) { bad = true; break; }
+      const int* row = d.cv + (size_t)c * k.S;
+      int j = -1;
+      for (int t = 0; t < n; ++t) if (row[t] == i) j = t;
+      if (j < 0) { bad = true; break; }
+      if (row[(j + 1) % n] != w || row[(j + n - 1) % n] != wn) bad = true;
+    }
+  }
+  if (bad) atomicOr((unsigned long long*)&d.ctr->error, 4ull);
+}
+
+// ---- export in user order ------------------------------------------------------------------------
+__global__ void export_vertices_kernel(const Dev d, const Consts k, double* pos, int* vn, int* vc) {
+  const int v = blockIdx.x * blockDim.x + threadIdx.x;
+  if (v >= k.V) return;
+  const int t = d.vtag[v];
+  if (pos) { const double2 h = d.pos[v]; pos[2 * t] = h.x; pos[2 * t + 1] = h.y; }
+  for (int s = 0; s < 3; ++s) {
+    if (vn) vn[3 * t + s] = d.vtag[d.vn[3 * v + s]];
+    if (vc) vc[3 * t + s] = d.ctag[d.vc[3 * v + s]];
+  }
+}
+__global__ void export_cells_kernel(const Dev d, const Consts k, int* cvn, int* cv, double* theta) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= k.N) return;
+  const int t = d.ctag[c];
+  const int n = d.cvn[c];
+  if (cvn) cvn[t] = n;
+  if (theta) theta[t] = d.theta[c];
+  if (cv)
+    for (int j = 0; j < k.S; ++j) cv[(size_t)t * k.S + j] = j < n ? d.vtag[d.cv[(size_t)c * k.S + j]] : -1;
+}
+__global__ void import_positions_kernel(const Dev d, const Consts k, const double* pos) {
+  const int v = blockIdx.x * blockDim.x + threadIdx.x;
+  if (v >= k.V) return;
+  const int t = d.vtag[v];
+  d.pos[v] = make_double2(pos[2 * t], pos[2 * t + 1]);
+}
+
+inline int cdiv(long long a, int b) { return (int)((a + b - 1) / b); }
+
+int do_sort(avm_sim* s) {
+  const Dev a = s->dev(), b = s->dev_alt();
+  s->launches += launch_hilbert_sort(a, b, s->k, s->sc, s->stream);
+  s->cur_pos = 1 - s->cur_pos;
+  s->cur_set = 1 - s->cur_set;
+  ++s->n_sorts;
+  return AVM_OK;
+}
+
+int read_counters(avm_sim* s, Counters* out) {
+  AVM_CUDA(cudaMemcpyAsync(out, s->ctr, sizeof(Counters), cudaMemcpyDeviceToHost, s->stream));
+  AVM_CUDA(cudaStreamSynchronize(s->stream));
+  return AVM_OK;
+}
+
+int create_common(const avm_params* params, const double* pos_xy, const int32_t* cvn, const int32_t* cv,
+                  const int32_t* vn, const int32_t* vc, const double* theta, void* workspace,
+                  size_t workspace_bytes, void* cuda_stream, avm_sim** out, bool host_inputs) {
+  if (!out) return AVM_EINVAL;
+  *out = nullptr;
+  if (!params_ok(params) || !pos_xy || !cvn || !cv || !vn || !vc || !theta || !workspace) return AVM_EINVAL;
+  const Layout L = make_layout(*params);
+  if (workspace_bytes < L.total || ((uintptr_t)workspace & 255)) return AVM_EWORKSPACE;
+  AVM_CUDA(cudaSetDevice(params->device));
+  avm_sim* s = new (std::nothrow) avm_sim();
+  if (!s) return AVM_ENOMEM;
+  s->p = *params;
+  s->stream = (cudaStream_t)cuda_stream;
+  s->ws = (char*)workspace;
+  s->L = L;
+  const int N = params->n_cells, V = params->n_vertices, S = params->max_cell_vertices;
+  Consts& k = s->k;
+  k.N = N; k.V = V; k.S = S;
+  k.Lx = params->Lx; k.Ly = params->Ly; k.hLx = 0.5 * params->Lx; k.hLy = 0.5 * params->Ly;
+  k.KA = params->KA; k.KP = params->KP; k.KA2 = 2.0 * params->KA; k.KP2 = 2.0 * params->KP;
+  k.A0 = params->A0; k.P0 = params->P0;
+  k.v0_3 = params->v0 / 3.0; k.mu = params->mu; k.dt = params->dt;
+  k.amp = sqrt(2.0 * params->Dr * params->dt);
+  k.lc = params->l_c; k.lc2 = params->l_c * params->l_c;
+  k.seed = params->seed;
+  char* w = s->ws;
+  for (int i = 0; i < 2; ++i) {
+    s->pos[i] = (double2*)(w + L.pos[i]);
+    BufferSet& b = s->set[i];
+    b.vn = (int*)(w + L.vn[i]); b.vc = (int*)(w + L.vc[i]); b.cv = (int*)(w + L.cv[i]);
+    b.cvn = (int*)(w + L.cvn[i]); b.theta = (double*)(w + L.theta[i]); b.rec = (CellRec*)(w + L.rec[i]);
+    b.vtag = (int*)(w + L.vtag[i]); b.ctag = (int*)(w + L.ctag[i]);
+    s->sc.key[i] = (unsigned int*)(w + L.key[i]); s->sc.val[i] = (int*)(w + L.val[i]);
+  }
+  s->minkey = (unsigned long long*)(w + L.minkey);
+  s->short_list = (int2*)(w + L.short_list);
+  s->cand = (Cand*)(w + L.cand);
+  s->ctr = (Counters*)(w + L.ctr);
+  s->ap = (double2*)(w + L.ap);
+  s->epart = (double*)(w + L.epart);
+  s->sc.hist = (unsigned int*)(w + L.hist);
+  s->sc.newidx_v = (int*)(w + L.newidx_v); s->sc.newidx_c = (int*)(w + L.newidx_c);
+  s->sc.order_v = (int*)(w + L.order_v); s->sc.order_c = (int*)(w + L.order_c);
+  s->cur_pos = 0; s->cur_set = 0;
+  s->step = params->step0;
+  s->n_sorts = 0; s->launches = 0;
+
+  cudaStream_t st = s->stream;
+  const cudaMemcpyKind kind = host_inputs ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+  const BufferSet& b = s->set[0];
+  auto fail = [&](int code) { delete s; return code; };
+#define AVM_CUDA_F(call)                                                                    \
+  do {                                                                                      \
+    cudaError_t e_ = (call);                                                                \
+    if (e_ != cudaSuccess) {                                                                \
+      g_cuda_error = std::string(#call) + ": " + cudaGetErrorString(e_);                    \
+      return fail(AVM_ECUDA);                                                               \
+    }                                                                                       \
+  } while (0)
+  AVM_CUDA_F(cudaMemcpyAsync(s->pos[0], pos_xy, 16 * (size_t)V, kind, st));
+  AVM_CUDA_F(cudaMemcpyAsync(b.vn, vn, 12 * (size_t)V, kind, st));
+  AVM_CUDA_F(cudaMemcpyAsync(b.vc, vc, 12 * (size_t)V, kind, st));
+  AVM_CUDA_F(cudaMemcpyAsync(b.cv, cv, 4 * (size_t)N * S, kind, st));
+  AVM_CUDA_F(cudaMemcpyAsync(b.cvn, cvn, 4 * (size_t)N, kind, st));
+  AVM_CUDA_F(cudaMemcpyAsync(b.theta, theta, 8 * (size_t)N, kind, st));
+  AVM_CUDA_F(cudaMemsetAsync(s->ctr, 0, sizeof(Counters), st));
+  const Dev d = s->dev();
+  validate_kernel<<<cdiv(V, 256), 256, 0, st>>>(d, k);
+  ++s->launches;
+  Counters c;
+  AVM_CUDA_F(cudaMemcpyAsync(&c, s->ctr, sizeof(Counters), cudaMemcpyDeviceToHost, st));
+  AVM_CUDA_F(cudaStreamSynchronize(st));
+  AVM_CUDA_F(cudaGetLastError());
+  if (c.error & 4) return fail(AVM_EINCONSISTENT);
+  init_kernel<<<cdiv(V, 256), 256, 0, st>>>(d, k);
+  ++s->launches;
+  s->launches += launch_refresh_cells(d, k, st);
+  if (params->flags & AVM_FLAG_SORT_AT_CREATE) do_sort(s);
+  AVM_CUDA_F(cudaGetLastError());
+#undef AVM_CUDA_F
+  *out = s;
+  return AVM_OK;
+}
+
+int get_state_common(avm_sim* s, double* pos_xy, int32_t* cvn, int32_t* cv, int32_t* vn, int32_t* vc,
+                     double* theta, avm_stats* stats, bool host_outputs) {
+  if (!s) return AVM_EINVAL;
+  const Consts& k = s->k;
+  const Dev d = s->dev();
+  cudaStream_t st = s->stream;
+  if (!host_outputs) {
+    if (pos_xy || vn || vc) { export_vertices_kernel<<<cdiv(k.V, 256), 256, 0, st>>>(d, k, pos_xy, vn, vc); ++s->launches; }
+    if (cvn || cv || theta) { export_cells_kernel<<<cdiv(k.N, 256), 256, 0, st>>>(d, k, cvn, cv, theta); ++s->launches; }
+  } else {
+    // stage in the idle buffers (ping-pong partner of pos, alternate buffer set), then copy out
+    const Dev a = s->dev_alt();
+    double* spos = (double*)a.pos;
+    if (pos_xy || vn || vc) {
+      export_vertices_kernel<<<cdiv(k.V, 256), 256, 0, st>>>(d, k, pos_xy ? spos : nullptr, vn ? a.vn : nullptr, vc ? a.vc : nullptr);
+      ++s->launches;
+    }
+    if (cvn || cv || theta) {
+      export_cells_kernel<<<cdiv(k.N, 256), 256, 0, st>>>(d, k, cvn ? a.cvn : nullptr, cv ? a.cv : nullptr, theta ? a.theta : nullptr);
+      ++s->launches;
+    }
+    if (pos_xy) AVM_CUDA(cudaMemcpyAsync(pos_xy, spos, 16 * (size_t)k.V, cudaMemcpyDeviceToHost, st));
+    if (vn) AVM_CUDA(cudaMemcpyAsync(vn, a.vn, 12 * (size_t)k.V, cudaMemcpyDeviceToHost, st));
+    if (vc) AVM_CUDA(cudaMemcpyAsync(vc, a.vc, 12 * (size_t)k.V, cudaMemcpyDeviceToHost, st));
+    if (cvn) AVM_CUDA(cudaMemcpyAsync(cvn, a.cvn, 4 * (size_t)k.N, cudaMemcpyDeviceToHost, st));
+    if (cv) AVM_CUDA(cudaMemcpyAsync(cv, a.cv, 4 * (size_t)k.N * k.S, cudaMemcpyDeviceToHost, st));
+    if (theta) AVM_CUDA(cudaMemcpyAsync(theta, a.theta, 8 * (size_t)k.N, cudaMemcpyDeviceToHost, st));
+  }
+  if (stats) {
+    Counters c;
+    int rc = read_counters(s, &c);
+    if (rc) return rc;
+    stats->step = (int64_t)s->step;
+    stats->t1_short = c.t1_short; stats->t1_candidates = c.t1_candidates; stats->t1_flips = c.t1_flips;
+    stats->t1_blocked = c.t1_blocked; stats->overflow_rejects = c.overflow_rejects; stats->error = c.error;
+    stats->n_sorts = s->n_sorts; stats->kernel_launches = s->launches;
+  } else if (host_outputs) {
+    AVM_CUDA(cudaStreamSynchronize(st));
+  }
+  AVM_CUDA(cudaGetLastError());
+  return AVM_OK;
+}
+
+}  // namespace
+
+// ===============================================================================================
+extern "C" {
+
+size_t avm_workspace_bytes(const avm_params* params) {
+  if (!params_ok(params)) return 0;
+  return make_layout(*params).total;
+}
+
+int avm_create(const avm_params* params, const double* pos_xy, const int32_t* cell_vertex_num,
+               const int32_t* cell_vertices, const int32_t* vertex_neighbors,
+               const int32_t* vertex_cell_neighbors, const double* theta, void* workspace,
+               size_t workspace_bytes, void* cuda_stream, avm_sim** out) {
+  return create_common(params, pos_xy, cell_vertex_num, cell_vertices, vertex_neighbors, vertex_cell_neighbors,
+                       theta, workspace, workspace_bytes, cuda_stream, out, false);
+}
+
+int avm_create_host(const avm_params* params, const double* pos_xy, const int32_t* cell_vertex_num,
+                    const int32_t* cell_vertices, const int32_t* vertex_neighbors,
+                    const int32_t* vertex_cell_neighbors, const double* theta, void* workspace,
+                    size_t workspace_bytes, void* cuda_stream, avm_sim** out) {
+  return create_common(params, pos_xy, cell_vertex_num, cell_vertices, vertex_neighbors, vertex_cell_neighbors,
+                       theta, workspace, workspace_bytes, cuda_stream, out, true);
+}
+
+int avm_step(avm_sim* s, int64_t n_steps) {
+  if (!s || n_steps < 0) return AVM_EINVAL;
+  for (int64_t i = 0; i < n_steps; ++i) {
+    s->launches += launch_step(s->dev(), s->k, s->step, s->stream);
+    s->cur_pos = 1 - s->cur_pos;
+    ++s->step;
+    if (s->p.sort_every > 0 && (s->step - s->p.step0) % (unsigned long long)s->p.sort_every == 0) do_sort(s);
+  }
+  AVM_CUDA(cudaPeekAtLastError());
+  return AVM_OK;
+}
+
+int avm_step_profile(avm_sim* s, int64_t n_steps, double* ms_per_kernel) {
+  if (!s || n_steps < 0 || !ms_per_kernel) return AVM_EINVAL;
+  cudaEvent_t ev[AVM_K_COUNT + 1];
+  for (int i = 0; i <= AVM_K_COUNT; ++i) AVM_CUDA(cudaEventCreate(&ev[i]));
+  for (int i = 0; i < AVM_K_COUNT; ++i) ms_per_kernel[i] = 0.0;
+  for (int64_t i = 0; i < n_steps; ++i) {
+    s->launches += launch_step(s->dev(), s->k, s->step, s->stream, ev);
+    s->cur_pos = 1 - s->cur_pos;
+    ++s->step;
+    AVM_CUDA(cudaEventSynchronize(ev[AVM_K_COUNT]));
+    for (int j = 0; j < AVM_K_COUNT; ++j) {
+      float ms = 0.f;
+      AVM_CUDA(cudaEventElapsedTime(&ms, ev[j], ev[j + 1]));
+      ms_per_kernel[j] += ms;
+    }
+    if (s->p.sort_every > 0 && (s->step - s->p.step0) % (unsigned long long)s->p.sort_every == 0) do_sort(s);
+  }
+  for (int i = 0; i <= AVM_K_COUNT; ++i) cudaEventDestroy(ev[i]);
+  AVM_CUDA(cudaGetLastError());
+  return AVM_OK;
+}
+
+int avm_compute_forces(avm_sim* s, double* force_xy, double* area_perim) {
+  if (!s) return AVM_EINVAL;
+  s->launches += launch_compute_forces(s->dev(), s->k, s->ap, force_xy, area_perim, s->stream);
+  AVM_CUDA(cudaPeekAtLastError());
+  return AVM_OK;
+}
+
+int avm_compute_forces_host(avm_sim* s, double* force_xy, double* area_perim) {
+  if (!s) return AVM_EINVAL;
+  const Dev a = s->dev_alt();
+  double* sf = (double*)a.pos;      // idle ping-pong partner
+  double* sap = (double*)a.rec;     // idle alternate record buffer (32N bytes >= 16N)
+  s->launches += launch_compute_forces(s->dev(), s->k, s->ap, force_xy ? sf : nullptr, area_perim ? sap : nullptr, s->stream);
+  if (force_xy) AVM_CUDA(cudaMemcpyAsync(force_xy, sf, 16 * (size_t)s->k.V, cudaMemcpyDeviceToHost, s->stream));
+  if (area_perim) AVM_CUDA(cudaMemcpyAsync(area_perim, sap, 16 * (size_t)s->k.N, cudaMemcpyDeviceToHost, s->stream));
+  AVM_CUDA(cudaStreamSynchronize(s->stream));
+  AVM_CUDA(cudaGetLastError());
+  return AVM_OK;
+}
+
+int avm_energy(avm_sim* s, double* energy) {
+  if (!s || !energy) return AVM_EINVAL;
+  s->launches += launch_energy(s->dev(), s->k, s->epart, s->stream);
+  Counters c;
+  int rc = read_counters(s, &c);
+  if (rc) return rc;
+  *energy = c.energy;
+  return AVM_OK;
+}
+
+int avm_get_state(avm_sim* s, double* pos_xy, int32_t* cell_vertex_num, int32_t* cell_vertices,
+                  int32_t* vertex_neighbors, int32_t* vertex_cell_neighbors, double* theta, avm_stats* stats) {
+  return get_state_common(s, pos_xy, cell_vertex_num, cell_vertices, vertex_neighbors, vertex_cell_neighbors, theta, stats, false);
+}
+
+int avm_get_state_host(avm_sim* s, double* pos_xy, int32_t* cell_vertex_num, int32_t* cell_vertices,
+                       int32_t* vertex_neighbors, int32_t* vertex_cell_neighbors, double* theta, avm_stats* stats) {
+  return get_state_common(s, pos_xy, cell_vertex_num, cell_vertices, vertex_neighbors, vertex_cell_neighbors, theta, stats, true);
+}
+
+int avm_debug_t1(avm_sim* s, int32_t* cand_pairs, int64_t* n_cand, int32_t* winner_pairs, int64_t* n_win, int64_t capacity) {
+  if (!s || !n_cand || !n_win || capacity < 0) return AVM_EINVAL;
+  const Dev a = s->dev_alt();
+  // staging in idle alternate buffers: cv (4*N*S bytes) and rec (32*N bytes) hold >= 3N/4N pairs
+  int* sc = a.cv;
+  int* sw = (int*)a.rec;
+  const long long cap_c = (long long)s->k.N * s->k.S / 2, cap_w = (long long)s->k.N * 4;
+  const long long cc = capacity < cap_c ? capacity : cap_c, cw = capacity < cap_w ? capacity : cap_w;
+  s->launches += launch_t1_debug(s->dev(), s->k, cand_pairs ? sc : nullptr, winner_pairs ? sw : nullptr, cc < cw ? cc : cw, s->stream);
+  Counters c;
+  int rc = read_counters(s, &c);
+  if (rc) return rc;
+  *n_cand = c.n_cand; *n_win = c.n_win;
+  const long long lim = cc < cw ? cc : cw;
+  const long long ncopy = (long long)c.n_cand < lim ? (long long)c.n_cand : lim;
+  const long long wcopy = (long long)c.n_win < lim ? (long long)c.n_win : lim;
+  if (cand_pairs && ncopy) AVM_CUDA(cudaMemcpyAsync(cand_pairs, sc, 8 * (size_t)ncopy, cudaMemcpyDeviceToHost, s->stream));
+  if (winner_pairs && wcopy) AVM_CUDA(cudaMemcpyAsync(winner_pairs, sw, 8 * (size_t)wcopy, cudaMemcpyDeviceToHost, s->stream));
+  AVM_CUDA(cudaMemsetAsync(&s->ctr->n_short, 0, 16, s->stream));
+  AVM_CUDA(cudaStreamSynchronize(s->stream));
+  return AVM_OK;
+}
+
+int avm_t1_pass(avm_sim* s) {
+  if (!s) return AVM_EINVAL;
+  s->launches += launch_t1_pass_only(s->dev(), s->k, s->stream);
+  AVM_CUDA(cudaPeekAtLastError());
+  return AVM_OK;
+}
+
+int avm_set_positions(avm_sim* s, const double* pos_xy) {
+  if (!s || !pos_xy) return AVM_EINVAL;
+  const Dev d = s->dev();
+  import_positions_kernel<<<cdiv(s->k.V, 256), 256, 0, s->stream>>>(d, s->k, pos_xy);
+  ++s->launches;
+  s->launches += launch_refresh_cells(d, s->k, s->stream);
+  AVM_CUDA(cudaPeekAtLastError());
+  return AVM_OK;
+}
+
+int avm_resort(avm_sim* s) {
+  if (!s) return AVM_EINVAL;
+  do_sort(s);
+  AVM_CUDA(cudaPeekAtLastError());
+  return AVM_OK;
+}
+
+int avm_philox_words(avm_sim* s, uint64_t seed, uint64_t step, uint64_t cell0, int64_t n, uint32_t* out_words) {
+  if (!s || !out_words || n < 0) return AVM_EINVAL;
+  s->launches += launch_philox_words(seed, step, cell0, n, out_words, s->stream);
+  AVM_CUDA(cudaPeekAtLastError());
+  return AVM_OK;
+}
+
+int avm_hilbert_index(avm_sim* s, int32_t m, int64_t n, const uint32_t* ix, const uint32_t* iy, uint32_t* out) {
+  if (!s || m < 1 || m > 16 || n < 0 || !ix || !iy || !out) return AVM_EINVAL;
+  s->launches += launch_hilbert_index(m, n, ix, iy, out, s->stream);
+  AVM_CUDA(cudaPeekAtLastError());
+  return AVM_OK;
+}
+
+uint32_t avm_hilbert_index_host(int32_t m, uint32_t ix, uint32_t iy) {
+  if (m < 1 || m > 16) return 0;
+  return hilbert_index_host(ix, iy, m);
+}
+
+void avm_destroy(avm_sim* s) { delete s; }
+
+const char* avm_strerror(int code) {
+  switch (code) {
+    case AVM_OK: return "ok";
+    case AVM_EINVAL: return "invalid argument (NULL pointer, V != 2N, bad stride or parameter)";
+    case AVM_EWORKSPACE: return "workspace too small or not 256-byte aligned";
+    case AVM_EINCONSISTENT: return "topology lists are out of range or inconsistent with each other";
+    case AVM_ECUDA: return "CUDA error (see avm_last_cuda_error)";
+    case AVM_ENOMEM: return "out of host memory";
+    default: return "unknown error";
+  }
+}
+
+const char* avm_last_cuda_error(void) { return g_cuda_error.c_str(); }
+
+}  // extern "C"

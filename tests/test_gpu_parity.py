@@ -1,0 +1,343 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element
+on the same seeded inputs.  Tolerances are BASELINE.json's `north_star`:
+  * per-step geometry and forces from an identical state: 1e-10 relative (fp64);
+  * T1 candidate sets and post-flip topology: bit-exact in canonical form (R19), excluding edges
+    within 1e-9 of l_c;
+  * trajectories: 1e-8 in positions over the first 100 steps of configs[0].
+Run on the B200 box with `pytest -m gpu`."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+import oracle
+from paper_1702_02939_b200 import workloads as w
+from tests import helpers as h
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "these tests need the B200"
+    from paper_1702_02939_b200 import build
+    build.build()
+    from paper_1702_02939_b200 import binding
+    return binding
+
+
+_TILINGS = {}
+
+
+def tiling(k):
+    if k not in _TILINGS:
+        _TILINGS[k] = w.config_tiling(k)
+    return _TILINGS[k]
+
+
+def to_np(state):
+    return {k: (v.cpu().numpy() if hasattr(v, "cpu") else v) for k, v in state.items()}
+
+
+def assert_forces_close(F, Fo, ap, apo):
+    # per-cell relative on A and P (areas can be tiny/negative transiently: guard with mean scale)
+    sa = np.maximum(np.abs(apo[:, 0]), np.abs(apo[:, 0]).mean())
+    assert (np.abs(ap[:, 0] - apo[:, 0]) <= 1e-10 * sa).all()
+    assert (np.abs(ap[:, 1] - apo[:, 1]) <= 1e-10 * np.abs(apo[:, 1])).all()
+    rms = np.sqrt((Fo ** 2).sum(axis=1).mean())
+    nf = np.linalg.norm(Fo, axis=1)
+    err = np.linalg.norm(F - Fo, axis=1)
+    assert (err <= 1e-10 * np.maximum(nf, rms)).all(), (err / np.maximum(nf, rms)).max()
+
+
+def assert_positions_close(p, po, Lx, Ly, tol):
+    d = p - po
+    d = np.hypot(h.min_image(d[:, 0], Lx), h.min_image(d[:, 1], Ly))
+    assert d.max() <= tol, d.max()
+
+
+def assert_states_match(sg, so, Lx, Ly, pos_tol=1e-8):
+    h.assert_same_topology(sg, so)
+    assert_positions_close(sg["pos"], so["pos"], Lx, Ly, pos_tol)
+    assert np.abs(sg["theta"] - so["theta"]).max() <= pos_tol
+    for key in ("step", "t1_short", "t1_candidates", "t1_flips", "t1_blocked", "overflow_rejects", "error"):
+        assert sg["stats"][key] == so["stats"][key], key
+
+
+# ------------------------------------------------------------------------------------------------
+def test_philox_words_bit_exact(B):
+    t = tiling(0)
+    sim = B.from_tiling(t, **w.config_params(0))
+    for seed, step, cell0 in [(7, 0, 0), (7, 99, 1000), (0xDEADBEEFCAFEF00D, (3 << 32) | 17, 2 ** 31 - 5000)]:
+        got = sim.philox_words(seed, step, cell0, 4096)
+        assert np.array_equal(got, oracle.philox_words(seed, step, cell0, 4096))
+
+
+@pytest.mark.parametrize("k", [0, 1, 2])
+@pytest.mark.parametrize("sort", [False, True])
+def test_geometry_and_forces_parity(B, k, sort):
+    t = tiling(k)
+    p = dict(w.config_params(k), sort_at_create=sort)
+    sim = B.from_tiling(t, **p)
+    F, ap = sim.compute_forces()
+    Fo, apo = oracle.from_tiling(t, **p).compute_forces()
+    assert_forces_close(F.cpu().numpy(), Fo, ap.cpu().numpy(), apo)
+    assert abs(sim.energy() - oracle.from_tiling(t, **p).energy()) <= 1e-11 * abs(oracle.from_tiling(t, **p).energy())
+    # host-pointer twin gives the same bits
+    Fh, aph = sim.compute_forces_host()
+    assert np.array_equal(Fh, F.cpu().numpy()) and np.array_equal(aph, ap.cpu().numpy())
+
+
+def test_hexagons_have_zero_force_on_gpu(B):
+    t = w.hex_tiling(8, 6, a=0.62)
+    sim = B.from_tiling(t, KA=1.3, KP=0.7, A0=1.0, P0=3.6)
+    F, ap = sim.compute_forces()
+    assert F.abs().max().item() <= 1e-12
+    assert np.allclose(ap.cpu().numpy()[:, 0], 1.5 * np.sqrt(3) * 0.62 ** 2, rtol=1e-13)
+
+
+def test_trajectory_parity_cfg0_100_steps(B):
+    """The headline trajectory bar: 100 steps of configs[0], positions within 1e-8 at EVERY step,
+    topology and T1 counters bit-exact, through the step-0 T1 burst."""
+    t = tiling(0)
+    p = w.config_params(0)
+    g = B.from_tiling(t, **p)
+    o = oracle.from_tiling(t, **p)
+    for s in range(100):
+        g.step(1)
+        o.step(1)
+        assert_states_match(to_np(g.get_state()), o.get_state(), t.Lx, t.Ly)
+    st = g.stats()
+    assert st["t1_flips"] > 0 and st["error"] == 0
+
+
+@pytest.mark.parametrize("k,steps,chunk", [(1, 60, 10), (2, 12, 4)])
+def test_trajectory_parity_larger_configs(B, k, steps, chunk):
+    t = tiling(k)
+    p = w.config_params(k)
+    g = B.from_tiling(t, **p)
+    o = oracle.from_tiling(t, **p)
+    for s in range(0, steps, chunk):
+        g.step(chunk)
+        o.step(chunk)
+        assert_states_match(to_np(g.get_state()), o.get_state(), t.Lx, t.Ly)
+    assert g.stats()["t1_flips"] > 50
+
+
+def near_threshold(state, pairs, Lx, Ly, l_c, band=1e-9):
+    pos = state["pos"]
+    out = set()
+    for a, b in pairs:
+        d = pos[b] - pos[a]
+        l = np.hypot(h.min_image(d[0], Lx), h.min_image(d[1], Ly))
+        if abs(l - l_c) < band:
+            out.add((a, b))
+    return out
+
+
+@pytest.mark.parametrize("k,harvest", [(0, [0, 1, 3, 10]), (1, [0, 1, 2, 5, 20]), (2, [0, 2])])
+def test_t1_sets_and_post_flip_topology_from_identical_states(B, k, harvest):
+    """States harvested from the oracle trajectory (including the step-0 burst) are loaded into the
+    CUDA path; candidate and winner sets must be equal as sets of (tag_min, tag_max), and one T1
+    pass from that state must give the identical topology."""
+    t = tiling(k)
+    p = w.config_params(k)
+    o = oracle.from_tiling(t, **p)
+    done = 0
+    for target in harvest:
+        o.step(target - done)
+        done = target
+        so = o.get_state()
+        tt = w.Tiling(t.Lx, t.Ly, t.S, so["pos"], so["cell_vertex_num"], so["cell_vertices"],
+                      so["vertex_neighbors"], so["vertex_cell_neighbors"], so["theta"])
+        for sort in (False, True):
+            g = B.from_tiling(tt, **dict(p, step0=target, sort_at_create=sort))
+            cand, win = g.debug_t1()
+            co, wo = o.debug_t1()
+            cg, wg = {tuple(x) for x in cand.tolist()}, {tuple(x) for x in win.tolist()}
+            cs, ws = {tuple(x) for x in co.tolist()}, {tuple(x) for x in wo.tolist()}
+            fuzzy = near_threshold(so, cg ^ cs, t.Lx, t.Ly, p["l_c"])
+            assert (cg ^ cs) <= fuzzy, f"candidate sets differ at step {target}"
+            if not fuzzy:
+                assert wg == ws, f"winner sets differ at step {target}"
+            # one pass from the identical state
+            o2 = oracle.OracleSim(so["pos"], so["cell_vertex_num"], so["cell_vertices"], so["vertex_neighbors"],
+                                  so["vertex_cell_neighbors"], so["theta"], **dict(p, step0=target))
+            o2.t1_pass()
+            g.t1_pass()
+            sg, s2 = to_np(g.get_state()), o2.get_state()
+            if not fuzzy:
+                h.assert_same_topology(sg, s2)
+                assert_positions_close(sg["pos"], s2["pos"], t.Lx, t.Ly, 1e-12)
+                for key in ("t1_short", "t1_candidates", "t1_flips", "t1_blocked", "overflow_rejects"):
+                    assert sg["stats"][key] == s2["stats"][key], key
+            h.check_topology(sg["cell_vertex_num"], sg["cell_vertices"], sg["vertex_neighbors"],
+                             sg["vertex_cell_neighbors"]) if k < 2 else None
+
+
+def test_hilbert_resort_is_a_noop_in_canonical_form(B):
+    t = tiling(1)
+    p = w.config_params(1)
+    g = B.from_tiling(t, **p)
+    g.step(7)
+    before = to_np(g.get_state())
+    F0, ap0 = g.compute_forces()
+    g.resort()
+    after = to_np(g.get_state())
+    h.assert_same_topology(before, after)
+    assert np.array_equal(before["pos"], after["pos"]) and np.array_equal(before["theta"], after["theta"])
+    F1, ap1 = g.compute_forces()
+    assert (F0 - F1).abs().max().item() <= 1e-13 and (ap0 - ap1).abs().max().item() <= 1e-13
+    assert after["stats"]["n_sorts"] == 1
+    # sorting twice changes nothing either
+    g.resort()
+    again = to_np(g.get_state())
+    h.assert_same_topology(before, again)
+
+
+def test_sort_every_trajectory_equals_unsorted(B):
+    t = tiling(1)
+    p = w.config_params(1)
+    a = B.from_tiling(t, **dict(p, sort_every=0))
+    b = B.from_tiling(t, **dict(p, sort_every=5, sort_at_create=True))
+    a.step(40)
+    b.step(40)
+    sa, sb = to_np(a.get_state()), to_np(b.get_state())
+    h.assert_same_topology(sa, sb)
+    assert_positions_close(sa["pos"], sb["pos"], t.Lx, t.Ly, 1e-8)
+    assert sb["stats"]["n_sorts"] == 9 and sa["stats"]["t1_flips"] == sb["stats"]["t1_flips"]
+
+
+def test_hilbert_sort_improves_locality(B):
+    """After the sort, vertices of a cell and neighbours of a vertex are close in memory; checked
+    through the Hilbert keys of the device function on the sorted positions."""
+    t = tiling(2)
+    g = B.from_tiling(t, **w.config_params(2))
+    m = 9
+    gx = np.minimum((t.pos[:, 0] / t.Lx * (1 << m)).astype(np.int64), (1 << m) - 1)
+    gy = np.minimum((t.pos[:, 1] / t.Ly * (1 << m)).astype(np.int64), (1 << m) - 1)
+    keys = g.hilbert_index(m, gx, gy)
+    host = np.array([B.hilbert_index_host(m, int(x), int(y)) for x, y in zip(gx[:2000], gy[:2000])], dtype=np.uint32)
+    assert np.array_equal(keys[:2000], host)
+    order = np.argsort(keys, kind="stable")
+    rank = np.empty_like(order)
+    rank[order] = np.arange(order.size)
+    nb = t.vertex_neighbors
+    spread_sorted = np.abs(rank[nb] - rank[:, None]).mean()
+    spread_unsorted = np.abs(nb - np.arange(t.V)[:, None]).mean()
+    assert spread_sorted < 0.05 * spread_unsorted
+
+
+def test_resume_and_determinism(B):
+    t = tiling(1)
+    p = w.config_params(1)
+    a = B.from_tiling(t, **p)
+    a.step(30)
+    sa = to_np(a.get_state())
+    b = B.from_tiling(t, **p)
+    b.step(30)
+    sb = to_np(b.get_state())
+    for key in ("pos", "theta", "cell_vertices", "vertex_neighbors", "vertex_cell_neighbors", "cell_vertex_num"):
+        assert np.array_equal(sa[key], sb[key]), f"run-to-run nondeterminism in {key}"
+    # resume from a saved state at step 12 continues bit-identically (Philox is counter-based)
+    c = B.from_tiling(t, **p)
+    c.step(12)
+    sc = to_np(c.get_state())
+    tt = w.Tiling(t.Lx, t.Ly, t.S, sc["pos"], sc["cell_vertex_num"], sc["cell_vertices"], sc["vertex_neighbors"],
+                  sc["vertex_cell_neighbors"], sc["theta"])
+    d = B.from_tiling(tt, **dict(p, step0=12))
+    d.step(18)
+    sd = to_np(d.get_state())
+    for key in ("pos", "theta"):
+        assert np.array_equal(sa[key], sd[key]), key
+    h.assert_same_topology(sa, sd)
+
+
+def test_host_pointer_entry_points_round_trip(B):
+    t = tiling(1)
+    p = w.config_params(1)
+    gh = B.from_tiling(t, host=True, **p)
+    gd = B.from_tiling(t, host=False, **p)
+    gh.step(5)
+    gd.step(5)
+    sh = gh.get_state_host()
+    sd = to_np(gd.get_state())
+    for key in ("pos", "theta", "cell_vertices", "vertex_neighbors", "vertex_cell_neighbors", "cell_vertex_num"):
+        assert np.array_equal(sh[key], sd[key]), key
+    assert sh["stats"]["step"] == 5 and sh["stats"]["kernel_launches"] > 0
+
+
+def test_create_rejects_inconsistent_topology(B):
+    t = tiling(0).copy()
+    t.vertex_cell_neighbors[5] = t.vertex_cell_neighbors[5][[1, 2, 0]]      # break the slot convention
+    with pytest.raises(B.AvmError, match="inconsistent"):
+        B.from_tiling(t, **w.config_params(0))
+    t = tiling(0).copy()
+    t.cell_vertex_num[3] = 17
+    with pytest.raises(B.AvmError, match="inconsistent"):
+        B.from_tiling(t, **w.config_params(0))
+    t = tiling(0).copy()
+    t.pos[0, 0] = np.nan
+    with pytest.raises(B.AvmError, match="inconsistent"):
+        B.from_tiling(t, **w.config_params(0))
+
+
+def test_degenerate_cases(B):
+    # l_c = 0: no T1 ever; Dr = 0, v0 = 0: pure gradient descent, energy decreases
+    t = tiling(0)
+    p = dict(w.config_params(0), l_c=0.0, v0=0.0, Dr=0.0, dt=1e-3)
+    g = B.from_tiling(t, **p)
+    E = [g.energy()]
+    for _ in range(20):
+        g.step(1)
+        E.append(g.energy())
+    assert all(b < a for a, b in zip(E, E[1:]))
+    st = g.stats()
+    assert st["t1_short"] == 0 and st["t1_flips"] == 0
+    # pure activity: closed-form translation (same pin as the oracle's)
+    th0 = 0.7
+    hx = w.hex_tiling(6, 4, a=1.0, theta=np.full(24, th0))
+    g = B.from_tiling(hx, KA=0.0, KP=0.0, v0=0.3, Dr=0.0, dt=0.01, l_c=0.0)
+    g.step(250)
+    s = to_np(g.get_state())
+    expect = hx.pos + 250 * 0.3 * 0.01 * np.array([np.cos(th0), np.sin(th0)])
+    assert_positions_close(s["pos"], expect, hx.Lx, hx.Ly, 1e-12)
+    # zero steps is a no-op
+    g.step(0)
+    assert g.stats()["step"] == 250
+
+
+def test_overflow_guard_on_gpu(B):
+    t16 = tiling(1)
+    nmax = int(t16.cell_vertex_num.max())
+    assert nmax % 4 == 0, "cfg1's largest cell has 12 vertices"
+    t = w.voronoi_tiling(4096, 64.0, 2, S=nmax)
+    p = w.config_params(1)
+    g = B.from_tiling(t, **p)
+    o = oracle.from_tiling(t, **p)
+    g.step(30)
+    o.step(30)
+    sg, so = to_np(g.get_state()), o.get_state()
+    assert_states_match(sg, so, t.Lx, t.Ly)
+
+
+@pytest.mark.parametrize("k,steps", [(3, 3), (4, 2)])
+def test_full_size_configs_against_oracle(B, k, steps):
+    """BASELINE.json's full sizes in the launch configuration bench.py times (Hilbert-sorted at
+    create): whole-state comparison after a few steps, plus forces from the identical state."""
+    t = tiling(k)
+    p = w.config_params(k)
+    g = B.from_tiling(t, **p)
+    o = oracle.from_tiling(t, **p)
+    F, ap = g.compute_forces()
+    Fo, apo = o.compute_forces()
+    assert_forces_close(F.cpu().numpy(), Fo, ap.cpu().numpy(), apo)
+    del F, ap
+    g.step(steps)
+    o.step(steps)
+    sg, so = to_np(g.get_state()), o.get_state()
+    assert_states_match(sg, so, t.Lx, t.Ly)
+    assert sg["stats"]["t1_flips"] > 1000
+    L2 = t.Lx * t.Ly
+    apg = g.compute_forces()[1].cpu().numpy()
+    assert abs(apg[:, 0].sum() - L2) <= 1e-12 * L2
+    _TILINGS.pop(k, None)
