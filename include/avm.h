@@ -115,8 +115,7 @@ int avm_step(avm_sim* sim, int64_t n_steps);
  * and the call synchronises after each step: ms_per_kernel (HOST pointer, [AVM_K_COUNT]) receives
  * the summed device time of each kernel class over the n_steps.  Measurement aid for the roofline
  * figures of bench.py; not the timed path. */
-enum { AVM_K_FORCE_MOVE = 0, AVM_K_CELL_UPDATE = 1, AVM_K_T1_MARK = 2, AVM_K_T1_FLIP = 3, AVM_K_T1_RESET = 4,
-       AVM_K_COUNT = 5 };
+enum { AVM_K_FORCE_MOVE = 0, AVM_K_CELL_UPDATE = 1, AVM_K_T1_FLIP = 2, AVM_K_COUNT = 3 };
 int avm_step_profile(avm_sim* sim, int64_t n_steps, double* ms_per_kernel);
 
 /* Geometry + forces of the current state, nothing modified (App. A.1, Eq. A1-A5):

@@ -174,7 +174,7 @@ class AvmSim:
     def step(self, n: int = 1) -> None:
         _check(lib.avm_step(self._h, n))
 
-    KERNEL_NAMES = ("force_move", "cell_update", "t1_mark", "t1_flip", "t1_reset")
+    KERNEL_NAMES = ("force_move", "cell_update", "t1_flip")
 
     def step_profile(self, n: int) -> dict:
         """n steps with every kernel bracketed by CUDA events; summed device ms per kernel class."""

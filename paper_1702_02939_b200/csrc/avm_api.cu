@@ -30,30 +30,33 @@ thread_local std::string g_cuda_error;
 
 inline size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
+inline int plane_stride(int V) { return (V + 63) & ~63; }
+
 struct BufferSet {
-  int *vn, *vc, *cv, *cvn, *vtag, *ctag;
+  int *vn, *vc, *cvn, *vtag, *ctag;
+  int4* cv;
   double* theta;
   CellRec* rec;
 };
 
 struct Layout {
   size_t pos[2], vn[2], vc[2], cv[2], cvn[2], theta[2], rec[2], vtag[2], ctag[2];
-  size_t minkey, short_list, cand, ctr, ap, epart, key[2], val[2], hist, newidx_v, newidx_c, order_v, order_c;
+  size_t minkey, cand, ctr, ap, epart, key[2], val[2], hist, newidx_v, newidx_c, order_v, order_c;
   size_t total;
 };
 
 Layout make_layout(const avm_params& p) {
   Layout L;
   const size_t N = (size_t)p.n_cells, V = (size_t)p.n_vertices, S = (size_t)p.max_cell_vertices;
+  const size_t Vs = (size_t)plane_stride(p.n_vertices);
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
   for (int i = 0; i < 2; ++i) L.pos[i] = take(16 * V);
   for (int i = 0; i < 2; ++i) {
-    L.vn[i] = take(12 * V); L.vc[i] = take(12 * V); L.cv[i] = take(4 * N * S); L.cvn[i] = take(4 * N);
+    L.vn[i] = take(12 * Vs); L.vc[i] = take(12 * Vs); L.cv[i] = take(4 * N * S); L.cvn[i] = take(4 * N);
     L.theta[i] = take(8 * N); L.rec[i] = take(32 * N); L.vtag[i] = take(4 * V); L.ctag[i] = take(4 * N);
   }
   L.minkey = take(8 * N);
-  L.short_list = take(8 * 3 * N);
   L.cand = take(sizeof(Cand) * 3 * N);
   L.ctr = take(sizeof(Counters));
   L.ap = take(16 * N);
@@ -86,7 +89,6 @@ struct avm_sim {
   double2* pos[2];
   BufferSet set[2];
   unsigned long long* minkey;
-  int2* short_list;
   Cand* cand;
   Counters* ctr;
   double2* ap;
@@ -102,7 +104,7 @@ struct avm_sim {
     const BufferSet& b = set[cur_set];
     d.vn = b.vn; d.vc = b.vc; d.cv = b.cv; d.cvn = b.cvn; d.theta = b.theta; d.rec = b.rec;
     d.vtag = b.vtag; d.ctag = b.ctag;
-    d.minkey = minkey; d.short_list = short_list; d.cand = cand; d.ctr = ctr;
+    d.minkey = minkey; d.cand = cand; d.ctr = ctr;
     return d;
   }
   Dev dev_alt() const {   // the other buffer set, target of a re-sort / staging area
@@ -118,15 +120,22 @@ struct avm_sim {
 namespace {
 
 // ---- creation-time kernels ---------------------------------------------------------------------
-__global__ void init_kernel(const Dev d, const Consts k) {
+// user layout (staged in the alternate buffer set: vn/vc [V][3], cv [N][S] row-major) -> internal
+// structure-of-arrays layout (vn/vc planes, cv int4 planes), tags, idle minimum keys
+__global__ void import_kernel(const Dev d, const Consts k, const int* __restrict__ vn_u, const int* __restrict__ vc_u,
+                              const int* __restrict__ cv_u) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < k.V) d.vtag[i] = i;
+  if (i < k.V) {
+    d.vtag[i] = i;
+#pragma unroll
+    for (int s = 0; s < 3; ++s) { d.vn[s * k.Vs + i] = vn_u[3 * i + s]; d.vc[s * k.Vs + i] = vc_u[3 * i + s]; }
+  }
   if (i < k.N) {
     d.ctag[i] = i;
     d.minkey[i] = ~0ull;
     int n = d.cvn[i];
     n = n < 0 ? 0 : (n > k.S ? k.S : n);
-    for (int j = n; j < k.S; ++j) d.cv[(size_t)i * k.S + j] = -1;   // normalise the padding
+    for (int j = 0; j < k.S; ++j) row_entry(d.cv, k.N, i, j) = j < n ? cv_u[(size_t)i * k.S + j] : -1;   // normalise the padding
   }
 }
 
@@ -139,9 +148,9 @@ __global__ void validate_kernel(const Dev d, const Consts k) {
     if (n < 3 || n > k.S) bad = true;
     else
       for (int j = 0; j < n; ++j) {
-        const int v = d.cv[(size_t)i * k.S + j];
+        const int v = row_entry(d.cv, k.N, i, j);
         if (v < 0 || v >= k.V) { bad = true; break; }
-        const int c0 = d.vc[3 * v], c1 = d.vc[3 * v + 1], c2 = d.vc[3 * v + 2];
+        const int c0 = d.vc[v], c1 = d.vc[k.Vs + v], c2 = d.vc[2 * k.Vs + v];
         if (c0 != i && c1 != i && c2 != i) bad = true;
       }
   }
@@ -149,15 +158,14 @@ __global__ void validate_kernel(const Dev d, const Consts k) {
     const double2 h = d.pos[i];
     if (!(h.x >= 0.0 && h.x < k.Lx && h.y >= 0.0 && h.y < k.Ly)) bad = true;
     for (int s = 0; s < 3 && !bad; ++s) {
-      const int w = d.vn[3 * i + s], c = d.vc[3 * i + s], wn = d.vn[3 * i + (s + 1) % 3];
+      const int w = d.vn[s * k.Vs + i], c = d.vc[s * k.Vs + i], wn = d.vn[((s + 1) % 3) * k.Vs + i];
       if (w < 0 || w >= k.V || c < 0 || c >= k.N || w == i) { bad = true; break; }
       const int n = d.cvn[c];
       if (n < 3 || n > k.S) { bad = true; break; }
-      const int* row = d.cv + (size_t)c * k.S;
       int j = -1;
-      for (int t = 0; t < n; ++t) if (row[t] == i) j = t;
+      for (int t = 0; t < n; ++t) if (row_entry(d.cv, k.N, c, t) == i) j = t;
       if (j < 0) { bad = true; break; }
-      if (row[(j + 1) % n] != w || row[(j + n - 1) % n] != wn) bad = true;
+      if (row_entry(d.cv, k.N, c, (j + 1) % n) != w || row_entry(d.cv, k.N, c, (j + n - 1) % n) != wn) bad = true;
     }
   }
   if (bad) atomicOr((unsigned long long*)&d.ctr->error, 4ull);
@@ -170,8 +178,8 @@ __global__ void export_vertices_kernel(const Dev d, const Consts k, double* pos,
   const int t = d.vtag[v];
   if (pos) { const double2 h = d.pos[v]; pos[2 * t] = h.x; pos[2 * t + 1] = h.y; }
   for (int s = 0; s < 3; ++s) {
-    if (vn) vn[3 * t + s] = d.vtag[d.vn[3 * v + s]];
-    if (vc) vc[3 * t + s] = d.ctag[d.vc[3 * v + s]];
+    if (vn) vn[3 * t + s] = d.vtag[d.vn[s * k.Vs + v]];
+    if (vc) vc[3 * t + s] = d.ctag[d.vc[s * k.Vs + v]];
   }
 }
 __global__ void export_cells_kernel(const Dev d, const Consts k, int* cvn, int* cv, double* theta) {
@@ -182,7 +190,7 @@ __global__ void export_cells_kernel(const Dev d, const Consts k, int* cvn, int* 
   if (cvn) cvn[t] = n;
   if (theta) theta[t] = d.theta[c];
   if (cv)
-    for (int j = 0; j < k.S; ++j) cv[(size_t)t * k.S + j] = j < n ? d.vtag[d.cv[(size_t)c * k.S + j]] : -1;
+    for (int j = 0; j < k.S; ++j) cv[(size_t)t * k.S + j] = j < n ? d.vtag[row_entry(d.cv, k.N, c, j)] : -1;
 }
 __global__ void import_positions_kernel(const Dev d, const Consts k, const double* pos) {
   const int v = blockIdx.x * blockDim.x + threadIdx.x;
@@ -195,6 +203,7 @@ inline int cdiv(long long a, int b) { return (int)((a + b - 1) / b); }
 
 int do_sort(avm_sim* s) {
   const Dev a = s->dev(), b = s->dev_alt();
+  s->launches += launch_t1_reset(a, s->k, s->stream);   // candidate lists hold pre-sort indices
   s->launches += launch_hilbert_sort(a, b, s->k, s->sc, s->stream);
   s->cur_pos = 1 - s->cur_pos;
   s->cur_set = 1 - s->cur_set;
@@ -225,7 +234,7 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   s->L = L;
   const int N = params->n_cells, V = params->n_vertices, S = params->max_cell_vertices;
   Consts& k = s->k;
-  k.N = N; k.V = V; k.S = S;
+  k.N = N; k.V = V; k.S = S; k.Vs = plane_stride(V);
   k.Lx = params->Lx; k.Ly = params->Ly; k.hLx = 0.5 * params->Lx; k.hLy = 0.5 * params->Ly;
   k.KA = params->KA; k.KP = params->KP; k.KA2 = 2.0 * params->KA; k.KP2 = 2.0 * params->KP;
   k.A0 = params->A0; k.P0 = params->P0;
@@ -237,13 +246,12 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   for (int i = 0; i < 2; ++i) {
     s->pos[i] = (double2*)(w + L.pos[i]);
     BufferSet& b = s->set[i];
-    b.vn = (int*)(w + L.vn[i]); b.vc = (int*)(w + L.vc[i]); b.cv = (int*)(w + L.cv[i]);
+    b.vn = (int*)(w + L.vn[i]); b.vc = (int*)(w + L.vc[i]); b.cv = (int4*)(w + L.cv[i]);
     b.cvn = (int*)(w + L.cvn[i]); b.theta = (double*)(w + L.theta[i]); b.rec = (CellRec*)(w + L.rec[i]);
     b.vtag = (int*)(w + L.vtag[i]); b.ctag = (int*)(w + L.ctag[i]);
     s->sc.key[i] = (unsigned int*)(w + L.key[i]); s->sc.val[i] = (int*)(w + L.val[i]);
   }
   s->minkey = (unsigned long long*)(w + L.minkey);
-  s->short_list = (int2*)(w + L.short_list);
   s->cand = (Cand*)(w + L.cand);
   s->ctr = (Counters*)(w + L.ctr);
   s->ap = (double2*)(w + L.ap);
@@ -258,6 +266,7 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   cudaStream_t st = s->stream;
   const cudaMemcpyKind kind = host_inputs ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
   const BufferSet& b = s->set[0];
+  const BufferSet& stage = s->set[1];   // user-layout staging for the import kernel
   auto fail = [&](int code) { delete s; return code; };
 #define AVM_CUDA_F(call)                                                                    \
   do {                                                                                      \
@@ -268,22 +277,21 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
     }                                                                                       \
   } while (0)
   AVM_CUDA_F(cudaMemcpyAsync(s->pos[0], pos_xy, 16 * (size_t)V, kind, st));
-  AVM_CUDA_F(cudaMemcpyAsync(b.vn, vn, 12 * (size_t)V, kind, st));
-  AVM_CUDA_F(cudaMemcpyAsync(b.vc, vc, 12 * (size_t)V, kind, st));
-  AVM_CUDA_F(cudaMemcpyAsync(b.cv, cv, 4 * (size_t)N * S, kind, st));
+  AVM_CUDA_F(cudaMemcpyAsync(stage.vn, vn, 12 * (size_t)V, kind, st));
+  AVM_CUDA_F(cudaMemcpyAsync(stage.vc, vc, 12 * (size_t)V, kind, st));
+  AVM_CUDA_F(cudaMemcpyAsync(stage.cv, cv, 4 * (size_t)N * S, kind, st));
   AVM_CUDA_F(cudaMemcpyAsync(b.cvn, cvn, 4 * (size_t)N, kind, st));
   AVM_CUDA_F(cudaMemcpyAsync(b.theta, theta, 8 * (size_t)N, kind, st));
   AVM_CUDA_F(cudaMemsetAsync(s->ctr, 0, sizeof(Counters), st));
   const Dev d = s->dev();
+  import_kernel<<<cdiv(V, 256), 256, 0, st>>>(d, k, stage.vn, stage.vc, (const int*)stage.cv);
   validate_kernel<<<cdiv(V, 256), 256, 0, st>>>(d, k);
-  ++s->launches;
+  s->launches += 2;
   Counters c;
   AVM_CUDA_F(cudaMemcpyAsync(&c, s->ctr, sizeof(Counters), cudaMemcpyDeviceToHost, st));
   AVM_CUDA_F(cudaStreamSynchronize(st));
   AVM_CUDA_F(cudaGetLastError());
   if (c.error & 4) return fail(AVM_EINCONSISTENT);
-  init_kernel<<<cdiv(V, 256), 256, 0, st>>>(d, k);
-  ++s->launches;
   s->launches += launch_refresh_cells(d, k, st);
   if (params->flags & AVM_FLAG_SORT_AT_CREATE) do_sort(s);
   AVM_CUDA_F(cudaGetLastError());
@@ -310,7 +318,7 @@ int get_state_common(avm_sim* s, double* pos_xy, int32_t* cvn, int32_t* cv, int3
       ++s->launches;
     }
     if (cvn || cv || theta) {
-      export_cells_kernel<<<cdiv(k.N, 256), 256, 0, st>>>(d, k, cvn ? a.cvn : nullptr, cv ? a.cv : nullptr, theta ? a.theta : nullptr);
+      export_cells_kernel<<<cdiv(k.N, 256), 256, 0, st>>>(d, k, cvn ? a.cvn : nullptr, cv ? (int*)a.cv : nullptr, theta ? a.theta : nullptr);
       ++s->launches;
     }
     if (pos_xy) AVM_CUDA(cudaMemcpyAsync(pos_xy, spos, 16 * (size_t)k.V, cudaMemcpyDeviceToHost, st));
@@ -439,7 +447,7 @@ int avm_debug_t1(avm_sim* s, int32_t* cand_pairs, int64_t* n_cand, int32_t* winn
   if (!s || !n_cand || !n_win || capacity < 0) return AVM_EINVAL;
   const Dev a = s->dev_alt();
   // staging in idle alternate buffers: cv (4*N*S bytes) and rec (32*N bytes) hold >= 3N/4N pairs
-  int* sc = a.cv;
+  int* sc = (int*)a.cv;
   int* sw = (int*)a.rec;
   const long long cap_c = (long long)s->k.N * s->k.S / 2, cap_w = (long long)s->k.N * 4;
   const long long cc = capacity < cap_c ? capacity : cap_c, cw = capacity < cap_w ? capacity : cap_w;
@@ -447,13 +455,13 @@ int avm_debug_t1(avm_sim* s, int32_t* cand_pairs, int64_t* n_cand, int32_t* winn
   Counters c;
   int rc = read_counters(s, &c);
   if (rc) return rc;
-  *n_cand = c.n_cand; *n_win = c.n_win;
+  *n_cand = c.n_cand[0]; *n_win = c.n_win;
   const long long lim = cc < cw ? cc : cw;
-  const long long ncopy = (long long)c.n_cand < lim ? (long long)c.n_cand : lim;
+  const long long ncopy = (long long)c.n_cand[0] < lim ? (long long)c.n_cand[0] : lim;
   const long long wcopy = (long long)c.n_win < lim ? (long long)c.n_win : lim;
   if (cand_pairs && ncopy) AVM_CUDA(cudaMemcpyAsync(cand_pairs, sc, 8 * (size_t)ncopy, cudaMemcpyDeviceToHost, s->stream));
   if (winner_pairs && wcopy) AVM_CUDA(cudaMemcpyAsync(winner_pairs, sw, 8 * (size_t)wcopy, cudaMemcpyDeviceToHost, s->stream));
-  AVM_CUDA(cudaMemsetAsync(&s->ctr->n_short, 0, 16, s->stream));
+  s->launches += launch_t1_reset(s->dev(), s->k, s->stream);
   AVM_CUDA(cudaStreamSynchronize(s->stream));
   return AVM_OK;
 }

@@ -16,7 +16,7 @@ namespace avm {
 //   nx = cos(theta_c), ny = sin(theta_c)   (director)
 struct __align__(32) CellRec { double a, p, nx, ny; };
 
-// One eligible T1 candidate (R10), decoded once by t1_mark and reused by t1_flip / t1_reset.
+// One eligible T1 candidate (R10), decoded once by the detecting thread and reused by the flip.
 struct __align__(16) Cand {
   int v1, v2;           // v1 = endpoint with the smaller tag
   int k1, k2;           // slot of v2 in v1, slot of v1 in v2
@@ -26,8 +26,9 @@ struct __align__(16) Cand {
 };
 
 struct Counters {
-  unsigned int n_short;   // short edges appended this step
-  unsigned int n_cand;    // eligible candidates this step
+  // candidate list length, double-buffered by step parity: the list of step s is flipped by
+  // t1_flip(s) and its per-cell minimum keys are cleared by the prologue of force_move(s+1)
+  unsigned int n_cand[2];
   unsigned int n_win;     // winners (debug hook only)
   unsigned int pad;
   long long t1_short, t1_candidates, t1_flips, t1_blocked, overflow_rejects, error;
@@ -37,6 +38,7 @@ struct Counters {
 // Model constants, passed by value to every kernel.
 struct Consts {
   int N, V, S;
+  int Vs;                    // plane stride of vn / vc (V rounded up to 64 entries)
   double Lx, Ly, hLx, hLy;
   double KA2, KP2, A0, P0;   // KA2 = 2 K_A, KP2 = 2 K_P
   double KA, KP;
@@ -47,19 +49,25 @@ struct Consts {
 };
 
 // Pointers into the caller's workspace (current buffer set).
+//
+// Layout: everything is structure-of-arrays.
+//   vn, vc : three planes of Vs ints each: vn[k*Vs + v] = k-th neighbour of v (slot convention R12)
+//   cv     : fixed-stride padded rows stored as S/4 planes of int4: entries 4q..4q+3 of cell c are
+//            cv[q*N + c]; unused entries = -1.  A warp reads 32 consecutive cells' quads with one
+//            fully coalesced 128-bit load per plane, and cells with <= 8 vertices (96 %) never
+//            touch planes 2, 3.
 struct Dev {
   double2* pos;       // [V] current positions
   double2* pos_next;  // [V] written by force_move, then swapped
-  int* vn;            // [3V] vertexNeighbors
-  int* vc;            // [3V] vertexCellNeighbors
-  int* cv;            // [N*S] cellVertices (rows), unused = -1
+  int* vn;            // [3*Vs] vertexNeighbors planes
+  int* vc;            // [3*Vs] vertexCellNeighbors planes
+  int4* cv;           // [(S/4)*N] cellVertices planes
   int* cvn;           // [N] cellVertexNum
   double* theta;      // [N]
   CellRec* rec;       // [N]
   int* vtag;          // [V] user index of each vertex
   int* ctag;          // [N] user index of each cell
   unsigned long long* minkey;  // [N] per-cell minimum candidate key, ~0 when idle
-  int2* short_list;   // [3N] short edges found by the detection pass
   Cand* cand;         // [3N]
   Counters* ctr;
 };
@@ -77,6 +85,30 @@ __device__ __forceinline__ double wrap_box(double x, double L) {
   if (x >= L) x -= L;
   return x;
 }
+__device__ __forceinline__ unsigned int hi_word(double x) { return (unsigned int)__double2hiint(x); }
+
+// entry j of cell c's row
+__device__ __forceinline__ int& row_entry(int4* cv, int N, int c, int j) {
+  return reinterpret_cast<int*>(cv + (size_t)(j >> 2) * N + c)[j & 3];
+}
+__device__ __forceinline__ int row_entry(const int4* cv, int N, int c, int j) {
+  return reinterpret_cast<const int*>(cv + (size_t)(j >> 2) * N + c)[j & 3];
+}
+
+// 1/sqrt(x) for x >= 0: MUFU.RSQ64H seed (rel. error ~2^-22) and one third-order step
+// y <- y (1 + e/2 + 3 e^2/8), e = 1 - x y^2, which leaves ~2^-64 before rounding.  Returns 0 for
+// x below the normal range: a zero-length edge contributes nothing (R15).
+__device__ __forceinline__ double rsqrt_pos(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double t = __dmul_rn(x, y);
+  const double e = __fma_rn(-t, y, 1.0);
+  const double p = __fma_rn(0.375, e, 0.5);
+  const double ye = __dmul_rn(y, e);
+  y = __fma_rn(ye, p, y);
+  return x >= 2.2250738585072014e-308 ? y : 0.0;
+}
+__device__ __forceinline__ double sqrt_pos(double x) { return __dmul_rn(x, rsqrt_pos(x)); }
 
 // Philox4x32-10 (Salmon et al., SC'11; R16).  Counter (c0..c3), key (k0,k1).
 __device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint2 k) {
@@ -105,26 +137,36 @@ __device__ __forceinline__ double director_noise(unsigned long long seed, unsign
   return sqrt(-2.0 * log(u1)) * cospi(2.0 * u2);
 }
 
-// Area and perimeter of one cell from its row (Eq. A1 inputs; shoelace with every vertex
-// unwrapped relative to the row's first vertex, R14).  Used by the cold paths (T1 flip refresh,
-// avm_compute_forces); the per-step pass has its own fused copy.
-__device__ __forceinline__ void cell_area_perimeter(const double2* __restrict__ pos, const int* __restrict__ row,
-                                                    int n, const Consts& k, double& A, double& P) {
-  const double2 h0 = pos[row[0]];
-  double rx_prev = 0.0, ry_prev = 0.0, acc = 0.0, per = 0.0;
+// One edge of the shoelace / perimeter sums (Eq. A1 inputs, R14): previous unwrapped vertex
+// (rxp, ryp), current (rx, ry), both relative to the row's first vertex.  Explicit rounding
+// intrinsics fix the operation order, so every kernel that sums a cell (the per-step pass, the T1
+// refresh, avm_compute_forces) produces the same bits.  Returns the squared edge length.
+__device__ __forceinline__ double geom_edge(double rxp, double ryp, double rx, double ry, double& acc, double& per) {
+  acc = __fma_rn(rxp, ry, acc);
+  acc = __fma_rn(-ryp, rx, acc);
+  const double dx = __dsub_rn(rx, rxp), dy = __dsub_rn(ry, ryp);
+  const double l2 = __fma_rn(dx, dx, __dmul_rn(dy, dy));
+  per = __dadd_rn(per, sqrt_pos(l2));
+  return l2;
+}
+
+// Area and perimeter of one cell from its row, one thread, plain loads (safe right after this
+// warp rewrote the row).  Used by the cold paths: T1 refresh, avm_compute_forces, energy.
+__device__ __forceinline__ void cell_area_perimeter(const double2* pos, const int4* cv, int c, int n,
+                                                    const Consts& k, double& A, double& P) {
+  const double2 h0 = pos[row_entry(cv, k.N, c, 0)];
+  double rxp = 0.0, ryp = 0.0, acc = 0.0, per = 0.0;
   for (int j = 1; j <= n; ++j) {
     double rx = 0.0, ry = 0.0;
     if (j < n) {
-      const double2 hj = pos[row[j]];
-      rx = min_image(hj.x - h0.x, k.Lx, k.hLx);
-      ry = min_image(hj.y - h0.y, k.Ly, k.hLy);
+      const double2 hj = pos[row_entry(cv, k.N, c, j)];
+      rx = min_image(__dsub_rn(hj.x, h0.x), k.Lx, k.hLx);
+      ry = min_image(__dsub_rn(hj.y, h0.y), k.Ly, k.hLy);
     }
-    acc += rx_prev * ry - ry_prev * rx;
-    const double dx = rx - rx_prev, dy = ry - ry_prev;
-    per += sqrt(dx * dx + dy * dy);
-    rx_prev = rx; ry_prev = ry;
+    geom_edge(rxp, ryp, rx, ry, acc, per);
+    rxp = rx; ryp = ry;
   }
-  A = 0.5 * acc; P = per;
+  A = __dmul_rn(0.5, acc); P = per;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -133,6 +175,7 @@ __device__ __forceinline__ void cell_area_perimeter(const double2* __restrict__ 
 // ---------------------------------------------------------------------------------------------
 int launch_step(const Dev& d, const Consts& k, unsigned long long step, cudaStream_t s, cudaEvent_t* ev = nullptr);
 int launch_refresh_cells(const Dev& d, const Consts& k, cudaStream_t s);
+int launch_t1_reset(const Dev& d, const Consts& k, cudaStream_t s);
 int launch_t1_pass_only(const Dev& d, const Consts& k, cudaStream_t s);
 int launch_t1_debug(const Dev& d, const Consts& k, int* cand_pairs, int* win_pairs, long long capacity, cudaStream_t s);
 int launch_compute_forces(const Dev& d, const Consts& k, double2* ap_scratch, double* force_user, double* ap_user, cudaStream_t s);

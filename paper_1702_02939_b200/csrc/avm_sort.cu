@@ -56,11 +56,10 @@ __global__ void cell_keys_kernel(const Dev d, const Consts k, int m, unsigned in
   const int c = blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= k.N) return;
   const int n = d.cvn[c];
-  const int* row = d.cv + (size_t)c * k.S;
-  const double2 h0 = d.pos[row[0]];
+  const double2 h0 = d.pos[row_entry(d.cv, k.N, c, 0)];
   double sx = 0.0, sy = 0.0;
   for (int j = 1; j < n; ++j) {
-    const double2 hj = d.pos[row[j]];
+    const double2 hj = d.pos[row_entry(d.cv, k.N, c, j)];
     sx += min_image(hj.x - h0.x, k.Lx, k.hLx);
     sy += min_image(hj.y - h0.y, k.Ly, k.hLy);
   }
@@ -153,8 +152,8 @@ __global__ void permute_vertices_kernel(const Dev a, const Dev b, const Consts k
   b.vtag[i] = a.vtag[o];
 #pragma unroll
   for (int s = 0; s < 3; ++s) {
-    b.vn[3 * i + s] = newidx_v[a.vn[3 * o + s]];
-    b.vc[3 * i + s] = newidx_c[a.vc[3 * o + s]];
+    b.vn[s * k.Vs + i] = newidx_v[a.vn[s * k.Vs + o]];
+    b.vc[s * k.Vs + i] = newidx_c[a.vc[s * k.Vs + o]];
   }
 }
 
@@ -168,9 +167,15 @@ __global__ void permute_cells_kernel(const Dev a, const Dev b, const Consts k, c
   b.theta[i] = a.theta[o];
   b.rec[i] = a.rec[o];
   b.ctag[i] = a.ctag[o];
-  const int* src = a.cv + (size_t)o * k.S;
-  int* dst = b.cv + (size_t)i * k.S;
-  for (int j = 0; j < k.S; ++j) dst[j] = j < n ? newidx_v[src[j]] : -1;
+  for (int q = 0; q < k.S / 4; ++q) {
+    const int4 src = a.cv[(size_t)q * k.N + o];
+    int4 dst;
+    dst.x = 4 * q + 0 < n ? newidx_v[src.x] : -1;
+    dst.y = 4 * q + 1 < n ? newidx_v[src.y] : -1;
+    dst.z = 4 * q + 2 < n ? newidx_v[src.z] : -1;
+    dst.w = 4 * q + 3 < n ? newidx_v[src.w] : -1;
+    b.cv[(size_t)q * k.N + i] = dst;
+  }
 }
 
 size_t sort_hist_entries(int n) { return (size_t)256 * (size_t)((n + kSeg - 1) / kSeg); }

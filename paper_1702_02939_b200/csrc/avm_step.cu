@@ -2,13 +2,19 @@
 //
 // Paper order of one step (PAPER.md:62-64 §II.B, :104-108 §II.D; R6):
 //   geometry -> forces -> move vertices -> rotate directors -> T1 test/update.
-// Kernel schedule used here:
+// Kernel schedule used here, three launches per step:
 //   force_move   (thread/vertex)  rows a2+a3: F_v from the 3 incident cells' cached (a,p) records
 //                                  and the 3 neighbour positions, Euler step of Eq. 4, wrap.
-//   cell_update  (thread/cell)    rows a4+a1+a5: director noise, then area/perimeter of the MOVED
-//                                  tiling (= the geometry the next step's forces need) and, from
-//                                  the same edge vectors, detection of edges shorter than l_c.
-//   t1_mark / t1_flip / t1_reset  rows a5-a7: eligibility, conflict rule, flip + list rewrite.
+//                                  Prologue: clears the per-cell minimum keys the previous step's
+//                                  T1 candidates left behind.
+//   cell_update  (thread/cell)    rows a4+a1+a5+a6: director noise, then area/perimeter of the MOVED
+//                                  tiling (= the geometry the next step's forces need); edges found
+//                                  shorter than l_c are tested for eligibility by the detecting
+//                                  thread, appended to the candidate list and their key is
+//                                  atomicMin-ed into the four cells (conflict rule, marking half).
+//   t1_flip      (warp/candidate) rows a6+a7: a candidate whose key is the minimum on all four of
+//                                  its cells flips; the warp rewrites the four lists cooperatively
+//                                  and refreshes the four cells' cached geometry.
 // Geometry is thus evaluated once per step on the positions the forces of the following step
 // act on; after a flip the records of its four cells are refreshed in place, so every force is
 // computed from the geometry of the current topology exactly as in the paper's cycle.
@@ -19,7 +25,27 @@ namespace avm {
 static constexpr int kVertexBlock = 256;
 static constexpr int kCellBlock = 128;
 static constexpr int kT1Block = 128;
-static constexpr int kT1Grid = 148 * 4;
+static constexpr int kT1Grid = 148 * 2;
+static constexpr unsigned kFull = 0xffffffffu;
+
+// ---- cache-hinted loads -------------------------------------------------------------------------
+// Pure streams (index lists, tags) are read once per step: evict-first so that they do not push
+// the re-used arrays (positions, cell records) out of L1/L2.
+__device__ __forceinline__ int ld_stream(const int* p) { return __ldcs(p); }
+__device__ __forceinline__ int4 ld_stream(const int4* p) { return __ldcs(p); }
+__device__ __forceinline__ double ld_stream(const double* p) { return __ldcs(p); }
+// one 32-byte record with a single 256-bit load (LDG.E.256, sm_100)
+__device__ __forceinline__ CellRec ld_rec(const CellRec* p) {
+  CellRec r;
+  asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(r.a), "=d"(r.p), "=d"(r.nx), "=d"(r.ny) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void st_rec(CellRec* p, const CellRec& r) {
+  asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(r.a), "d"(r.p), "d"(r.nx), "d"(r.ny) : "memory");
+}
+// |d| >= L/2 decided conservatively on the high word with integer ALU ops (keeps the FP64 pipe
+// for arithmetic); the exact minimum image runs only where this fires.
+__device__ __forceinline__ unsigned may_wrap(double d, unsigned hi_half) { return (hi_word(d) & 0x7fffffffu) >= hi_half; }
 
 // ---------------------------------------------------------------------------------------------
 // rows a2 + a3: vertex forces (Eq. A2-A5) and displacement (Eq. 4, :56).
@@ -30,15 +56,17 @@ static constexpr int kT1Grid = 148 * 4;
 //   F_v = -sum_k [ a_k dA + p_k dP ],  a = 2K_A(A-A0), p = 2K_P(P-P0)  (A2, A3)
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ double2 vertex_force(const double2 h, const double2 q0, const double2 q1,
-                                                const double2 q2, const CellRec c0, const CellRec c1,
-                                                const CellRec c2, const Consts& k) {
-  const double r0x = min_image(q0.x - h.x, k.Lx, k.hLx), r0y = min_image(q0.y - h.y, k.Ly, k.hLy);
-  const double r1x = min_image(q1.x - h.x, k.Lx, k.hLx), r1y = min_image(q1.y - h.y, k.Ly, k.hLy);
-  const double r2x = min_image(q2.x - h.x, k.Lx, k.hLx), r2y = min_image(q2.y - h.y, k.Ly, k.hLy);
-  const double s0 = r0x * r0x + r0y * r0y, s1 = r1x * r1x + r1y * r1y, s2 = r2x * r2x + r2y * r2y;
-  const double i0 = s0 > 0.0 ? rsqrt(s0) : 0.0;   // zero-length edge contributes 0 (R15)
-  const double i1 = s1 > 0.0 ? rsqrt(s1) : 0.0;
-  const double i2 = s2 > 0.0 ? rsqrt(s2) : 0.0;
+                                                const double2 q2, const CellRec& c0, const CellRec& c1,
+                                                const CellRec& c2, const Consts& k) {
+  double r0x = q0.x - h.x, r0y = q0.y - h.y, r1x = q1.x - h.x, r1y = q1.y - h.y, r2x = q2.x - h.x, r2y = q2.y - h.y;
+  const unsigned hx = hi_word(k.hLx), hy = hi_word(k.hLy);
+  if (may_wrap(r0x, hx) | may_wrap(r1x, hx) | may_wrap(r2x, hx) | may_wrap(r0y, hy) | may_wrap(r1y, hy) | may_wrap(r2y, hy)) {
+    r0x = min_image(r0x, k.Lx, k.hLx); r1x = min_image(r1x, k.Lx, k.hLx); r2x = min_image(r2x, k.Lx, k.hLx);
+    r0y = min_image(r0y, k.Ly, k.hLy); r1y = min_image(r1y, k.Ly, k.hLy); r2y = min_image(r2y, k.Ly, k.hLy);
+  }
+  const double i0 = rsqrt_pos(r0x * r0x + r0y * r0y);   // zero-length edge contributes 0 (R15)
+  const double i1 = rsqrt_pos(r1x * r1x + r1y * r1y);
+  const double i2 = rsqrt_pos(r2x * r2x + r2y * r2y);
   const double u0x = r0x * i0, u0y = r0y * i0, u1x = r1x * i1, u1y = r1y * i1, u2x = r2x * i2, u2y = r2y * i2;
   // cell k uses (next, prev) = (r_k, r_{k+1})
   double fx = -0.5 * (c0.a * (r0y - r1y) + c1.a * (r1y - r2y) + c2.a * (r2y - r0y));
@@ -48,243 +76,335 @@ __device__ __forceinline__ double2 vertex_force(const double2 h, const double2 q
   return make_double2(fx, fy);
 }
 
+struct VertexIn { double2 h; int n0, n1, n2, c0, c1, c2; };
+__device__ __forceinline__ VertexIn load_vertex(const Dev& d, const Consts& k, int v) {
+  VertexIn in;
+  in.h = __ldg(d.pos + v);
+  in.n0 = ld_stream(d.vn + v); in.n1 = ld_stream(d.vn + k.Vs + v); in.n2 = ld_stream(d.vn + 2 * k.Vs + v);
+  in.c0 = ld_stream(d.vc + v); in.c1 = ld_stream(d.vc + k.Vs + v); in.c2 = ld_stream(d.vc + 2 * k.Vs + v);
+  return in;
+}
+
+// Persistent grid-stride kernel: each thread keeps the streaming loads of its NEXT vertex in
+// flight while it gathers and computes the current one.
 __global__ void __launch_bounds__(kVertexBlock)
-force_move_kernel(const Dev d, const Consts k) {
-  const int v = blockIdx.x * kVertexBlock + threadIdx.x;
-  if (v == 0) { d.ctr->n_short = 0; d.ctr->n_cand = 0; }   // T1 lists of the previous step are done
+force_move_kernel(const Dev d, const Consts k, const unsigned parity) {
+  const int tid = blockIdx.x * kVertexBlock + threadIdx.x;
+  const int stride = gridDim.x * kVertexBlock;
+  {  // the previous step's T1 candidates are done: clear their cells' minimum keys (row a6)
+    const unsigned prev = d.ctr->n_cand[parity ^ 1u];
+    for (unsigned i = tid; i < prev; i += stride) {
+      const Cand c = d.cand[i];
+      d.minkey[c.cL] = ~0ull; d.minkey[c.cR] = ~0ull; d.minkey[c.cE1] = ~0ull; d.minkey[c.cE2] = ~0ull;
+    }
+    if (tid == 0) d.ctr->n_cand[parity] = 0;
+  }
+  int v = tid;
   if (v >= k.V) return;
-  const double2 h = d.pos[v];
-  const int n0 = d.vn[3 * v], n1 = d.vn[3 * v + 1], n2 = d.vn[3 * v + 2];
-  const int e0 = d.vc[3 * v], e1 = d.vc[3 * v + 1], e2 = d.vc[3 * v + 2];
-  const double2 q0 = d.pos[n0], q1 = d.pos[n1], q2 = d.pos[n2];
-  const CellRec c0 = d.rec[e0], c1 = d.rec[e1], c2 = d.rec[e2];
-  const double2 f = vertex_force(h, q0, q1, q2, c0, c1, c2, k);
-  // Eq. 4: dh/dt = mu F + (v0/3) sum of the three unit directors (R5), directors of the start
-  // of the step (R7); explicit Euler; wrap into the box (R13)
-  const double vx = k.mu * f.x + k.v0_3 * (c0.nx + c1.nx + c2.nx);
-  const double vy = k.mu * f.y + k.v0_3 * (c0.ny + c1.ny + c2.ny);
-  const double x = wrap_box(h.x + k.dt * vx, k.Lx), y = wrap_box(h.y + k.dt * vy, k.Ly);
-  if (!(isfinite(x) && isfinite(y))) atomicOr((unsigned long long*)&d.ctr->error, 1ull);
-  d.pos_next[v] = make_double2(x, y);
+  const unsigned hiLx = hi_word(k.Lx), hiLy = hi_word(k.Ly);
+  VertexIn in = load_vertex(d, k, v);
+  for (;;) {
+    const double2 q0 = __ldg(d.pos + in.n0), q1 = __ldg(d.pos + in.n1), q2 = __ldg(d.pos + in.n2);
+    const CellRec c0 = ld_rec(d.rec + in.c0), c1 = ld_rec(d.rec + in.c1), c2 = ld_rec(d.rec + in.c2);
+    const double2 h = in.h;
+    const int vnext = v + stride;
+    if (vnext < k.V) in = load_vertex(d, k, vnext);
+    const double2 f = vertex_force(h, q0, q1, q2, c0, c1, c2, k);
+    // Eq. 4: dh/dt = mu F + (v0/3) sum of the three unit directors (R5), directors of the start
+    // of the step (R7); explicit Euler; wrap into the box (R13)
+    const double vx = k.mu * f.x + k.v0_3 * (c0.nx + c1.nx + c2.nx);
+    const double vy = k.mu * f.y + k.v0_3 * (c0.ny + c1.ny + c2.ny);
+    double x = h.x + k.dt * vx, y = h.y + k.dt * vy;
+    // negative, >= L (conservatively) and non-finite values all have a large unsigned high word
+    if ((hi_word(x) >= hiLx) | (hi_word(y) >= hiLy)) {
+      x = wrap_box(x, k.Lx); y = wrap_box(y, k.Ly);
+      if (!(isfinite(x) && isfinite(y))) atomicOr((unsigned long long*)&d.ctr->error, 1ull);
+    }
+    d.pos_next[v] = make_double2(x, y);
+    if (vnext >= k.V) break;
+    v = vnext;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// rows a5 (eligibility, R10) + a6 (marking half of the conflict rule, R11) for ONE short edge,
+// run by the thread that found it.  (va, vb) are current vertex indices.  Cold path.
+// ---------------------------------------------------------------------------------------------
+__device__ __noinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va, int vb, unsigned parity, bool count_stats) {
+  // canonical test (R9): strict l < l_c on the minimum-image separation of the two endpoints
+  const double2 ha = d.pos[va], hb = d.pos[vb];
+  const double dx = min_image(hb.x - ha.x, k.Lx, k.hLx), dy = min_image(hb.y - ha.y, k.Ly, k.hLy);
+  if (!(dx * dx + dy * dy < k.lc2)) return;
+  if (count_stats) atomicAdd((unsigned long long*)&d.ctr->t1_short, 1ull);
+  int v1 = va, v2 = vb;
+  unsigned int t1 = (unsigned int)d.vtag[v1], t2 = (unsigned int)d.vtag[v2];
+  if (t1 > t2) { int tv = v1; v1 = v2; v2 = tv; unsigned int tt = t1; t1 = t2; t2 = tt; }
+  int k1 = 0, k2 = 0;
+#pragma unroll
+  for (int s = 0; s < 3; ++s) {
+    if (d.vn[s * k.Vs + v1] == v2) k1 = s;
+    if (d.vn[s * k.Vs + v2] == v1) k2 = s;
+  }
+  // cyclic from the partner's slot the cells of u are (C0, C1, C2); C0 is left of u -> partner
+  const int cL = d.vc[k1 * k.Vs + v1], cE1 = d.vc[((k1 + 1) % 3) * k.Vs + v1];
+  const int cR = d.vc[k2 * k.Vs + v2], cE2 = d.vc[((k2 + 1) % 3) * k.Vs + v2];
+  const bool distinct = cL != cR && cL != cE1 && cL != cE2 && cR != cE1 && cR != cE2 && cE1 != cE2;
+  if (!distinct) return;
+  if (!(d.cvn[cL] > 3 && d.cvn[cR] > 3)) return;               // no 2-gons (T2 absent)
+  if (!(d.cvn[cE1] < k.S && d.cvn[cE2] < k.S)) {               // row would exceed the stride
+    if (count_stats) {
+      atomicAdd((unsigned long long*)&d.ctr->overflow_rejects, 1ull);
+      atomicOr((unsigned long long*)&d.ctr->error, 2ull);
+    }
+    return;
+  }
+  Cand cd;
+  cd.v1 = v1; cd.v2 = v2; cd.k1 = k1; cd.k2 = k2;
+  cd.cL = cL; cd.cR = cR; cd.cE1 = cE1; cd.cE2 = cE2;
+  cd.key = ((unsigned long long)t1 << 32) | t2;
+  cd.pad = 0;
+  const unsigned int slot = atomicAdd(&d.ctr->n_cand[parity], 1u);
+  d.cand[slot] = cd;
+  atomicMin(&d.minkey[cL], cd.key);
+  atomicMin(&d.minkey[cR], cd.key);
+  atomicMin(&d.minkey[cE1], cd.key);
+  atomicMin(&d.minkey[cE2], cd.key);
+}
+
+// The geometry pass flagged edges of cell c (bit j-1 = the edge ending at row entry j, j = n
+// being the closing edge) as possibly short.  Each edge is seen by its two cells in opposite
+// directions: it is reported from the cell that traverses it from the smaller to the larger
+// (current) vertex index.
+__device__ __noinline__ void t1_report_cell(const Dev& d, const Consts& k, int c, int n, unsigned smask, unsigned parity) {
+  while (smask) {
+    const int j = __ffs(smask);     // edge (j-1) -> (j mod n)
+    smask &= smask - 1u;
+    const int va = row_entry(d.cv, k.N, c, j - 1), vb = row_entry(d.cv, k.N, c, j == n ? 0 : j);
+    if (va < vb) t1_mark_edge(d, k, va, vb, parity, true);
+  }
 }
 
 // ---------------------------------------------------------------------------------------------
 // rows a4 + a1 + a5: director update (R8, R16), geometry of the moved tiling
 // (R14) and short-edge detection (R9).
-// `pos` is the position buffer AFTER the move.  kUpdateTheta = false gives the plain geometry
-// refresh used at creation / after avm_set_positions.
+// d.pos is the position buffer AFTER the move.  kStep = false gives the plain geometry refresh
+// used at creation / after avm_set_positions (no noise, no detection).
+//
+// One thread per cell.  Row entries 0..7 come from planes 0 and 1 (two coalesced 128-bit loads);
+// their positions are gathered with up to eight independent predicated 128-bit loads, and the
+// director arithmetic (Philox, Box-Muller, sincos) is placed between issuing those gathers and
+// consuming them.  Entries beyond the cell's n are treated as copies of entry 0 (r = 0): the
+// edge into the first of them is the closing edge and the rest are exact no-ops, so the edge
+// loop has a fixed trip count and no divergent exits.  Planes 2.. are visited only by warps that
+// hold a cell with more than 8 vertices.
+// Cells are walked in DESCENDING index order while force_move walks vertices in ascending order,
+// so each pass starts on the lines the previous pass touched last (L2 recency).
 // ---------------------------------------------------------------------------------------------
-template <bool kUpdateTheta, bool kDetect>
+template <bool kStep>
 __global__ void __launch_bounds__(kCellBlock)
-cell_update_kernel(const Dev d, const double2* __restrict__ pos, const Consts k, const unsigned long long step) {
-  const int c = blockIdx.x * kCellBlock + threadIdx.x;
-  if (c >= k.N) return;
-  const int n = d.cvn[c];
-  double th = d.theta[c];
-  if (kUpdateTheta) {
-    th += k.amp * director_noise(k.seed, step, (unsigned long long)(unsigned int)d.ctag[c]);
-    d.theta[c] = th;
+cell_update_kernel(const Dev d, const Consts k, const unsigned long long step, const unsigned parity) {
+  const int gid = blockIdx.x * kCellBlock + threadIdx.x;
+  const bool valid = gid < k.N;
+  const int c = valid ? k.N - 1 - gid : 0;
+  const double2* __restrict__ pos = d.pos;
+  const int n = valid ? ld_stream(d.cvn + c) : 0;
+  const int4 qa = ld_stream(d.cv + c), qb = ld_stream(d.cv + k.N + c);
+  const int e[8] = {qa.x, qa.y, qa.z, qa.w, qb.x, qb.y, qb.z, qb.w};
+  double th = ld_stream(d.theta + c);
+  const unsigned int tag = (unsigned int)ld_stream(d.ctag + c);
+  double2 h[8];
+  h[0] = __ldg(pos + e[0]);
+#pragma unroll
+  for (int j = 1; j < 8; ++j) {
+    h[j] = make_double2(0.0, 0.0);
+    if (j < n) h[j] = __ldg(pos + e[j]);
+  }
+  // ---- director (independent of the gathers above) ----
+  if (kStep) {
+    th += k.amp * director_noise(k.seed, step, (unsigned long long)tag);
+    if (valid) d.theta[c] = th;
   }
   double sn, cs;
   sincos(th, &sn, &cs);
-
-  const int4* row4 = reinterpret_cast<const int4*>(d.cv + (size_t)c * k.S);
-  double acc = 0.0, per = 0.0;
-  double rxp = 0.0, ryp = 0.0;
-  int4 q = row4[0];
-  const int first = q.x;
-  int vprev = first;
-  const double2 h0 = pos[first];
-  for (int j = 1; j <= n; ++j) {
-    if ((j & 3) == 0 && j < n) q = row4[j >> 2];
-    const int sel = j & 3;
-    int vj = sel == 0 ? q.x : sel == 1 ? q.y : sel == 2 ? q.z : q.w;
-    double rx = 0.0, ry = 0.0;
-    if (j < n) {
-      const double2 hj = pos[vj];
-      rx = min_image(hj.x - h0.x, k.Lx, k.hLx);
-      ry = min_image(hj.y - h0.y, k.Ly, k.hLy);
-    } else {
-      vj = first;
-    }
-    acc += rxp * ry - ryp * rx;
-    const double dx = rx - rxp, dy = ry - ryp;
-    const double l2 = dx * dx + dy * dy;
-    per += sqrt(l2);
-    if (kDetect) {
-      // each edge is seen by its two cells in opposite directions: report it from the cell that
-      // traverses it from the smaller to the larger (current) vertex index
-      if (l2 < k.lc2 && vprev < vj) {
-        const unsigned int slot = atomicAdd(&d.ctr->n_short, 1u);
-        d.short_list[slot] = make_int2(vprev, vj);
-      }
-    }
-    rxp = rx; ryp = ry; vprev = vj;
+  // ---- unwrap relative to entry 0 (R14) ----
+  const unsigned hx = hi_word(k.hLx), hy = hi_word(k.hLy), hlc = hi_word(k.lc2);
+  double rx[8], ry[8];
+  unsigned wrapf = 0;
+#pragma unroll
+  for (int j = 1; j < 8; ++j) {
+    rx[j] = j < n ? __dsub_rn(h[j].x, h[0].x) : 0.0;
+    ry[j] = j < n ? __dsub_rn(h[j].y, h[0].y) : 0.0;
+    wrapf |= may_wrap(rx[j], hx) | may_wrap(ry[j], hy);
   }
+  if (wrapf) {
+#pragma unroll
+    for (int j = 1; j < 8; ++j) { rx[j] = min_image(rx[j], k.Lx, k.hLx); ry[j] = min_image(ry[j], k.Ly, k.hLy); }
+  }
+  // ---- shoelace + perimeter, edges ending at entries 1..7 ----
+  double acc = 0.0, per = 0.0, rxp = 0.0, ryp = 0.0;
+  unsigned smask = 0;
+#pragma unroll
+  for (int j = 1; j < 8; ++j) {
+    const double l2 = geom_edge(rxp, ryp, rx[j], ry[j], acc, per);
+    if (kStep && hi_word(l2) <= hlc && j <= n) smask |= 1u << (j - 1);
+    rxp = rx[j]; ryp = ry[j];
+  }
+  // ---- entries 8.. (planes 2..), only in warps that hold such a cell ----
+  for (int q = 2;; ++q) {
+    const int j0 = 4 * q;
+    if (!(j0 < k.S && __any_sync(kFull, n > j0))) {
+      const double l2 = geom_edge(rxp, ryp, 0.0, 0.0, acc, per);     // closing edge of an n == j0 cell
+      if (kStep && hi_word(l2) <= hlc && j0 <= n) smask |= 1u << (j0 - 1);
+      break;
+    }
+    int4 qq = make_int4(0, 0, 0, 0);
+    if (n > j0) qq = d.cv[(size_t)q * k.N + c];
+    const int ee[4] = {qq.x, qq.y, qq.z, qq.w};
+    double2 hh[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      hh[i] = make_double2(0.0, 0.0);
+      if (j0 + i < n) hh[i] = __ldg(pos + ee[i]);
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      double x = 0.0, y = 0.0;
+      if (j0 + i < n) {
+        x = min_image(__dsub_rn(hh[i].x, h[0].x), k.Lx, k.hLx);
+        y = min_image(__dsub_rn(hh[i].y, h[0].y), k.Ly, k.hLy);
+      }
+      const double l2 = geom_edge(rxp, ryp, x, y, acc, per);
+      if (kStep && hi_word(l2) <= hlc && j0 + i <= n) smask |= 1u << (j0 + i - 1);
+      rxp = x; ryp = y;
+    }
+  }
+  if (!valid) return;
   CellRec r;
-  r.a = k.KA2 * (0.5 * acc - k.A0);
+  r.a = k.KA2 * (__dmul_rn(0.5, acc) - k.A0);
   r.p = k.KP2 * (per - k.P0);
   r.nx = cs; r.ny = sn;
-  d.rec[c] = r;
+  st_rec(d.rec + c, r);
+  if (kStep && smask) t1_report_cell(d, k, c, n, smask, parity);
 }
 
 // Detection alone (test hooks avm_t1_pass / avm_debug_t1): thread per vertex, edge owned by the
 // smaller current index.
-__global__ void detect_short_edges_kernel(const Dev d, const Consts k) {
+__global__ void detect_mark_kernel(const Dev d, const Consts k, const unsigned parity, const bool count_stats) {
   const int v = blockIdx.x * blockDim.x + threadIdx.x;
   if (v >= k.V) return;
-  const double2 h = d.pos[v];
   for (int s = 0; s < 3; ++s) {
-    const int w = d.vn[3 * v + s];
-    if (v < w) {
-      const double2 q = d.pos[w];
-      const double dx = min_image(q.x - h.x, k.Lx, k.hLx), dy = min_image(q.y - h.y, k.Ly, k.hLy);
-      if (dx * dx + dy * dy < k.lc2) {
-        const unsigned int slot = atomicAdd(&d.ctr->n_short, 1u);
-        d.short_list[slot] = make_int2(v, w);
-      }
-    }
+    const int w = d.vn[s * k.Vs + v];
+    if (v < w) t1_mark_edge(d, k, v, w, parity, count_stats);
   }
 }
 
-__global__ void zero_counts_kernel(const Dev d) { d.ctr->n_short = 0; d.ctr->n_cand = 0; d.ctr->n_win = 0; }
-
 // ---------------------------------------------------------------------------------------------
-// rows a5 (eligibility) + a6 (conflict rule): R10, R11.
-// ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kT1Block)
-t1_mark_kernel(const Dev d, const Consts k, const bool count_stats) {
-  const unsigned int n_short = d.ctr->n_short;
-  if (count_stats && blockIdx.x == 0 && threadIdx.x == 0) d.ctr->t1_short += n_short;
-  for (unsigned int i = blockIdx.x * kT1Block + threadIdx.x; i < n_short; i += gridDim.x * kT1Block) {
-    const int2 e = d.short_list[i];
-    int v1 = e.x, v2 = e.y;
-    unsigned int t1 = (unsigned int)d.vtag[v1], t2 = (unsigned int)d.vtag[v2];
-    if (t1 > t2) { int tv = v1; v1 = v2; v2 = tv; unsigned int tt = t1; t1 = t2; t2 = tt; }
-    int k1 = 0, k2 = 0;
-#pragma unroll
-    for (int s = 0; s < 3; ++s) {
-      if (d.vn[3 * v1 + s] == v2) k1 = s;
-      if (d.vn[3 * v2 + s] == v1) k2 = s;
-    }
-    // cyclic from the partner's slot the cells of u are (C0, C1, C2); C0 is left of u -> partner
-    const int cL = d.vc[3 * v1 + k1], cE1 = d.vc[3 * v1 + (k1 + 1) % 3];
-    const int cR = d.vc[3 * v2 + k2], cE2 = d.vc[3 * v2 + (k2 + 1) % 3];
-    const bool distinct = cL != cR && cL != cE1 && cL != cE2 && cR != cE1 && cR != cE2 && cE1 != cE2;
-    if (!distinct) continue;
-    if (!(d.cvn[cL] > 3 && d.cvn[cR] > 3)) continue;             // no 2-gons (T2 absent)
-    if (!(d.cvn[cE1] < k.S && d.cvn[cE2] < k.S)) {               // row would exceed the stride
-      if (count_stats) {
-        atomicAdd((unsigned long long*)&d.ctr->overflow_rejects, 1ull);
-        atomicOr((unsigned long long*)&d.ctr->error, 2ull);
-      }
-      continue;
-    }
-    Cand cd;
-    cd.v1 = v1; cd.v2 = v2; cd.k1 = k1; cd.k2 = k2;
-    cd.cL = cL; cd.cR = cR; cd.cE1 = cE1; cd.cE2 = cE2;
-    cd.key = ((unsigned long long)t1 << 32) | t2;
-    cd.pad = 0;
-    const unsigned int slot = atomicAdd(&d.ctr->n_cand, 1u);
-    d.cand[slot] = cd;
-    atomicMin(&d.minkey[cL], cd.key);
-    atomicMin(&d.minkey[cR], cd.key);
-    atomicMin(&d.minkey[cE1], cd.key);
-    atomicMin(&d.minkey[cE2], cd.key);
-  }
-}
-
-__device__ __forceinline__ void row_delete(int* __restrict__ row, int* __restrict__ cvn_c, int v) {
-  const int n = *cvn_c;
-  int j = 0;
-  while (j < n && row[j] != v) ++j;
-  for (int t = j; t + 1 < n; ++t) row[t] = row[t + 1];
-  row[n - 1] = -1;
-  *cvn_c = n - 1;
-}
-__device__ __forceinline__ void row_insert_after(int* __restrict__ row, int* __restrict__ cvn_c, int after, int v) {
-  const int n = *cvn_c;
-  int j = 0;
-  while (j < n && row[j] != after) ++j;
-  for (int t = n; t > j + 1; --t) row[t] = row[t - 1];
-  row[j + 1] = v;
-  *cvn_c = n + 1;
-}
-
-// ---------------------------------------------------------------------------------------------
-// row a7: flip + rewrite (R9 geometry, R12 lists).  A candidate flips iff its key is the minimum
-// recorded on all four of its cells (R11); winners therefore own disjoint cell quadruples and
-// every word written below belongs to a vertex or row inside the winner's own quadruple.
+// rows a6 (deciding half) + a7: flip + rewrite (R9 geometry, R12 lists), one WARP per candidate.
+// A candidate flips iff its key is the minimum recorded on all four of its cells (R11); winners
+// therefore own disjoint cell quadruples and every word written below belongs to a vertex or row
+// inside the winner's own quadruple.  minkey is only read here (cleared by the next force_move).
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kT1Block)
-t1_flip_kernel(const Dev d, const Consts k) {
-  const unsigned int n_cand = d.ctr->n_cand;
+t1_flip_kernel(const Dev d, const Consts k, const unsigned parity, const bool count_stats) {
+  const unsigned int n_cand = d.ctr->n_cand[parity];
+  const int lane = threadIdx.x & 31;
+  const unsigned gwarp = (blockIdx.x * kT1Block + threadIdx.x) >> 5, nwarps = (gridDim.x * kT1Block) >> 5;
+  if (count_stats && gwarp == 0 && lane == 0 && n_cand) atomicAdd((unsigned long long*)&d.ctr->t1_candidates, (unsigned long long)n_cand);
   unsigned int flips = 0, blocked = 0;
-  for (unsigned int i = blockIdx.x * kT1Block + threadIdx.x; i < n_cand; i += gridDim.x * kT1Block) {
+  for (unsigned int i = gwarp; i < n_cand; i += nwarps) {
     const Cand c = d.cand[i];
-    const bool win = d.minkey[c.cL] == c.key && d.minkey[c.cR] == c.key && d.minkey[c.cE1] == c.key &&
-                     d.minkey[c.cE2] == c.key;
-    if (!win) { ++blocked; continue; }
+    const int cells[4] = {c.cL, c.cR, c.cE1, c.cE2};
+    const int l4 = lane & 3;
+    const unsigned long long mk = d.minkey[l4 == 0 ? c.cL : l4 == 1 ? c.cR : l4 == 2 ? c.cE1 : c.cE2];
+    if (!__all_sync(kFull, mk == c.key)) { ++blocked; continue; }
     ++flips;
     const int v1 = c.v1, v2 = c.v2, k1 = c.k1, k2 = c.k2;
-    // geometry: rigid counter-clockwise quarter turn about the midpoint, new length 1.5 l_c (R9)
+    const int a1 = (k1 + 1) % 3, b1 = (k1 + 2) % 3, a2 = (k2 + 1) % 3, b2 = (k2 + 2) % 3;
+    // ---- everything is read before anything is written ----
     const double2 h1 = d.pos[v1], h2 = d.pos[v2];
+    const int x1 = d.vn[a1 * k.Vs + v1], y1 = d.vn[b1 * k.Vs + v1];
+    const int x2 = d.vn[a2 * k.Vs + v2], y2 = d.vn[b2 * k.Vs + v2];
+    int row[4], nrow[4];
+#pragma unroll
+    for (int t = 0; t < 4; ++t) {
+      nrow[t] = d.cvn[cells[t]];
+      row[t] = lane < k.S ? row_entry(d.cv, k.N, cells[t], lane) : -1;
+    }
+    int outer = -1;   // lanes 0-2: slots of x1, lanes 3-5: slots of x2
+    if (lane < 3) outer = d.vn[lane * k.Vs + x1];
+    else if (lane < 6) outer = d.vn[(lane - 3) * k.Vs + x2];
+    // ---- geometry: rigid counter-clockwise quarter turn about the midpoint, new length 1.5 l_c (R9)
     const double dx = min_image(h2.x - h1.x, k.Lx, k.hLx), dy = min_image(h2.y - h1.y, k.Ly, k.hLy);
     const double l = sqrt(dx * dx + dy * dy);
     const double mx = h1.x + 0.5 * dx, my = h1.y + 0.5 * dy;
     double px = 0.0, py = 1.0;
     if (l > 0.0) { px = -dy / l; py = dx / l; }
     const double half = 0.75 * k.lc;
-    d.pos[v2] = make_double2(wrap_box(mx + half * px, k.Lx), wrap_box(my + half * py, k.Ly));
-    d.pos[v1] = make_double2(wrap_box(mx - half * px, k.Lx), wrap_box(my - half * py, k.Ly));
-    // lists: u = ([w, x, y]; [C0, C1, C2]) cyclic from the partner slot
-    //     -> ([w, y, z]; [C1, C2, C']), z = partner's old x, C' = partner's old C1 (R12)
-    const int a1 = (k1 + 1) % 3, b1 = (k1 + 2) % 3, a2 = (k2 + 1) % 3, b2 = (k2 + 2) % 3;
-    const int x1 = d.vn[3 * v1 + a1], y1 = d.vn[3 * v1 + b1];
-    const int x2 = d.vn[3 * v2 + a2], y2 = d.vn[3 * v2 + b2];
-    d.vn[3 * v1 + a1] = y1; d.vn[3 * v1 + b1] = x2;
-    d.vc[3 * v1 + k1] = c.cE1; d.vc[3 * v1 + a1] = c.cR; d.vc[3 * v1 + b1] = c.cE2;
-    d.vn[3 * v2 + a2] = y2; d.vn[3 * v2 + b2] = x1;
-    d.vc[3 * v2 + k2] = c.cE2; d.vc[3 * v2 + a2] = c.cL; d.vc[3 * v2 + b2] = c.cE1;
-#pragma unroll
-    for (int s = 0; s < 3; ++s) {
-      if (d.vn[3 * x1 + s] == v1) d.vn[3 * x1 + s] = v2;
+    if (lane == 0) {
+      d.pos[v2] = make_double2(wrap_box(mx + half * px, k.Lx), wrap_box(my + half * py, k.Ly));
+      d.pos[v1] = make_double2(wrap_box(mx - half * px, k.Lx), wrap_box(my - half * py, k.Ly));
+      // lists: u = ([w, x, y]; [C0, C1, C2]) cyclic from the partner slot
+      //     -> ([w, y, z]; [C1, C2, C']), z = partner's old x, C' = partner's old C1 (R12)
+      d.vn[a1 * k.Vs + v1] = y1; d.vn[b1 * k.Vs + v1] = x2;
+      d.vc[k1 * k.Vs + v1] = c.cE1; d.vc[a1 * k.Vs + v1] = c.cR; d.vc[b1 * k.Vs + v1] = c.cE2;
+      d.vn[a2 * k.Vs + v2] = y2; d.vn[b2 * k.Vs + v2] = x1;
+      d.vc[k2 * k.Vs + v2] = c.cE2; d.vc[a2 * k.Vs + v2] = c.cL; d.vc[b2 * k.Vs + v2] = c.cE1;
     }
+    // outer vertices: x1 was joined to v1 and is now joined to v2 (same slot); x2 likewise
+    if (lane < 3 && outer == v1) d.vn[lane * k.Vs + x1] = v2;
+    if (lane >= 3 && lane < 6 && outer == v2) d.vn[(lane - 3) * k.Vs + x2] = v1;
+    // rows: L deletes v1, R deletes v2 (later entries shift down)
 #pragma unroll
-    for (int s = 0; s < 3; ++s) {
-      if (d.vn[3 * x2 + s] == v2) d.vn[3 * x2 + s] = v1;
+    for (int t = 0; t < 2; ++t) {
+      const int victim = t == 0 ? v1 : v2;
+      const int p = __ffs(__ballot_sync(kFull, lane < nrow[t] && row[t] == victim)) - 1;
+      const int nxt = __shfl_down_sync(kFull, row[t], 1);
+      if (lane >= p && lane < nrow[t]) row_entry(d.cv, k.N, cells[t], lane) = lane == nrow[t] - 1 ? -1 : nxt;
+      if (lane == 0) d.cvn[cells[t]] = nrow[t] - 1;
     }
-    row_delete(d.cv + (size_t)c.cL * k.S, d.cvn + c.cL, v1);
-    row_delete(d.cv + (size_t)c.cR * k.S, d.cvn + c.cR, v2);
-    row_insert_after(d.cv + (size_t)c.cE1 * k.S, d.cvn + c.cE1, v1, v2);
-    row_insert_after(d.cv + (size_t)c.cE2 * k.S, d.cvn + c.cE2, v2, v1);
-    // refresh the cached geometry of the four cells (directors unchanged)
-    const int cells[4] = {c.cL, c.cR, c.cE1, c.cE2};
+    // E1 inserts v2 immediately after v1, E2 inserts v1 immediately after v2 (later entries shift up)
 #pragma unroll
-    for (int t = 0; t < 4; ++t) {
+    for (int t = 2; t < 4; ++t) {
+      const int after = t == 2 ? v1 : v2, ins = t == 2 ? v2 : v1;
+      const int p = __ffs(__ballot_sync(kFull, lane < nrow[t] && row[t] == after)) - 1;
+      const int prv = __shfl_up_sync(kFull, row[t], 1);
+      if (lane > p && lane <= nrow[t]) row_entry(d.cv, k.N, cells[t], lane) = lane == p + 1 ? ins : prv;
+      if (lane == 0) d.cvn[cells[t]] = nrow[t] + 1;
+    }
+    __syncwarp();
+    // refresh the cached geometry of the four cells (directors unchanged); same serial sum as
+    // the per-step pass so that a resumed run reproduces these records bit for bit
+    if (lane < 4) {
+      const int cc = lane == 0 ? c.cL : lane == 1 ? c.cR : lane == 2 ? c.cE1 : c.cE2;
       double A, P;
-      cell_area_perimeter(d.pos, d.cv + (size_t)cells[t] * k.S, d.cvn[cells[t]], k, A, P);
-      d.rec[cells[t]].a = k.KA2 * (A - k.A0);
-      d.rec[cells[t]].p = k.KP2 * (P - k.P0);
+      cell_area_perimeter(d.pos, d.cv, cc, d.cvn[cc], k, A, P);
+      d.rec[cc].a = k.KA2 * (A - k.A0);
+      d.rec[cc].p = k.KP2 * (P - k.P0);
     }
+    __syncwarp();
   }
-  if (flips) atomicAdd((unsigned long long*)&d.ctr->t1_flips, (unsigned long long)flips);
-  if (blocked) atomicAdd((unsigned long long*)&d.ctr->t1_blocked, (unsigned long long)blocked);
+  if (count_stats && lane == 0) {
+    if (flips) atomicAdd((unsigned long long*)&d.ctr->t1_flips, (unsigned long long)flips);
+    if (blocked) atomicAdd((unsigned long long*)&d.ctr->t1_blocked, (unsigned long long)blocked);
+  }
 }
 
+// Clears the minimum keys of both candidate lists and empties them (before a re-sort, around the
+// test hooks).  Inside avm_step this work rides in force_move's prologue instead.
 __global__ void __launch_bounds__(kT1Block)
-t1_reset_kernel(const Dev d, const bool count_stats) {
-  const unsigned int n_cand = d.ctr->n_cand;
-  if (count_stats && blockIdx.x == 0 && threadIdx.x == 0) d.ctr->t1_candidates += n_cand;
-  for (unsigned int i = blockIdx.x * kT1Block + threadIdx.x; i < n_cand; i += gridDim.x * kT1Block) {
+t1_reset_kernel(const Dev d) {
+  const unsigned n0 = d.ctr->n_cand[0], n1 = d.ctr->n_cand[1];
+  const unsigned n = n0 > n1 ? n0 : n1;
+  for (unsigned int i = blockIdx.x * kT1Block + threadIdx.x; i < n; i += gridDim.x * kT1Block) {
     const Cand c = d.cand[i];
     d.minkey[c.cL] = ~0ull; d.minkey[c.cR] = ~0ull; d.minkey[c.cE1] = ~0ull; d.minkey[c.cE2] = ~0ull;
   }
 }
+__global__ void zero_counts_kernel(const Dev d) { d.ctr->n_cand[0] = 0; d.ctr->n_cand[1] = 0; d.ctr->n_win = 0; }
 
 // debug hook: winners without flipping; (tag_min, tag_max) pairs out
 __global__ void t1_debug_kernel(const Dev d, int* cand_pairs, int* win_pairs, long long capacity) {
-  const unsigned int n_cand = d.ctr->n_cand;
+  const unsigned int n_cand = d.ctr->n_cand[0];
   for (unsigned int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_cand; i += gridDim.x * blockDim.x) {
     const Cand c = d.cand[i];
     if (cand_pairs && i < capacity) {
@@ -312,7 +432,7 @@ __global__ void geometry_kernel(const Dev d, const Consts k, double2* __restrict
   const int c = blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= k.N) return;
   double A, P;
-  cell_area_perimeter(d.pos, d.cv + (size_t)c * k.S, d.cvn[c], k, A, P);
+  cell_area_perimeter(d.pos, d.cv, c, d.cvn[c], k, A, P);
   ap[c] = make_double2(A, P);
   if (ap_user) {
     const int t = d.ctag[c];
@@ -328,8 +448,8 @@ __global__ void forces_kernel(const Dev d, const Consts k, const double2* __rest
   double2 q[3];
 #pragma unroll
   for (int s = 0; s < 3; ++s) {
-    q[s] = d.pos[d.vn[3 * v + s]];
-    const double2 a = ap[d.vc[3 * v + s]];
+    q[s] = d.pos[d.vn[s * k.Vs + v]];
+    const double2 a = ap[d.vc[s * k.Vs + v]];
     c[s].a = k.KA2 * (a.x - k.A0); c[s].p = k.KP2 * (a.y - k.P0); c[s].nx = 0.0; c[s].ny = 0.0;
   }
   const double2 f = vertex_force(h, q[0], q[1], q[2], c[0], c[1], c[2], k);
@@ -344,7 +464,7 @@ __global__ void energy_partial_kernel(const Dev d, const Consts k, double* __res
   double e = 0.0;
   for (int c = blockIdx.x * 256 + threadIdx.x; c < k.N; c += gridDim.x * 256) {
     double A, P;
-    cell_area_perimeter(d.pos, d.cv + (size_t)c * k.S, d.cvn[c], k, A, P);
+    cell_area_perimeter(d.pos, d.cv, c, d.cvn[c], k, A, P);
     e += k.KA * (A - k.A0) * (A - k.A0) + k.KP * (P - k.P0) * (P - k.P0);
   }
   sm[threadIdx.x] = e;
@@ -379,48 +499,60 @@ __global__ void philox_words_kernel(unsigned long long seed, unsigned long long 
 // ---------------------------------------------------------------------------------------------
 static inline int cdiv(long long a, int b) { return (int)((a + b - 1) / b); }
 
+static int force_move_grid(const Consts& k) {
+  // persistent: a whole number of CTAs per SM (148 SMs), never more CTAs than there is work
+  static int per_sm = 0;
+  if (!per_sm) {
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, force_move_kernel, kVertexBlock, 0);
+    if (per_sm < 1) per_sm = 1;
+  }
+  const int want = cdiv(k.V, kVertexBlock);
+  const int cap = 148 * per_sm;
+  return want < cap ? want : cap;
+}
+
 // One timestep.  d.pos = positions at the start of the step, d.pos_next = buffer for the moved
 // positions (the caller swaps them afterwards).
-// ev (optional, 6 events): recorded before/after each kernel by avm_step_profile.
+// ev (optional, AVM_K_COUNT+1 events): recorded before/after each kernel by avm_step_profile.
 int launch_step(const Dev& d, const Consts& k, unsigned long long step, cudaStream_t s, cudaEvent_t* ev) {
+  const unsigned parity = (unsigned)(step & 1ull);
   if (ev) cudaEventRecord(ev[0], s);
-  force_move_kernel<<<cdiv(k.V, kVertexBlock), kVertexBlock, 0, s>>>(d, k);
+  force_move_kernel<<<force_move_grid(k), kVertexBlock, 0, s>>>(d, k, parity);
   if (ev) cudaEventRecord(ev[1], s);
   Dev m = d;                      // from here on the moved positions are "the" positions
   m.pos = d.pos_next; m.pos_next = d.pos;
-  cell_update_kernel<true, true><<<cdiv(k.N, kCellBlock), kCellBlock, 0, s>>>(m, m.pos, k, step);
+  cell_update_kernel<true><<<cdiv(k.N, kCellBlock), kCellBlock, 0, s>>>(m, k, step, parity);
   if (ev) cudaEventRecord(ev[2], s);
-  t1_mark_kernel<<<kT1Grid, kT1Block, 0, s>>>(m, k, true);
+  t1_flip_kernel<<<kT1Grid, kT1Block, 0, s>>>(m, k, parity, true);
   if (ev) cudaEventRecord(ev[3], s);
-  t1_flip_kernel<<<kT1Grid, kT1Block, 0, s>>>(m, k);
-  if (ev) cudaEventRecord(ev[4], s);
-  t1_reset_kernel<<<kT1Grid, kT1Block, 0, s>>>(m, true);
-  if (ev) cudaEventRecord(ev[5], s);
-  return 5;
+  return 3;
 }
 
 int launch_refresh_cells(const Dev& d, const Consts& k, cudaStream_t s) {
-  cell_update_kernel<false, false><<<cdiv(k.N, kCellBlock), kCellBlock, 0, s>>>(d, d.pos, k, 0ull);
+  cell_update_kernel<false><<<cdiv(k.N, kCellBlock), kCellBlock, 0, s>>>(d, k, 0ull, 0u);
   return 1;
 }
 
+// leaves minkey all-idle and both candidate lists empty
+int launch_t1_reset(const Dev& d, const Consts& k, cudaStream_t s) {
+  t1_reset_kernel<<<kT1Grid, kT1Block, 0, s>>>(d);
+  zero_counts_kernel<<<1, 1, 0, s>>>(d);
+  return 2;
+}
+
 int launch_t1_pass_only(const Dev& d, const Consts& k, cudaStream_t s) {
-  zero_counts_kernel<<<1, 1, 0, s>>>(d);
-  detect_short_edges_kernel<<<cdiv(k.V, 256), 256, 0, s>>>(d, k);
-  t1_mark_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, k, true);
-  t1_flip_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, k);
-  t1_reset_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, true);
-  zero_counts_kernel<<<1, 1, 0, s>>>(d);
-  return 6;
+  int n = launch_t1_reset(d, k, s);
+  detect_mark_kernel<<<cdiv(k.V, 256), 256, 0, s>>>(d, k, 0u, true);
+  t1_flip_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, k, 0u, true);
+  n += 2;
+  return n + launch_t1_reset(d, k, s);
 }
 
 int launch_t1_debug(const Dev& d, const Consts& k, int* cand_pairs, int* win_pairs, long long capacity, cudaStream_t s) {
-  zero_counts_kernel<<<1, 1, 0, s>>>(d);
-  detect_short_edges_kernel<<<cdiv(k.V, 256), 256, 0, s>>>(d, k);
-  t1_mark_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, k, false);
+  int n = launch_t1_reset(d, k, s);
+  detect_mark_kernel<<<cdiv(k.V, 256), 256, 0, s>>>(d, k, 0u, false);
   t1_debug_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, cand_pairs, win_pairs, capacity);
-  t1_reset_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, false);
-  return 5;
+  return n + 2;   // the caller reads the counters, then calls launch_t1_reset
 }
 
 int launch_compute_forces(const Dev& d, const Consts& k, double2* ap_scratch, double* force_user, double* ap_user, cudaStream_t s) {
