@@ -202,7 +202,8 @@ __device__ __noinline__ void t1_report_cell(const Dev& d, const Consts& k, int c
 // ---------------------------------------------------------------------------------------------
 template <bool kStep>
 __global__ void __launch_bounds__(kCellBlock)
-cell_update_kernel(const Dev d, const Consts k, const unsigned long long step, const unsigned parity) {
+cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, const unsigned long long step,
+                   const unsigned parity) {
   const int gid = blockIdx.x * kCellBlock + threadIdx.x;
   const bool valid = gid < k.N;
   const int c = valid ? k.N - 1 - gid : 0;
@@ -289,7 +290,8 @@ cell_update_kernel(const Dev d, const Consts k, const unsigned long long step, c
 
 // Detection alone (test hooks avm_t1_pass / avm_debug_t1): thread per vertex, edge owned by the
 // smaller current index.
-__global__ void detect_mark_kernel(const Dev d, const Consts k, const unsigned parity, const bool count_stats) {
+__global__ void detect_mark_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, const unsigned parity,
+                                   const bool count_stats) {
   const int v = blockIdx.x * blockDim.x + threadIdx.x;
   if (v >= k.V) return;
   for (int s = 0; s < 3; ++s) {
