@@ -128,6 +128,7 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (default 3: N=1,048,576)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (kernel experiments only)")
     ap.add_argument("--profile-steps", type=int, default=100)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
@@ -203,35 +204,37 @@ def main():
     # ---------------- end to end through the host-pointer entry points --------------------------
     # One job = avm_create_host (H2D of the whole state from pinned memory) + K steps +
     # avm_get_state_host (D2H of the whole state into pinned memory), all inside the timed region.
-    pinned = {}
-    for name in ("pos", "cell_vertex_num", "cell_vertices", "vertex_neighbors", "vertex_cell_neighbors", "theta"):
-        a = np.ascontiguousarray(getattr(t, name))
-        tp = torch.from_numpy(a.copy()).pin_memory()
-        pinned[name] = tp.numpy()
-    tin = w.Tiling(t.Lx, t.Ly, t.S, pinned["pos"], pinned["cell_vertex_num"], pinned["cell_vertices"],
-                   pinned["vertex_neighbors"], pinned["vertex_cell_neighbors"], pinned["theta"])
-    out = {k: torch.empty(v.shape, dtype=torch.from_numpy(v).dtype).pin_memory().numpy() for k, v in pinned.items()}
-    h2d = sum(v.nbytes for v in pinned.values())
-    d2h = sum(v.nbytes for v in out.values())
-    e2e_ms = []
-    for rep in range(2):                      # first repetition warms allocator and page locks
-        barrier()
-        t0 = time.perf_counter()
-        s2 = B.from_tiling(tin, host=True, **p)
-        s2.step(args.steps)
-        s2.get_state_host(out)
-        torch.cuda.synchronize()
-        e2e_ms.append((time.perf_counter() - t0) * 1e3)
-        s2.close()
-        del s2
-    e2e_t = e2e_ms[-1]
-    if dist is not None:
-        tms = torch.tensor([e2e_t], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-        e2e_t = float(tms.item())
-    e2e = {"value": world * V * args.steps / (e2e_t * 1e-3), "unit": UNIT,
-           "h2d_bytes_per_step": h2d / args.steps, "d2h_bytes_per_step": d2h / args.steps,
-           "job": "avm_create_host + avm_step(K) + avm_get_state_host, pinned host buffers", "ms": e2e_t}
+    e2e = None
+    if not args.no_e2e:
+        pinned = {}
+        for name in ("pos", "cell_vertex_num", "cell_vertices", "vertex_neighbors", "vertex_cell_neighbors", "theta"):
+            a = np.ascontiguousarray(getattr(t, name))
+            tp = torch.from_numpy(a.copy()).pin_memory()
+            pinned[name] = tp.numpy()
+        tin = w.Tiling(t.Lx, t.Ly, t.S, pinned["pos"], pinned["cell_vertex_num"], pinned["cell_vertices"],
+                       pinned["vertex_neighbors"], pinned["vertex_cell_neighbors"], pinned["theta"])
+        out = {k: torch.empty(v.shape, dtype=torch.from_numpy(v).dtype).pin_memory().numpy() for k, v in pinned.items()}
+        h2d = sum(v.nbytes for v in pinned.values())
+        d2h = sum(v.nbytes for v in out.values())
+        e2e_ms = []
+        for rep in range(2):                      # first repetition warms allocator and page locks
+            barrier()
+            t0 = time.perf_counter()
+            s2 = B.from_tiling(tin, host=True, **p)
+            s2.step(args.steps)
+            s2.get_state_host(out)
+            torch.cuda.synchronize()
+            e2e_ms.append((time.perf_counter() - t0) * 1e3)
+            s2.close()
+            del s2
+        e2e_t = e2e_ms[-1]
+        if dist is not None:
+            tms = torch.tensor([e2e_t], device="cuda", dtype=torch.float64)
+            dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+            e2e_t = float(tms.item())
+        e2e = {"value": world * V * args.steps / (e2e_t * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": h2d / args.steps, "d2h_bytes_per_step": d2h / args.steps,
+               "job": "avm_create_host + avm_step(K) + avm_get_state_host, pinned host buffers", "ms": e2e_t}
 
     # ---------------- CPU baseline: the oracle as it stands, one core, bounded sample ------------
     cpu = None

@@ -15,7 +15,8 @@ from typing import Optional
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libavm_b200.so")
+# AVM_B200_LIB overrides the location (an alternative build of the same library)
+LIB_PATH = os.environ.get("AVM_B200_LIB") or os.path.join(_HERE, "libavm_b200.so")
 
 # every symbol include/avm.h declares (tests check that the library exports all of them)
 ABI_SYMBOLS = [

@@ -95,20 +95,34 @@ __device__ __forceinline__ int row_entry(const int4* cv, int N, int c, int j) {
   return reinterpret_cast<const int*>(cv + (size_t)(j >> 2) * N + c)[j & 3];
 }
 
-// 1/sqrt(x) for x >= 0: MUFU.RSQ64H seed (rel. error ~2^-22) and one third-order step
-// y <- y (1 + e/2 + 3 e^2/8), e = 1 - x y^2, which leaves ~2^-64 before rounding.  Returns 0 for
-// x below the normal range: a zero-length edge contributes nothing (R15).
-__device__ __forceinline__ double rsqrt_pos(double x) {
+// Square roots of squared lengths.  Every squared length in this library is formed as
+//   l2 = dx*dx + dy*dy + kTiny            (kTiny = 1e-300, far below one ulp of any real length)
+// so that l2 is never zero or subnormal: a zero-length edge then yields rsqrt = 1e150 and
+// r * rsqrt = 0 exactly, i.e. it contributes nothing (R15), without a compare/select per edge.
+//
+// MUFU.RSQ64H seed y0 (relative error ~2^-22) followed by one third-order correction, with
+// e = 1 - x y0^2:   1/sqrt(x) = y0 (1 + e/2 + 3 e^2/8 + O(e^3)),   sqrt(x) = x y0 (1 + e/2 + 3 e^2/8 + ...)
+// which leaves ~2^-66 before the final rounding.  5 FP64 operations each.
+static constexpr double kTiny = 1e-300;
+__device__ __forceinline__ double rsqrt_seed(double x) {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  return y;
+}
+__device__ __forceinline__ double rsqrt_pos(double x) {   // x >= kTiny
+  const double y = rsqrt_seed(x);
   const double t = __dmul_rn(x, y);
   const double e = __fma_rn(-t, y, 1.0);
   const double p = __fma_rn(0.375, e, 0.5);
-  const double ye = __dmul_rn(y, e);
-  y = __fma_rn(ye, p, y);
-  return x >= 2.2250738585072014e-308 ? y : 0.0;
+  return __fma_rn(__dmul_rn(y, e), p, y);
 }
-__device__ __forceinline__ double sqrt_pos(double x) { return __dmul_rn(x, rsqrt_pos(x)); }
+__device__ __forceinline__ double sqrt_pos(double x) {    // x >= kTiny
+  const double y = rsqrt_seed(x);
+  const double g = __dmul_rn(x, y);
+  const double e = __fma_rn(-g, y, 1.0);
+  const double p = __fma_rn(0.375, e, 0.5);
+  return __fma_rn(__dmul_rn(g, e), p, g);
+}
 
 // Philox4x32-10 (Salmon et al., SC'11; R16).  Counter (c0..c3), key (k0,k1).
 __device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint2 k) {
@@ -126,15 +140,18 @@ __device__ __forceinline__ uint4 philox_for(unsigned long long seed, unsigned lo
   return philox4x32_10(make_uint4((unsigned)step, (unsigned)(step >> 32), (unsigned)cell, (unsigned)(cell >> 32)),
                        make_uint2((unsigned)seed, (unsigned)(seed >> 32)));
 }
-// Standard normal from one Philox block: two 52-bit uniforms in (0,1), Box-Muller cosine branch.
+// Standard normal from one Philox block: two 52-bit uniforms in (0,1), Box-Muller cosine branch (R16).
+// u = (m + 1/2) 2^-52 with m the top 52 bits of a 64-bit word.  Built without an integer->double
+// conversion: the double with exponent 0 and mantissa m is 1 + m 2^-52, and adding (2^-53 - 1) is exact.
+__device__ __forceinline__ double uniform52(unsigned int lo, unsigned int hi) {
+  const double one_plus = __hiloint2double((int)(0x3ff00000u | (hi >> 12)), (int)((hi << 20) | (lo >> 12)));
+  return __dadd_rn(one_plus, 1.1102230246251565e-16 - 1.0);
+}
 __device__ __forceinline__ double director_noise(unsigned long long seed, unsigned long long step,
                                                  unsigned long long cell) {
   const uint4 x = philox_for(seed, step, cell);
-  const unsigned long long a = ((unsigned long long)x.y << 32) | x.x;
-  const unsigned long long b = ((unsigned long long)x.w << 32) | x.z;
-  const double u1 = ((double)(a >> 12) + 0.5) * 2.220446049250313e-16;   // 2^-52
-  const double u2 = ((double)(b >> 12) + 0.5) * 2.220446049250313e-16;
-  return sqrt(-2.0 * log(u1)) * cospi(2.0 * u2);
+  const double u1 = uniform52(x.x, x.y), u2 = uniform52(x.z, x.w);
+  return sqrt_pos(-2.0 * log(u1)) * cospi(2.0 * u2);   // -2 ln u1 >= 2.2e-16 > kTiny
 }
 
 // One edge of the shoelace / perimeter sums (Eq. A1 inputs, R14): previous unwrapped vertex
@@ -145,7 +162,7 @@ __device__ __forceinline__ double geom_edge(double rxp, double ryp, double rx, d
   acc = __fma_rn(rxp, ry, acc);
   acc = __fma_rn(-ryp, rx, acc);
   const double dx = __dsub_rn(rx, rxp), dy = __dsub_rn(ry, ryp);
-  const double l2 = __fma_rn(dx, dx, __dmul_rn(dy, dy));
+  const double l2 = __fma_rn(dx, dx, __fma_rn(dy, dy, kTiny));
   per = __dadd_rn(per, sqrt_pos(l2));
   return l2;
 }

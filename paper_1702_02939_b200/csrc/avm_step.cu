@@ -28,6 +28,19 @@ static constexpr int kT1Block = 128;
 static constexpr int kT1Grid = 148 * 2;
 static constexpr unsigned kFull = 0xffffffffu;
 
+// tuning knobs (compile-time; the defaults are the measured best, profiles/)
+#ifndef AVM_FM_PF
+#define AVM_FM_PF 0        // force_move: L2 prefetch distance in grid sweeps (0 = off; measured: no gain, the pass is LSU-bound)
+#endif
+#ifndef AVM_FM_MINB
+#define AVM_FM_MINB 3      // force_move: minimum resident CTAs per SM asked of the compiler
+#endif
+#ifndef AVM_FM_REGPF
+#define AVM_FM_REGPF 1     // force_move: keep the next vertex's streaming loads in registers
+#endif
+
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 // ---- cache-hinted loads -------------------------------------------------------------------------
 // Pure streams (index lists, tags) are read once per step: evict-first so that they do not push
 // the re-used arrays (positions, cell records) out of L1/L2.
@@ -64,9 +77,10 @@ __device__ __forceinline__ double2 vertex_force(const double2 h, const double2 q
     r0x = min_image(r0x, k.Lx, k.hLx); r1x = min_image(r1x, k.Lx, k.hLx); r2x = min_image(r2x, k.Lx, k.hLx);
     r0y = min_image(r0y, k.Ly, k.hLy); r1y = min_image(r1y, k.Ly, k.hLy); r2y = min_image(r2y, k.Ly, k.hLy);
   }
-  const double i0 = rsqrt_pos(r0x * r0x + r0y * r0y);   // zero-length edge contributes 0 (R15)
-  const double i1 = rsqrt_pos(r1x * r1x + r1y * r1y);
-  const double i2 = rsqrt_pos(r2x * r2x + r2y * r2y);
+  // + kTiny: a zero-length edge gives r * rsqrt = 0, i.e. contributes nothing (R15)
+  const double i0 = rsqrt_pos(__fma_rn(r0x, r0x, __fma_rn(r0y, r0y, kTiny)));
+  const double i1 = rsqrt_pos(__fma_rn(r1x, r1x, __fma_rn(r1y, r1y, kTiny)));
+  const double i2 = rsqrt_pos(__fma_rn(r2x, r2x, __fma_rn(r2y, r2y, kTiny)));
   const double u0x = r0x * i0, u0y = r0y * i0, u1x = r1x * i1, u1y = r1y * i1, u2x = r2x * i2, u2y = r2y * i2;
   // cell k uses (next, prev) = (r_k, r_{k+1})
   double fx = -0.5 * (c0.a * (r0y - r1y) + c1.a * (r1y - r2y) + c2.a * (r2y - r0y));
@@ -87,7 +101,7 @@ __device__ __forceinline__ VertexIn load_vertex(const Dev& d, const Consts& k, i
 
 // Persistent grid-stride kernel: each thread keeps the streaming loads of its NEXT vertex in
 // flight while it gathers and computes the current one.
-__global__ void __launch_bounds__(kVertexBlock)
+__global__ void __launch_bounds__(kVertexBlock, AVM_FM_MINB)
 force_move_kernel(const Dev d, const Consts k, const unsigned parity) {
   const int tid = blockIdx.x * kVertexBlock + threadIdx.x;
   const int stride = gridDim.x * kVertexBlock;
@@ -103,12 +117,27 @@ force_move_kernel(const Dev d, const Consts k, const unsigned parity) {
   if (v >= k.V) return;
   const unsigned hiLx = hi_word(k.Lx), hiLy = hi_word(k.Ly);
   VertexIn in = load_vertex(d, k, v);
+  const int lane = threadIdx.x & 31;
   for (;;) {
+    if (AVM_FM_PF) {
+      // pull the contiguous streams of a later sweep into L2: positions, both index lists and the
+      // cell records around v/2 (cells and vertices share the Hilbert order, so this window also
+      // holds most of that sweep's gather targets)
+      const long long vb = (long long)(v - lane) + (long long)AVM_FM_PF * stride;
+      if (vb + 32 <= k.V) {
+        const char* a = nullptr;
+        if (lane < 4) a = reinterpret_cast<const char*>(d.pos + vb) + 128 * lane;
+        else if (lane < 7) a = reinterpret_cast<const char*>(d.vn + (size_t)(lane - 4) * k.Vs + vb);
+        else if (lane < 10) a = reinterpret_cast<const char*>(d.vc + (size_t)(lane - 7) * k.Vs + vb);
+        else if (lane < 14) a = reinterpret_cast<const char*>(d.rec + (vb >> 1)) + 128 * (lane - 10);
+        if (a) prefetch_l2(a);
+      }
+    }
     const double2 q0 = __ldg(d.pos + in.n0), q1 = __ldg(d.pos + in.n1), q2 = __ldg(d.pos + in.n2);
     const CellRec c0 = ld_rec(d.rec + in.c0), c1 = ld_rec(d.rec + in.c1), c2 = ld_rec(d.rec + in.c2);
     const double2 h = in.h;
     const int vnext = v + stride;
-    if (vnext < k.V) in = load_vertex(d, k, vnext);
+    if (AVM_FM_REGPF && vnext < k.V) in = load_vertex(d, k, vnext);
     const double2 f = vertex_force(h, q0, q1, q2, c0, c1, c2, k);
     // Eq. 4: dh/dt = mu F + (v0/3) sum of the three unit directors (R5), directors of the start
     // of the step (R7); explicit Euler; wrap into the box (R13)
@@ -123,6 +152,7 @@ force_move_kernel(const Dev d, const Consts k, const unsigned parity) {
     d.pos_next[v] = make_double2(x, y);
     if (vnext >= k.V) break;
     v = vnext;
+    if (!AVM_FM_REGPF) in = load_vertex(d, k, v);
   }
 }
 
@@ -193,10 +223,10 @@ __device__ __noinline__ void t1_report_cell(const Dev& d, const Consts& k, int c
 // One thread per cell.  Row entries 0..7 come from planes 0 and 1 (two coalesced 128-bit loads);
 // their positions are gathered with up to eight independent predicated 128-bit loads, and the
 // director arithmetic (Philox, Box-Muller, sincos) is placed between issuing those gathers and
-// consuming them.  Entries beyond the cell's n are treated as copies of entry 0 (r = 0): the
-// edge into the first of them is the closing edge and the rest are exact no-ops, so the edge
-// loop has a fixed trip count and no divergent exits.  Planes 2.. are visited only by warps that
-// hold a cell with more than 8 vertices.
+// consuming them.  Entries beyond the cell's n are copies of entry 0 (r = 0): the edge into the
+// first of them is the closing edge and the rest are exact no-ops, so the eight-entry head has a
+// fixed trip count and no divergent exits.  Only lanes whose cell has more than 8 vertices (4 %
+// of a Voronoi tiling) run the tail over planes 2.. .
 // Cells are walked in DESCENDING index order while force_move walks vertices in ascending order,
 // so each pass starts on the lines the previous pass touched last (L2 recency).
 // ---------------------------------------------------------------------------------------------
@@ -217,7 +247,7 @@ cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts
   h[0] = __ldg(pos + e[0]);
 #pragma unroll
   for (int j = 1; j < 8; ++j) {
-    h[j] = make_double2(0.0, 0.0);
+    h[j] = h[0];
     if (j < n) h[j] = __ldg(pos + e[j]);
   }
   // ---- director (independent of the gathers above) ----
@@ -227,57 +257,57 @@ cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts
   }
   double sn, cs;
   sincos(th, &sn, &cs);
-  // ---- unwrap relative to entry 0 (R14) ----
-  const unsigned hx = hi_word(k.hLx), hy = hi_word(k.hLy), hlc = hi_word(k.lc2);
+  // ---- unwrap relative to entry 0 (R14); |r| >= L/2 is decided conservatively on the high
+  // words with integer ALU operations, the exact minimum image runs only where that fires ----
+  const unsigned hmin = min(hi_word(k.hLx), hi_word(k.hLy)), hlc = hi_word(k.lc2);
   double rx[8], ry[8];
-  unsigned wrapf = 0;
+  unsigned far = 0;
 #pragma unroll
   for (int j = 1; j < 8; ++j) {
-    rx[j] = j < n ? __dsub_rn(h[j].x, h[0].x) : 0.0;
-    ry[j] = j < n ? __dsub_rn(h[j].y, h[0].y) : 0.0;
-    wrapf |= may_wrap(rx[j], hx) | may_wrap(ry[j], hy);
+    rx[j] = __dsub_rn(h[j].x, h[0].x);
+    ry[j] = __dsub_rn(h[j].y, h[0].y);
+    far = max(far, max(hi_word(rx[j]) & 0x7fffffffu, hi_word(ry[j]) & 0x7fffffffu));
   }
-  if (wrapf) {
+  if (far >= hmin) {
 #pragma unroll
     for (int j = 1; j < 8; ++j) { rx[j] = min_image(rx[j], k.Lx, k.hLx); ry[j] = min_image(ry[j], k.Ly, k.hLy); }
   }
-  // ---- shoelace + perimeter, edges ending at entries 1..7 ----
+  // ---- shoelace + perimeter; bit j-1 of smask = the edge ending at row entry j looks short ----
   double acc = 0.0, per = 0.0, rxp = 0.0, ryp = 0.0;
   unsigned smask = 0;
 #pragma unroll
   for (int j = 1; j < 8; ++j) {
     const double l2 = geom_edge(rxp, ryp, rx[j], ry[j], acc, per);
-    if (kStep && hi_word(l2) <= hlc && j <= n) smask |= 1u << (j - 1);
+    if (kStep && hi_word(l2) <= hlc) smask |= 1u << (j - 1);
     rxp = rx[j]; ryp = ry[j];
   }
-  // ---- entries 8.. (planes 2..), only in warps that hold such a cell ----
-  for (int q = 2;; ++q) {
-    const int j0 = 4 * q;
-    if (!(j0 < k.S && __any_sync(kFull, n > j0))) {
-      const double l2 = geom_edge(rxp, ryp, 0.0, 0.0, acc, per);     // closing edge of an n == j0 cell
-      if (kStep && hi_word(l2) <= hlc && j0 <= n) smask |= 1u << (j0 - 1);
-      break;
-    }
-    int4 qq = make_int4(0, 0, 0, 0);
-    if (n > j0) qq = d.cv[(size_t)q * k.N + c];
-    const int ee[4] = {qq.x, qq.y, qq.z, qq.w};
-    double2 hh[4];
+  // ---- entries 8.. (planes 2..): divergent, only the lanes that hold such a cell ----
+  if (n > 8) {
+    for (int q = 2; 4 * q < n; ++q) {
+      const int j0 = 4 * q;
+      const int4 qq = d.cv[(size_t)q * k.N + c];
+      const int ee[4] = {qq.x, qq.y, qq.z, qq.w};
+      double2 hh[4];
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      hh[i] = make_double2(0.0, 0.0);
-      if (j0 + i < n) hh[i] = __ldg(pos + ee[i]);
-    }
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      double x = 0.0, y = 0.0;
-      if (j0 + i < n) {
-        x = min_image(__dsub_rn(hh[i].x, h[0].x), k.Lx, k.hLx);
-        y = min_image(__dsub_rn(hh[i].y, h[0].y), k.Ly, k.hLy);
+      for (int i = 0; i < 4; ++i) {
+        hh[i] = h[0];
+        if (j0 + i < n) hh[i] = __ldg(pos + ee[i]);
       }
-      const double l2 = geom_edge(rxp, ryp, x, y, acc, per);
-      if (kStep && hi_word(l2) <= hlc && j0 + i <= n) smask |= 1u << (j0 + i - 1);
-      rxp = x; ryp = y;
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        if (j0 + i < n) {
+          const double x = min_image(__dsub_rn(hh[i].x, h[0].x), k.Lx, k.hLx);
+          const double y = min_image(__dsub_rn(hh[i].y, h[0].y), k.Ly, k.hLy);
+          const double l2 = geom_edge(rxp, ryp, x, y, acc, per);
+          if (kStep && hi_word(l2) <= hlc) smask |= 1u << (j0 + i - 1);
+          rxp = x; ryp = y;
+        }
+      }
     }
+  }
+  {  // closing edge of an n >= 8 cell (an exact no-op for smaller ones, which closed above)
+    const double l2 = geom_edge(rxp, ryp, 0.0, 0.0, acc, per);
+    if (kStep && hi_word(l2) <= hlc) smask |= 1u << ((n > 8 ? n : 8) - 1);
   }
   if (!valid) return;
   CellRec r;
@@ -285,6 +315,7 @@ cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts
   r.p = k.KP2 * (per - k.P0);
   r.nx = cs; r.ny = sn;
   st_rec(d.rec + c, r);
+  smask &= n >= 32 ? ~0u : (1u << n) - 1u;     // edges beyond the closing one are padding
   if (kStep && smask) t1_report_cell(d, k, c, n, smask, parity);
 }
 
@@ -342,9 +373,11 @@ t1_flip_kernel(const Dev d, const Consts k, const unsigned parity, const bool co
     double px = 0.0, py = 1.0;
     if (l > 0.0) { px = -dy / l; py = dx / l; }
     const double half = 0.75 * k.lc;
+    const double2 n2 = make_double2(wrap_box(mx + half * px, k.Lx), wrap_box(my + half * py, k.Ly));
+    const double2 n1 = make_double2(wrap_box(mx - half * px, k.Lx), wrap_box(my - half * py, k.Ly));
     if (lane == 0) {
-      d.pos[v2] = make_double2(wrap_box(mx + half * px, k.Lx), wrap_box(my + half * py, k.Ly));
-      d.pos[v1] = make_double2(wrap_box(mx - half * px, k.Lx), wrap_box(my - half * py, k.Ly));
+      d.pos[v2] = n2;
+      d.pos[v1] = n1;
       // lists: u = ([w, x, y]; [C0, C1, C2]) cyclic from the partner slot
       //     -> ([w, y, z]; [C1, C2, C']), z = partner's old x, C' = partner's old C1 (R12)
       d.vn[a1 * k.Vs + v1] = y1; d.vn[b1 * k.Vs + v1] = x2;
@@ -355,33 +388,59 @@ t1_flip_kernel(const Dev d, const Consts k, const unsigned parity, const bool co
     // outer vertices: x1 was joined to v1 and is now joined to v2 (same slot); x2 likewise
     if (lane < 3 && outer == v1) d.vn[lane * k.Vs + x1] = v2;
     if (lane >= 3 && lane < 6 && outer == v2) d.vn[(lane - 3) * k.Vs + x2] = v1;
-    // rows: L deletes v1, R deletes v2 (later entries shift down)
+    // rows (lane = row entry): L deletes v1, R deletes v2 (later entries shift down); E1 inserts
+    // v2 immediately after v1, E2 inserts v1 immediately after v2 (later entries shift up).
+    // The new rows are formed in registers, written back, and reused by the refresh below.
+    int nnew[4];
 #pragma unroll
-    for (int t = 0; t < 2; ++t) {
-      const int victim = t == 0 ? v1 : v2;
-      const int p = __ffs(__ballot_sync(kFull, lane < nrow[t] && row[t] == victim)) - 1;
-      const int nxt = __shfl_down_sync(kFull, row[t], 1);
-      if (lane >= p && lane < nrow[t]) row_entry(d.cv, k.N, cells[t], lane) = lane == nrow[t] - 1 ? -1 : nxt;
-      if (lane == 0) d.cvn[cells[t]] = nrow[t] - 1;
+    for (int t = 0; t < 4; ++t) {
+      int r = row[t];
+      if (t < 2) {
+        const int victim = t == 0 ? v1 : v2;
+        const int p = __ffs(__ballot_sync(kFull, lane < nrow[t] && r == victim)) - 1;
+        const int nxt = __shfl_down_sync(kFull, r, 1);
+        nnew[t] = nrow[t] - 1;
+        if (lane >= p) r = lane < nnew[t] ? nxt : -1;
+      } else {
+        const int after = t == 2 ? v1 : v2, ins = t == 2 ? v2 : v1;
+        const int p = __ffs(__ballot_sync(kFull, lane < nrow[t] && r == after)) - 1;
+        const int prv = __shfl_up_sync(kFull, r, 1);
+        nnew[t] = nrow[t] + 1;
+        if (lane > p) r = lane == p + 1 ? ins : (lane < nnew[t] ? prv : -1);
+      }
+      if (lane < k.S && r != row[t]) row_entry(d.cv, k.N, cells[t], lane) = r;
+      if (lane == 0) d.cvn[cells[t]] = nnew[t];
+      row[t] = r;
     }
-    // E1 inserts v2 immediately after v1, E2 inserts v1 immediately after v2 (later entries shift up)
+    // refresh the cached geometry of the four cells (directors unchanged): every lane fetches
+    // the position of "its" entry of each row (v1 and v2 take their new positions from
+    // registers), then the warp runs the same serial sum as the per-step pass, so that a resumed
+    // run reproduces these records bit for bit.  Lane t keeps cell t's result.
+    double2 hr[4];
 #pragma unroll
-    for (int t = 2; t < 4; ++t) {
-      const int after = t == 2 ? v1 : v2, ins = t == 2 ? v2 : v1;
-      const int p = __ffs(__ballot_sync(kFull, lane < nrow[t] && row[t] == after)) - 1;
-      const int prv = __shfl_up_sync(kFull, row[t], 1);
-      if (lane > p && lane <= nrow[t]) row_entry(d.cv, k.N, cells[t], lane) = lane == p + 1 ? ins : prv;
-      if (lane == 0) d.cvn[cells[t]] = nrow[t] + 1;
+    for (int t = 0; t < 4; ++t) {
+      hr[t] = make_double2(0.0, 0.0);
+      const int v = row[t];
+      if (lane < nnew[t]) hr[t] = v == v1 ? n1 : v == v2 ? n2 : d.pos[v];
     }
-    __syncwarp();
-    // refresh the cached geometry of the four cells (directors unchanged); same serial sum as
-    // the per-step pass so that a resumed run reproduces these records bit for bit
+    double myA = 0.0, myP = 0.0;
+#pragma unroll
+    for (int t = 0; t < 4; ++t) {
+      const double h0x = __shfl_sync(kFull, hr[t].x, 0), h0y = __shfl_sync(kFull, hr[t].y, 0);
+      const double ux = min_image(__dsub_rn(hr[t].x, h0x), k.Lx, k.hLx), uy = min_image(__dsub_rn(hr[t].y, h0y), k.Ly, k.hLy);
+      double rxp = 0.0, ryp = 0.0, acc = 0.0, per = 0.0;
+      for (int j = 1; j <= nnew[t]; ++j) {
+        const int src = j < nnew[t] ? j : 0;       // j == n: the closing edge back to entry 0 (r = 0)
+        const double x = __shfl_sync(kFull, ux, src), y = __shfl_sync(kFull, uy, src);
+        geom_edge(rxp, ryp, x, y, acc, per);
+        rxp = x; ryp = y;
+      }
+      if (lane == t) { myA = __dmul_rn(0.5, acc); myP = per; }
+    }
     if (lane < 4) {
-      const int cc = lane == 0 ? c.cL : lane == 1 ? c.cR : lane == 2 ? c.cE1 : c.cE2;
-      double A, P;
-      cell_area_perimeter(d.pos, d.cv, cc, d.cvn[cc], k, A, P);
-      d.rec[cc].a = k.KA2 * (A - k.A0);
-      d.rec[cc].p = k.KP2 * (P - k.P0);
+      const int cc = cells[lane == 0 ? 0 : lane == 1 ? 1 : lane == 2 ? 2 : 3];
+      d.rec[cc].a = k.KA2 * (myA - k.A0);
+      d.rec[cc].p = k.KP2 * (myP - k.P0);
     }
     __syncwarp();
   }
