@@ -22,7 +22,8 @@ struct __align__(16) Cand {
   int k1, k2;           // slot of v2 in v1, slot of v1 in v2
   int cL, cR, cE1, cE2; // the two cells sharing the edge, the two end cells (R12)
   unsigned long long key;  // (tag(v1) << 32) | tag(v2)  (R11)
-  unsigned long long pad;
+  int sx1, sx2;         // slot of v1 in x1, slot of v2 in x2
+  int x1, y1, x2, y2;   // the other two neighbours of v1 (cyclic after v2) and of v2 (cyclic after v1)
 };
 
 struct Counters {

@@ -32,12 +32,23 @@ static constexpr unsigned kFull = 0xffffffffu;
 #ifndef AVM_FM_PF
 #define AVM_FM_PF 0        // force_move: L2 prefetch distance in grid sweeps (0 = off; measured: no gain, the pass is LSU-bound)
 #endif
+#ifndef AVM_PDL
+#define AVM_PDL 1          // chain the step's kernels with programmatic dependent launch
+#endif
 #ifndef AVM_FM_MINB
 #define AVM_FM_MINB 3      // force_move: minimum resident CTAs per SM asked of the compiler
 #endif
 #ifndef AVM_FM_REGPF
 #define AVM_FM_REGPF 1     // force_move: keep the next vertex's streaming loads in registers
 #endif
+
+// Programmatic dependent launch (sm_90+): the three kernels of a step form a chain on one stream.
+// Each kernel lets its successor's CTAs be scheduled as soon as all of its own CTAs have started
+// (pdl_launch_dependents) and itself waits for the predecessor's completion and memory flush
+// before it touches anything (pdl_wait), so launch latency and the drain of the last wave are
+// hidden while the ordering of plain stream semantics is kept.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
 
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
@@ -103,6 +114,8 @@ __device__ __forceinline__ VertexIn load_vertex(const Dev& d, const Consts& k, i
 // flight while it gathers and computes the current one.
 __global__ void __launch_bounds__(kVertexBlock, AVM_FM_MINB)
 force_move_kernel(const Dev d, const Consts k, const unsigned parity) {
+  pdl_launch_dependents();
+  pdl_wait();
   const int tid = blockIdx.x * kVertexBlock + threadIdx.x;
   const int stride = gridDim.x * kVertexBlock;
   {  // the previous step's T1 candidates are done: clear their cells' minimum keys (row a6)
@@ -169,11 +182,12 @@ __device__ __noinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va,
   int v1 = va, v2 = vb;
   unsigned int t1 = (unsigned int)d.vtag[v1], t2 = (unsigned int)d.vtag[v2];
   if (t1 > t2) { int tv = v1; v1 = v2; v2 = tv; unsigned int tt = t1; t1 = t2; t2 = tt; }
-  int k1 = 0, k2 = 0;
+  int k1 = 0, k2 = 0, nb1[3], nb2[3];
 #pragma unroll
   for (int s = 0; s < 3; ++s) {
-    if (d.vn[s * k.Vs + v1] == v2) k1 = s;
-    if (d.vn[s * k.Vs + v2] == v1) k2 = s;
+    nb1[s] = d.vn[s * k.Vs + v1]; nb2[s] = d.vn[s * k.Vs + v2];
+    if (nb1[s] == v2) k1 = s;
+    if (nb2[s] == v1) k2 = s;
   }
   // cyclic from the partner's slot the cells of u are (C0, C1, C2); C0 is left of u -> partner
   const int cL = d.vc[k1 * k.Vs + v1], cE1 = d.vc[((k1 + 1) % 3) * k.Vs + v1];
@@ -192,7 +206,15 @@ __device__ __noinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va,
   cd.v1 = v1; cd.v2 = v2; cd.k1 = k1; cd.k2 = k2;
   cd.cL = cL; cd.cR = cR; cd.cE1 = cE1; cd.cE2 = cE2;
   cd.key = ((unsigned long long)t1 << 32) | t2;
-  cd.pad = 0;
+  // the flip's outer vertices, decoded here so that the flip kernel needs no dependent loads
+  cd.x1 = k1 == 0 ? nb1[1] : k1 == 1 ? nb1[2] : nb1[0]; cd.y1 = k1 == 0 ? nb1[2] : k1 == 1 ? nb1[0] : nb1[1];
+  cd.x2 = k2 == 0 ? nb2[1] : k2 == 1 ? nb2[2] : nb2[0]; cd.y2 = k2 == 0 ? nb2[2] : k2 == 1 ? nb2[0] : nb2[1];
+  cd.sx1 = 0; cd.sx2 = 0;
+#pragma unroll
+  for (int s = 1; s < 3; ++s) {
+    if (d.vn[s * k.Vs + cd.x1] == v1) cd.sx1 = s;
+    if (d.vn[s * k.Vs + cd.x2] == v2) cd.sx2 = s;
+  }
   const unsigned int slot = atomicAdd(&d.ctr->n_cand[parity], 1u);
   d.cand[slot] = cd;
   atomicMin(&d.minkey[cL], cd.key);
@@ -234,6 +256,8 @@ template <bool kStep>
 __global__ void __launch_bounds__(kCellBlock)
 cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, const unsigned long long step,
                    const unsigned parity) {
+  pdl_launch_dependents();
+  pdl_wait();
   const int gid = blockIdx.x * kCellBlock + threadIdx.x;
   const bool valid = gid < k.N;
   const int c = valid ? k.N - 1 - gid : 0;
@@ -339,6 +363,8 @@ __global__ void detect_mark_kernel(const __grid_constant__ Dev d, const __grid_c
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kT1Block)
 t1_flip_kernel(const Dev d, const Consts k, const unsigned parity, const bool count_stats) {
+  pdl_launch_dependents();
+  pdl_wait();
   const unsigned int n_cand = d.ctr->n_cand[parity];
   const int lane = threadIdx.x & 31;
   const unsigned gwarp = (blockIdx.x * kT1Block + threadIdx.x) >> 5, nwarps = (gridDim.x * kT1Block) >> 5;
@@ -348,24 +374,22 @@ t1_flip_kernel(const Dev d, const Consts k, const unsigned parity, const bool co
     const Cand c = d.cand[i];
     const int cells[4] = {c.cL, c.cR, c.cE1, c.cE2};
     const int l4 = lane & 3;
+    // ---- everything is read before anything is written; the loads below are independent of
+    // one another (the marking thread decoded the neighbourhood), so the minimum-key test
+    // costs no extra round trip ----
     const unsigned long long mk = d.minkey[l4 == 0 ? c.cL : l4 == 1 ? c.cR : l4 == 2 ? c.cE1 : c.cE2];
-    if (!__all_sync(kFull, mk == c.key)) { ++blocked; continue; }
-    ++flips;
     const int v1 = c.v1, v2 = c.v2, k1 = c.k1, k2 = c.k2;
     const int a1 = (k1 + 1) % 3, b1 = (k1 + 2) % 3, a2 = (k2 + 1) % 3, b2 = (k2 + 2) % 3;
-    // ---- everything is read before anything is written ----
     const double2 h1 = d.pos[v1], h2 = d.pos[v2];
-    const int x1 = d.vn[a1 * k.Vs + v1], y1 = d.vn[b1 * k.Vs + v1];
-    const int x2 = d.vn[a2 * k.Vs + v2], y2 = d.vn[b2 * k.Vs + v2];
+    const int x1 = c.x1, y1 = c.y1, x2 = c.x2, y2 = c.y2;
     int row[4], nrow[4];
 #pragma unroll
     for (int t = 0; t < 4; ++t) {
       nrow[t] = d.cvn[cells[t]];
       row[t] = lane < k.S ? row_entry(d.cv, k.N, cells[t], lane) : -1;
     }
-    int outer = -1;   // lanes 0-2: slots of x1, lanes 3-5: slots of x2
-    if (lane < 3) outer = d.vn[lane * k.Vs + x1];
-    else if (lane < 6) outer = d.vn[(lane - 3) * k.Vs + x2];
+    if (!__all_sync(kFull, mk == c.key)) { ++blocked; continue; }
+    ++flips;
     // ---- geometry: rigid counter-clockwise quarter turn about the midpoint, new length 1.5 l_c (R9)
     const double dx = min_image(h2.x - h1.x, k.Lx, k.hLx), dy = min_image(h2.y - h1.y, k.Ly, k.hLy);
     const double l = sqrt(dx * dx + dy * dy);
@@ -386,8 +410,8 @@ t1_flip_kernel(const Dev d, const Consts k, const unsigned parity, const bool co
       d.vc[k2 * k.Vs + v2] = c.cE2; d.vc[a2 * k.Vs + v2] = c.cL; d.vc[b2 * k.Vs + v2] = c.cE1;
     }
     // outer vertices: x1 was joined to v1 and is now joined to v2 (same slot); x2 likewise
-    if (lane < 3 && outer == v1) d.vn[lane * k.Vs + x1] = v2;
-    if (lane >= 3 && lane < 6 && outer == v2) d.vn[(lane - 3) * k.Vs + x2] = v1;
+    if (lane == 1) d.vn[c.sx1 * k.Vs + x1] = v2;
+    if (lane == 2) d.vn[c.sx2 * k.Vs + x2] = v1;
     // rows (lane = row entry): L deletes v1, R deletes v2 (later entries shift down); E1 inserts
     // v2 immediately after v1, E2 inserts v1 immediately after v2 (later entries shift up).
     // The new rows are formed in registers, written back, and reused by the refresh below.
@@ -572,19 +596,32 @@ static int force_move_grid(const Consts& k) {
   return want < cap ? want : cap;
 }
 
+// Launch with the programmatic-stream-serialization attribute (see pdl_wait above).
+template <typename... KArgs, typename... Args>
+static void launch_chained(void (*kernel)(KArgs...), int grid, int block, cudaStream_t s, bool pdl, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block); cfg.dynamicSmemBytes = 0; cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 // One timestep.  d.pos = positions at the start of the step, d.pos_next = buffer for the moved
 // positions (the caller swaps them afterwards).
 // ev (optional, AVM_K_COUNT+1 events): recorded before/after each kernel by avm_step_profile.
 int launch_step(const Dev& d, const Consts& k, unsigned long long step, cudaStream_t s, cudaEvent_t* ev) {
   const unsigned parity = (unsigned)(step & 1ull);
   if (ev) cudaEventRecord(ev[0], s);
-  force_move_kernel<<<force_move_grid(k), kVertexBlock, 0, s>>>(d, k, parity);
+  const bool pdl = AVM_PDL && ev == nullptr;   // events between the kernels would break the chain anyway
+  launch_chained(force_move_kernel, force_move_grid(k), kVertexBlock, s, pdl, d, k, parity);
   if (ev) cudaEventRecord(ev[1], s);
   Dev m = d;                      // from here on the moved positions are "the" positions
   m.pos = d.pos_next; m.pos_next = d.pos;
-  cell_update_kernel<true><<<cdiv(k.N, kCellBlock), kCellBlock, 0, s>>>(m, k, step, parity);
+  launch_chained(cell_update_kernel<true>, cdiv(k.N, kCellBlock), kCellBlock, s, pdl, m, k, step, parity);
   if (ev) cudaEventRecord(ev[2], s);
-  t1_flip_kernel<<<kT1Grid, kT1Block, 0, s>>>(m, k, parity, true);
+  launch_chained(t1_flip_kernel, kT1Grid, kT1Block, s, pdl, m, k, parity, true);
   if (ev) cudaEventRecord(ev[3], s);
   return 3;
 }
