@@ -242,6 +242,7 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   k.amp = sqrt(2.0 * params->Dr * params->dt);
   k.lc = params->l_c; k.lc2 = params->l_c * params->l_c;
   k.seed = params->seed;
+  for (int r = 0; r < 10; ++r) k.rkey[r] = philox_round_key(params->seed, r);
   char* w = s->ws;
   for (int i = 0; i < 2; ++i) {
     s->pos[i] = (double2*)(w + L.pos[i]);

@@ -7,6 +7,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include "../../include/avm.h"
+#include "avm_math.cuh"
 
 namespace avm {
 
@@ -47,6 +48,7 @@ struct Consts {
   double amp;                // sqrt(2 Dr dt) (R8)
   double lc, lc2;
   unsigned long long seed;
+  uint2 rkey[10];            // Philox round keys of `seed` (the key schedule is uniform: done once on the host)
 };
 
 // Pointers into the caller's workspace (current buffer set).
@@ -125,21 +127,29 @@ __device__ __forceinline__ double sqrt_pos(double x) {    // x >= kTiny
   return __fma_rn(__dmul_rn(g, e), p, g);
 }
 
-// Philox4x32-10 (Salmon et al., SC'11; R16).  Counter (c0..c3), key (k0,k1).
-__device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint2 k) {
-#pragma unroll
-  for (int r = 0; r < 10; ++r) {
-    const unsigned int hi0 = __umulhi(0xD2511F53u, c.x), lo0 = 0xD2511F53u * c.x;
-    const unsigned int hi1 = __umulhi(0xCD9E8D57u, c.z), lo1 = 0xCD9E8D57u * c.z;
-    c = make_uint4(hi1 ^ c.y ^ k.x, lo1, hi0 ^ c.w ^ k.y, lo0);
-    k.x += 0x9E3779B9u; k.y += 0xBB67AE85u;
-  }
-  return c;
+// Philox4x32-10 (Salmon et al., SC'11; R16).  Counter (c0..c3), key (k0,k1); round r uses the
+// key (k0 + r 0x9E3779B9, k1 + r 0xBB67AE85).
+__host__ __device__ __forceinline__ uint2 philox_round_key(unsigned long long seed, int r) {
+  return make_uint2((unsigned)seed + (unsigned)r * 0x9E3779B9u, (unsigned)(seed >> 32) + (unsigned)r * 0xBB67AE85u);
+}
+__device__ __forceinline__ uint4 philox_round(uint4 c, uint2 k) {
+  const unsigned int hi0 = __umulhi(0xD2511F53u, c.x), lo0 = 0xD2511F53u * c.x;
+  const unsigned int hi1 = __umulhi(0xCD9E8D57u, c.z), lo1 = 0xCD9E8D57u * c.z;
+  return make_uint4(hi1 ^ c.y ^ k.x, lo1, hi0 ^ c.w ^ k.y, lo0);
 }
 __device__ __forceinline__ uint4 philox_for(unsigned long long seed, unsigned long long step,
                                             unsigned long long cell) {
-  return philox4x32_10(make_uint4((unsigned)step, (unsigned)(step >> 32), (unsigned)cell, (unsigned)(cell >> 32)),
-                       make_uint2((unsigned)seed, (unsigned)(seed >> 32)));
+  uint4 c = make_uint4((unsigned)step, (unsigned)(step >> 32), (unsigned)cell, (unsigned)(cell >> 32));
+#pragma unroll
+  for (int r = 0; r < 10; ++r) c = philox_round(c, philox_round_key(seed, r));
+  return c;
+}
+// the same block with the round keys taken from the kernel constants
+__device__ __forceinline__ uint4 philox_for(const Consts& k, unsigned long long step, unsigned long long cell) {
+  uint4 c = make_uint4((unsigned)step, (unsigned)(step >> 32), (unsigned)cell, (unsigned)(cell >> 32));
+#pragma unroll
+  for (int r = 0; r < 10; ++r) c = philox_round(c, k.rkey[r]);
+  return c;
 }
 // Standard normal from one Philox block: two 52-bit uniforms in (0,1), Box-Muller cosine branch (R16).
 // u = (m + 1/2) 2^-52 with m the top 52 bits of a 64-bit word.  Built without an integer->double
@@ -148,11 +158,10 @@ __device__ __forceinline__ double uniform52(unsigned int lo, unsigned int hi) {
   const double one_plus = __hiloint2double((int)(0x3ff00000u | (hi >> 12)), (int)((hi << 20) | (lo >> 12)));
   return __dadd_rn(one_plus, 1.1102230246251565e-16 - 1.0);
 }
-__device__ __forceinline__ double director_noise(unsigned long long seed, unsigned long long step,
-                                                 unsigned long long cell) {
-  const uint4 x = philox_for(seed, step, cell);
+__device__ __forceinline__ double director_noise(const Consts& k, unsigned long long step, unsigned long long cell) {
+  const uint4 x = philox_for(k, step, cell);
   const double u1 = uniform52(x.x, x.y), u2 = uniform52(x.z, x.w);
-  return sqrt_pos(-2.0 * log(u1)) * cospi(2.0 * u2);   // -2 ln u1 >= 2.2e-16 > kTiny
+  return sqrt_pos(-2.0 * log_unit(u1)) * cos_2pi(u2);   // -2 ln u1 >= 2.2e-16 > kTiny
 }
 
 // One edge of the shoelace / perimeter sums (Eq. A1 inputs, R14): previous unwrapped vertex

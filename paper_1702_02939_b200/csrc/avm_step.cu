@@ -276,11 +276,11 @@ cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts
   }
   // ---- director (independent of the gathers above) ----
   if (kStep) {
-    th += k.amp * director_noise(k.seed, step, (unsigned long long)tag);
+    th += k.amp * director_noise(k, step, (unsigned long long)tag);
     if (valid) d.theta[c] = th;
   }
   double sn, cs;
-  sincos(th, &sn, &cs);
+  sincos_any(th, &sn, &cs);
   // ---- unwrap relative to entry 0 (R14); |r| >= L/2 is decided conservatively on the high
   // words with integer ALU operations, the exact minimum image runs only where that fires ----
   const unsigned hmin = min(hi_word(k.hLx), hi_word(k.hLy)), hlc = hi_word(k.lc2);
