@@ -135,7 +135,7 @@ __global__ void import_kernel(const Dev d, const Consts k, const int* __restrict
     d.minkey[i] = ~0ull;
     int n = d.cvn[i];
     n = n < 0 ? 0 : (n > k.S ? k.S : n);
-    for (int j = 0; j < k.S; ++j) row_entry(d.cv, k.N, i, j) = j < n ? cv_u[(size_t)i * k.S + j] : -1;   // normalise the padding
+    for (int j = 0; j < k.S; ++j) row_entry(d.cv, k.N, i, j) = cv_u[(size_t)i * k.S + (j < n ? j : 0)];   // padding repeats entry 0
   }
 }
 

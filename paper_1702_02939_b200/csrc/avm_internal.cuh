@@ -56,7 +56,7 @@ struct Consts {
 // Layout: everything is structure-of-arrays.
 //   vn, vc : three planes of Vs ints each: vn[k*Vs + v] = k-th neighbour of v (slot convention R12)
 //   cv     : fixed-stride padded rows stored as S/4 planes of int4: entries 4q..4q+3 of cell c are
-//            cv[q*N + c]; unused entries = -1.  A warp reads 32 consecutive cells' quads with one
+//            cv[q*N + c]; unused entries repeat entry 0 (always a valid index).  A warp reads 32 consecutive cells' quads with one
 //            fully coalesced 128-bit load per plane, and cells with <= 8 vertices (96 %) never
 //            touch planes 2, 3.
 struct Dev {

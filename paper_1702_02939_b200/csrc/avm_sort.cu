@@ -170,10 +170,8 @@ __global__ void permute_cells_kernel(const Dev a, const Dev b, const Consts k, c
   for (int q = 0; q < k.S / 4; ++q) {
     const int4 src = a.cv[(size_t)q * k.N + o];
     int4 dst;
-    dst.x = 4 * q + 0 < n ? newidx_v[src.x] : -1;
-    dst.y = 4 * q + 1 < n ? newidx_v[src.y] : -1;
-    dst.z = 4 * q + 2 < n ? newidx_v[src.z] : -1;
-    dst.w = 4 * q + 3 < n ? newidx_v[src.w] : -1;
+    // padding entries repeat entry 0, so every entry is a valid index
+    dst.x = newidx_v[src.x]; dst.y = newidx_v[src.y]; dst.z = newidx_v[src.z]; dst.w = newidx_v[src.w];
     b.cv[(size_t)q * k.N + i] = dst;
   }
 }

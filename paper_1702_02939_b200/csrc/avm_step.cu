@@ -268,12 +268,8 @@ cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts
   double th = ld_stream(d.theta + c);
   const unsigned int tag = (unsigned int)ld_stream(d.ctag + c);
   double2 h[8];
-  h[0] = __ldg(pos + e[0]);
 #pragma unroll
-  for (int j = 1; j < 8; ++j) {
-    h[j] = h[0];
-    if (j < n) h[j] = __ldg(pos + e[j]);
-  }
+  for (int j = 0; j < 8; ++j) h[j] = __ldg(pos + e[j]);   // padding entries repeat entry 0: r = 0, no predicate
   // ---- director (independent of the gathers above) ----
   if (kStep) {
     th += k.amp * director_noise(k, step, (unsigned long long)tag);
@@ -386,7 +382,7 @@ t1_flip_kernel(const Dev d, const Consts k, const unsigned parity, const bool co
 #pragma unroll
     for (int t = 0; t < 4; ++t) {
       nrow[t] = d.cvn[cells[t]];
-      row[t] = lane < k.S ? row_entry(d.cv, k.N, cells[t], lane) : -1;
+      row[t] = row_entry(d.cv, k.N, cells[t], lane < k.S ? lane : 0);
     }
     if (!__all_sync(kFull, mk == c.key)) { ++blocked; continue; }
     ++flips;
@@ -424,14 +420,16 @@ t1_flip_kernel(const Dev d, const Consts k, const unsigned parity, const bool co
         const int p = __ffs(__ballot_sync(kFull, lane < nrow[t] && r == victim)) - 1;
         const int nxt = __shfl_down_sync(kFull, r, 1);
         nnew[t] = nrow[t] - 1;
-        if (lane >= p) r = lane < nnew[t] ? nxt : -1;
+        if (lane >= p) r = nxt;
       } else {
         const int after = t == 2 ? v1 : v2, ins = t == 2 ? v2 : v1;
         const int p = __ffs(__ballot_sync(kFull, lane < nrow[t] && r == after)) - 1;
         const int prv = __shfl_up_sync(kFull, r, 1);
         nnew[t] = nrow[t] + 1;
-        if (lane > p) r = lane == p + 1 ? ins : (lane < nnew[t] ? prv : -1);
+        if (lane > p) r = lane == p + 1 ? ins : prv;
       }
+      const int r0 = __shfl_sync(kFull, r, 0);
+      if (lane >= nnew[t]) r = r0;                         // padding repeats entry 0
       if (lane < k.S && r != row[t]) row_entry(d.cv, k.N, cells[t], lane) = r;
       if (lane == 0) d.cvn[cells[t]] = nnew[t];
       row[t] = r;
