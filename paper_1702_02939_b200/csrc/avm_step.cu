@@ -445,20 +445,42 @@ t1_flip_kernel(const Dev d, const Consts k, const unsigned parity, const bool co
       const int v = row[t];
       if (lane < nnew[t]) hr[t] = v == v1 ? n1 : v == v2 ? n2 : d.pos[v];
     }
-    double myA = 0.0, myP = 0.0;
+    // lane j holds entry j of each row: unwrapped position (ux, uy) and the length of the edge
+    // that ENDS at entry j (lane 0: the closing edge), computed in parallel with geom_edge's
+    // arithmetic; the order-dependent sums then run as four interleaved serial chains.
+    double ux[4], uy[4], sl[4];
+    int nmax = 0;
 #pragma unroll
     for (int t = 0; t < 4; ++t) {
       const double h0x = __shfl_sync(kFull, hr[t].x, 0), h0y = __shfl_sync(kFull, hr[t].y, 0);
-      const double ux = min_image(__dsub_rn(hr[t].x, h0x), k.Lx, k.hLx), uy = min_image(__dsub_rn(hr[t].y, h0y), k.Ly, k.hLy);
-      double rxp = 0.0, ryp = 0.0, acc = 0.0, per = 0.0;
-      for (int j = 1; j <= nnew[t]; ++j) {
-        const int src = j < nnew[t] ? j : 0;       // j == n: the closing edge back to entry 0 (r = 0)
-        const double x = __shfl_sync(kFull, ux, src), y = __shfl_sync(kFull, uy, src);
-        geom_edge(rxp, ryp, x, y, acc, per);
-        rxp = x; ryp = y;
-      }
-      if (lane == t) { myA = __dmul_rn(0.5, acc); myP = per; }
+      ux[t] = min_image(__dsub_rn(hr[t].x, h0x), k.Lx, k.hLx);
+      uy[t] = min_image(__dsub_rn(hr[t].y, h0y), k.Ly, k.hLy);
+      const int prev = lane == 0 ? nnew[t] - 1 : lane - 1;
+      const double pxv = __shfl_sync(kFull, ux[t], prev), pyv = __shfl_sync(kFull, uy[t], prev);
+      const double dx = __dsub_rn(ux[t], pxv), dy = __dsub_rn(uy[t], pyv);
+      sl[t] = sqrt_pos(__fma_rn(dx, dx, __fma_rn(dy, dy, kTiny)));
+      nmax = max(nmax, nnew[t]);
     }
+    double rxp[4] = {0.0, 0.0, 0.0, 0.0}, ryp[4] = {0.0, 0.0, 0.0, 0.0}, acc[4] = {0.0, 0.0, 0.0, 0.0},
+           per[4] = {0.0, 0.0, 0.0, 0.0};
+    for (int j = 1; j <= nmax; ++j) {
+#pragma unroll
+      for (int t = 0; t < 4; ++t) {
+        if (j <= nnew[t]) {                          // warp-uniform
+          const int src = j < nnew[t] ? j : 0;       // j == n: the closing edge back to entry 0 (r = 0)
+          const double x = __shfl_sync(kFull, ux[t], src), y = __shfl_sync(kFull, uy[t], src);
+          const double l = __shfl_sync(kFull, sl[t], src);
+          acc[t] = __fma_rn(rxp[t], y, acc[t]);
+          acc[t] = __fma_rn(-ryp[t], x, acc[t]);
+          per[t] = __dadd_rn(per[t], l);
+          rxp[t] = x; ryp[t] = y;
+        }
+      }
+    }
+    double myA = 0.0, myP = 0.0;
+#pragma unroll
+    for (int t = 0; t < 4; ++t)
+      if (lane == t) { myA = __dmul_rn(0.5, acc[t]); myP = per[t]; }
     if (lane < 4) {
       const int cc = cells[lane == 0 ? 0 : lane == 1 ? 1 : lane == 2 ? 2 : 3];
       d.rec[cc].a = k.KA2 * (myA - k.A0);
