@@ -2,6 +2,7 @@
 // loop, state export in user order.  Host logic only enqueues work; the arithmetic of the hot
 // path lives in avm_step.cu / avm_sort.cu.
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -14,6 +15,10 @@ unsigned int hilbert_index_host(unsigned int x, unsigned int y, int m);
 }
 
 using namespace avm;
+
+#ifndef AVM_FUSED_T1
+#define AVM_FUSED_T1 1   // apply T1 flips in the prologue of the next force/move launch (two launches per step)
+#endif
 
 namespace {
 
@@ -41,7 +46,7 @@ struct BufferSet {
 
 struct Layout {
   size_t pos[2], vn[2], vc[2], cv[2], cvn[2], theta[2], rec[2], vtag[2], ctag[2];
-  size_t minkey, cand, ctr, ap, epart, key[2], val[2], hist, newidx_v, newidx_c, order_v, order_c;
+  size_t minkey, cand, ctr, dirty, ap, epart, key[2], val[2], hist, newidx_v, newidx_c, order_v, order_c;
   size_t total;
 };
 
@@ -59,6 +64,7 @@ Layout make_layout(const avm_params& p) {
   L.minkey = take(8 * N);
   L.cand = take(sizeof(Cand) * 3 * N);
   L.ctr = take(sizeof(Counters));
+  L.dirty = take(4 * ((V + 31) / 32));
   L.ap = take(16 * N);
   L.epart = take(8 * 1024);
   for (int i = 0; i < 2; ++i) { L.key[i] = take(4 * V); L.val[i] = take(4 * V); }
@@ -91,6 +97,8 @@ struct avm_sim {
   unsigned long long* minkey;
   Cand* cand;
   Counters* ctr;
+  unsigned int* dirty;
+  bool fused;            // T1 flips ride in force_move's prologue (cooperative launch available)
   double2* ap;
   double* epart;
   SortScratch sc;
@@ -104,7 +112,7 @@ struct avm_sim {
     const BufferSet& b = set[cur_set];
     d.vn = b.vn; d.vc = b.vc; d.cv = b.cv; d.cvn = b.cvn; d.theta = b.theta; d.rec = b.rec;
     d.vtag = b.vtag; d.ctag = b.ctag;
-    d.minkey = minkey; d.cand = cand; d.ctr = ctr;
+    d.minkey = minkey; d.cand = cand; d.ctr = ctr; d.dirty = dirty;
     return d;
   }
   Dev dev_alt() const {   // the other buffer set, target of a re-sort / staging area
@@ -255,6 +263,7 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   s->minkey = (unsigned long long*)(w + L.minkey);
   s->cand = (Cand*)(w + L.cand);
   s->ctr = (Counters*)(w + L.ctr);
+  s->dirty = (unsigned int*)(w + L.dirty);
   s->ap = (double2*)(w + L.ap);
   s->epart = (double*)(w + L.epart);
   s->sc.hist = (unsigned int*)(w + L.hist);
@@ -263,6 +272,7 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   s->cur_pos = 0; s->cur_set = 0;
   s->step = params->step0;
   s->n_sorts = 0; s->launches = 0;
+  s->fused = AVM_FUSED_T1 && !getenv("AVM_B200_UNFUSED");
 
   cudaStream_t st = s->stream;
   const cudaMemcpyKind kind = host_inputs ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
@@ -284,6 +294,7 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   AVM_CUDA_F(cudaMemcpyAsync(b.cvn, cvn, 4 * (size_t)N, kind, st));
   AVM_CUDA_F(cudaMemcpyAsync(b.theta, theta, 8 * (size_t)N, kind, st));
   AVM_CUDA_F(cudaMemsetAsync(s->ctr, 0, sizeof(Counters), st));
+  AVM_CUDA_F(cudaMemsetAsync(s->dirty, 0, 4 * (((size_t)V + 31) / 32), st));
   const Dev d = s->dev();
   import_kernel<<<cdiv(V, 256), 256, 0, st>>>(d, k, stage.vn, stage.vc, (const int*)stage.cv);
   validate_kernel<<<cdiv(V, 256), 256, 0, st>>>(d, k);
@@ -372,12 +383,25 @@ int avm_create_host(const avm_params* params, const double* pos_xy, const int32_
 
 int avm_step(avm_sim* s, int64_t n_steps) {
   if (!s || n_steps < 0) return AVM_EINVAL;
+  // Fused schedule: the flips of step i are applied by the force/move launch of step i+1, so
+  // the last step of this call (and the step before a re-sort) is completed by a flush.
+  bool pending = false;
   for (int64_t i = 0; i < n_steps; ++i) {
-    s->launches += launch_step(s->dev(), s->k, s->step, s->stream);
+    int n = -1;
+    if (s->fused) {
+      n = launch_step(s->dev(), s->k, s->step, s->stream, nullptr, true);
+      if (n < 0) s->fused = false; else pending = true;
+    }
+    if (n < 0) n = launch_step(s->dev(), s->k, s->step, s->stream, nullptr, false);
+    s->launches += n;
     s->cur_pos = 1 - s->cur_pos;
     ++s->step;
-    if (s->p.sort_every > 0 && (s->step - s->p.step0) % (unsigned long long)s->p.sort_every == 0) do_sort(s);
+    if (s->p.sort_every > 0 && (s->step - s->p.step0) % (unsigned long long)s->p.sort_every == 0) {
+      if (pending) { s->launches += launch_t1_flush(s->dev(), s->k, s->step - 1, s->stream); pending = false; }
+      do_sort(s);
+    }
   }
+  if (pending) s->launches += launch_t1_flush(s->dev(), s->k, s->step - 1, s->stream);
   AVM_CUDA(cudaPeekAtLastError());
   return AVM_OK;
 }

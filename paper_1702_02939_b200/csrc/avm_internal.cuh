@@ -32,7 +32,10 @@ struct Counters {
   // t1_flip(s) and its per-cell minimum keys are cleared by the prologue of force_move(s+1)
   unsigned int n_cand[2];
   unsigned int n_win;     // winners (debug hook only)
-  unsigned int pad;
+  unsigned int flip_done; // fused schedule: candidates decided so far          } zeroed by the
+  unsigned int next_cand; // fused schedule: next candidate index to be claimed  } cell pass of
+  unsigned int next_quad; // fused schedule: next candidate whose cells' flagged } every step
+  unsigned int pad;       //                 vertices are to be moved
   long long t1_short, t1_candidates, t1_flips, t1_blocked, overflow_rejects, error;
   double energy;
 };
@@ -72,6 +75,7 @@ struct Dev {
   int* ctag;          // [N] user index of each cell
   unsigned long long* minkey;  // [N] per-cell minimum candidate key, ~0 when idle
   Cand* cand;         // [3N]
+  unsigned int* dirty; // [ceil(V/32)] bit v: vertex v belongs to a cell of some pending T1 candidate
   Counters* ctr;
 };
 
@@ -200,7 +204,8 @@ __device__ __forceinline__ void cell_area_perimeter(const double2* pos, const in
 // host-side launchers (defined in the .cu files); every launcher returns the number of kernels
 // it enqueued so that the API can keep avm_stats.kernel_launches honest.
 // ---------------------------------------------------------------------------------------------
-int launch_step(const Dev& d, const Consts& k, unsigned long long step, cudaStream_t s, cudaEvent_t* ev = nullptr);
+int launch_step(const Dev& d, const Consts& k, unsigned long long step, cudaStream_t s, cudaEvent_t* ev = nullptr, bool fused = false);
+int launch_t1_flush(const Dev& d, const Consts& k, unsigned long long last_step, cudaStream_t s);
 int launch_refresh_cells(const Dev& d, const Consts& k, cudaStream_t s);
 int launch_t1_reset(const Dev& d, const Consts& k, cudaStream_t s);
 int launch_t1_pass_only(const Dev& d, const Consts& k, cudaStream_t s);

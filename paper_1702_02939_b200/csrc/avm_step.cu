@@ -18,6 +18,8 @@
 // Geometry is thus evaluated once per step on the positions the forces of the following step
 // act on; after a flip the records of its four cells are refreshed in place, so every force is
 // computed from the geometry of the current topology exactly as in the paper's cycle.
+#include <cstdio>
+#include <cstdlib>
 #include "avm_internal.cuh"
 
 namespace avm {
@@ -30,16 +32,22 @@ static constexpr unsigned kFull = 0xffffffffu;
 
 // tuning knobs (compile-time; the defaults are the measured best, profiles/)
 #ifndef AVM_FM_PF
-#define AVM_FM_PF 0        // force_move: L2 prefetch distance in grid sweeps (0 = off; measured: no gain, the pass is LSU-bound)
+#define AVM_FM_PF 1        // force_move: L2 prefetch distance in grid sweeps (0 = off)
 #endif
 #ifndef AVM_PDL
 #define AVM_PDL 1          // chain the step's kernels with programmatic dependent launch
+#endif
+#ifndef AVM_CU_MINB
+#define AVM_CU_MINB 9      // cell pass: resident CTAs per SM asked of the compiler (56 registers)
+#endif
+#ifndef AVM_FM_COOP
+#define AVM_FM_COOP 0       // launch the fused force_move as a cooperative grid (not needed: work is claimed, see flipper_work)
 #endif
 #ifndef AVM_FM_MINB
 #define AVM_FM_MINB 3      // force_move: minimum resident CTAs per SM asked of the compiler
 #endif
 #ifndef AVM_FM_REGPF
-#define AVM_FM_REGPF 1     // force_move: keep the next vertex's streaming loads in registers
+#define AVM_FM_REGPF 0     // force_move: keep the next vertex's streaming loads in registers (measured: the L2 prefetch does better)
 #endif
 
 // Programmatic dependent launch (sm_90+): the three kernels of a step form a chain on one stream.
@@ -110,33 +118,61 @@ __device__ __forceinline__ VertexIn load_vertex(const Dev& d, const Consts& k, i
   return in;
 }
 
-// Persistent grid-stride kernel: each thread keeps the streaming loads of its NEXT vertex in
-// flight while it gathers and computes the current one.
-__global__ void __launch_bounds__(kVertexBlock, AVM_FM_MINB)
-force_move_kernel(const Dev d, const Consts k, const unsigned parity) {
-  pdl_launch_dependents();
-  pdl_wait();
-  const int tid = blockIdx.x * kVertexBlock + threadIdx.x;
-  const int stride = gridDim.x * kVertexBlock;
-  {  // the previous step's T1 candidates are done: clear their cells' minimum keys (row a6)
-    const unsigned prev = d.ctr->n_cand[parity ^ 1u];
-    for (unsigned i = tid; i < prev; i += stride) {
-      const Cand c = d.cand[i];
-      d.minkey[c.cL] = ~0ull; d.minkey[c.cR] = ~0ull; d.minkey[c.cE1] = ~0ull; d.minkey[c.cE2] = ~0ull;
-    }
-    if (tid == 0) d.ctr->n_cand[parity] = 0;
+// Eq. 4: dh/dt = mu F + (v0/3) sum of the three unit directors (R5), directors of the start of
+// the step (R7); explicit Euler; wrap into the box (R13).
+__device__ __forceinline__ void move_vertex(const Dev& d, const Consts& k, int v, const double2 h, const double2 q0,
+                                            const double2 q1, const double2 q2, const CellRec& c0, const CellRec& c1,
+                                            const CellRec& c2) {
+  const double2 f = vertex_force(h, q0, q1, q2, c0, c1, c2, k);
+  const double vx = k.mu * f.x + k.v0_3 * (c0.nx + c1.nx + c2.nx);
+  const double vy = k.mu * f.y + k.v0_3 * (c0.ny + c1.ny + c2.ny);
+  double x = h.x + k.dt * vx, y = h.y + k.dt * vy;
+  // negative, >= L (conservatively) and non-finite values all have a large unsigned high word
+  if ((hi_word(x) >= hi_word(k.Lx)) | (hi_word(y) >= hi_word(k.Ly))) {
+    x = wrap_box(x, k.Lx); y = wrap_box(y, k.Ly);
+    if (!(isfinite(x) && isfinite(y))) atomicOr((unsigned long long*)&d.ctr->error, 1ull);
   }
-  int v = tid;
-  if (v >= k.V) return;
-  const unsigned hiLx = hi_word(k.Lx), hiLy = hi_word(k.Ly);
+  d.pos_next[v] = make_double2(x, y);
+}
+
+// the same vertex update with every input read from L2 (after another warp of this launch
+// rewrote the neighbourhood: L1 may hold stale lines)
+__device__ __noinline__ void move_vertex_coherent(const Dev& d, const Consts& k, int v) {
+  const double2 h = __ldcg(d.pos + v);
+  double2 q[3];
+  CellRec c[3];
+#pragma unroll
+  for (int s = 0; s < 3; ++s) {
+    q[s] = __ldcg(d.pos + __ldcg(d.vn + s * k.Vs + v));
+    const double2* r = reinterpret_cast<const double2*>(d.rec + __ldcg(d.vc + s * k.Vs + v));
+    const double2 ap = __ldcg(r), nn = __ldcg(r + 1);
+    c[s].a = ap.x; c[s].p = ap.y; c[s].nx = nn.x; c[s].ny = nn.y;
+  }
+  move_vertex(d, k, v, h, q[0], q[1], q[2], c[0], c[1], c[2]);
+}
+
+__device__ __forceinline__ unsigned int ld_volatile(const unsigned int* p) {
+  unsigned int x;
+  asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(x) : "l"(p) : "memory");
+  return x;
+}
+
+__device__ __noinline__ bool t1_try_flip(const Dev& d, const Consts& k, const Cand& c, const int lane);
+
+// The sweep of one thread over vertices first, first + step_v, ...  kSkipDirty: vertices
+// flagged in d.dirty are left to the flippers.
+template <bool kSkipDirty>
+__device__ __forceinline__ void sweep(const Dev& d, const Consts& k, const int first, const int step_v, const int lane) {
+  if (first >= k.V) return;
+  int v = first;
   VertexIn in = load_vertex(d, k, v);
-  const int lane = threadIdx.x & 31;
+  unsigned dw = kSkipDirty ? __ldg(d.dirty + (v >> 5)) : 0u;
   for (;;) {
     if (AVM_FM_PF) {
       // pull the contiguous streams of a later sweep into L2: positions, both index lists and the
       // cell records around v/2 (cells and vertices share the Hilbert order, so this window also
       // holds most of that sweep's gather targets)
-      const long long vb = (long long)(v - lane) + (long long)AVM_FM_PF * stride;
+      const long long vb = (long long)(v - lane) + (long long)AVM_FM_PF * step_v;
       if (vb + 32 <= k.V) {
         const char* a = nullptr;
         if (lane < 4) a = reinterpret_cast<const char*>(d.pos + vb) + 128 * lane;
@@ -146,26 +182,116 @@ force_move_kernel(const Dev d, const Consts k, const unsigned parity) {
         if (a) prefetch_l2(a);
       }
     }
-    const double2 q0 = __ldg(d.pos + in.n0), q1 = __ldg(d.pos + in.n1), q2 = __ldg(d.pos + in.n2);
-    const CellRec c0 = ld_rec(d.rec + in.c0), c1 = ld_rec(d.rec + in.c1), c2 = ld_rec(d.rec + in.c2);
-    const double2 h = in.h;
-    const int vnext = v + stride;
-    if (AVM_FM_REGPF && vnext < k.V) in = load_vertex(d, k, vnext);
-    const double2 f = vertex_force(h, q0, q1, q2, c0, c1, c2, k);
-    // Eq. 4: dh/dt = mu F + (v0/3) sum of the three unit directors (R5), directors of the start
-    // of the step (R7); explicit Euler; wrap into the box (R13)
-    const double vx = k.mu * f.x + k.v0_3 * (c0.nx + c1.nx + c2.nx);
-    const double vy = k.mu * f.y + k.v0_3 * (c0.ny + c1.ny + c2.ny);
-    double x = h.x + k.dt * vx, y = h.y + k.dt * vy;
-    // negative, >= L (conservatively) and non-finite values all have a large unsigned high word
-    if ((hi_word(x) >= hiLx) | (hi_word(y) >= hiLy)) {
-      x = wrap_box(x, k.Lx); y = wrap_box(y, k.Ly);
-      if (!(isfinite(x) && isfinite(y))) atomicOr((unsigned long long*)&d.ctr->error, 1ull);
+    const bool skip = kSkipDirty && ((dw >> (v & 31)) & 1u);
+    const int vnext = v + step_v;
+    if (!skip) {
+      const double2 q0 = __ldg(d.pos + in.n0), q1 = __ldg(d.pos + in.n1), q2 = __ldg(d.pos + in.n2);
+      const CellRec c0 = ld_rec(d.rec + in.c0), c1 = ld_rec(d.rec + in.c1), c2 = ld_rec(d.rec + in.c2);
+      const double2 h = in.h;
+      if (AVM_FM_REGPF && vnext < k.V) { in = load_vertex(d, k, vnext); if (kSkipDirty) dw = __ldg(d.dirty + (vnext >> 5)); }
+      move_vertex(d, k, v, h, q0, q1, q2, c0, c1, c2);
+    } else if (AVM_FM_REGPF && vnext < k.V) {
+      in = load_vertex(d, k, vnext);
+      dw = __ldg(d.dirty + (vnext >> 5));
     }
-    d.pos_next[v] = make_double2(x, y);
     if (vnext >= k.V) break;
     v = vnext;
-    if (!AVM_FM_REGPF) in = load_vertex(d, k, v);
+    if (!AVM_FM_REGPF) { in = load_vertex(d, k, v); if (kSkipDirty) dw = __ldg(d.dirty + (v >> 5)); }
+  }
+}
+
+// Rows a6 + a7 of the previous step inside the fused force_move launch, run by the "flipper"
+// warps (the first F warps of the grid, which take no share of the sweep).  Work is CLAIMED with
+// atomic counters, so a candidate always belongs to a warp that is running: the wait below can
+// never depend on a CTA that has not been scheduled yet (no co-residency assumption).
+//   1. claim candidates one by one; decide and flip each (t1_try_flip);
+//   2. wait until every candidate has been decided (flip_done == prev);
+//   3. claim candidates again: move the flagged vertices of the candidate's four cells with
+//      loads that bypass L1 (whoever clears a vertex's bit moves it) and release the cells'
+//      minimum keys (row a6).
+__device__ __noinline__ void flipper_work(const Dev& d, const Consts& k, const unsigned prev, const int lane) {
+  unsigned mine = 0, flips = 0;
+  for (;;) {
+    unsigned i = 0;
+    if (lane == 0) i = atomicAdd(&d.ctr->next_cand, 1u);
+    i = __shfl_sync(kFull, i, 0);
+    if (i >= prev) break;
+    const Cand c = d.cand[i];
+    if (t1_try_flip(d, k, c, lane)) ++flips;
+    ++mine;
+  }
+  if (mine) {
+    __threadfence();
+    __syncwarp();
+    if (lane == 0) {
+      if (flips) atomicAdd((unsigned long long*)&d.ctr->t1_flips, (unsigned long long)flips);
+      if (mine - flips) atomicAdd((unsigned long long*)&d.ctr->t1_blocked, (unsigned long long)(mine - flips));
+      atomicAdd(&d.ctr->flip_done, mine);
+    }
+  }
+  while (ld_volatile(&d.ctr->flip_done) < prev) __nanosleep(64);
+  __threadfence();
+  for (;;) {
+    unsigned i = 0;
+    if (lane == 0) i = atomicAdd(&d.ctr->next_quad, 1u);
+    i = __shfl_sync(kFull, i, 0);
+    if (i >= prev) break;
+    const Cand c = d.cand[i];
+    const int quad[4] = {c.cL, c.cR, c.cE1, c.cE2};
+#pragma unroll 1
+    for (int t = 0; t < 4; ++t) {
+      const int n = __ldcg(d.cvn + quad[t]);
+      if (lane < n) {
+        const int u = __ldcg(reinterpret_cast<const int*>(d.cv + (size_t)(lane >> 2) * k.N + quad[t]) + (lane & 3));
+        const unsigned bit = 1u << (u & 31);
+        if (atomicAnd(&d.dirty[u >> 5], ~bit) & bit) move_vertex_coherent(d, k, u);
+      }
+    }
+    if (lane < 4) d.minkey[quad[lane & 3]] = ~0ull;
+  }
+}
+
+// Persistent grid-stride kernel: each thread keeps the streaming loads of its NEXT vertex in
+// flight while it gathers and computes the current one.
+//
+// kFused (cooperative launch: every CTA is resident) also carries rows a6 + a7 of the PREVIOUS
+// step: warp i of the grid decides and flips candidate i of the previous step's list first
+// (t1_try_flip), while all other warps start moving vertices at once.  A vertex whose inputs a
+// flip may rewrite has its bit set in d.dirty (the marking thread flagged every vertex of the
+// candidate's four cells); such vertices are skipped in the main sweep and moved in a short
+// second sweep, after the grid-wide counter flip_done shows that every candidate has been
+// decided, with loads that bypass L1.  The latency-bound flips thus overlap the bandwidth-bound
+// sweep and the step needs no third launch.
+template <bool kFused>
+__global__ void __launch_bounds__(kVertexBlock, AVM_FM_MINB)
+force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, const unsigned parity) {
+  pdl_launch_dependents();
+  pdl_wait();
+  const int tid = blockIdx.x * kVertexBlock + threadIdx.x;
+  const int stride = gridDim.x * kVertexBlock;
+  const int lane = threadIdx.x & 31;
+  const unsigned prev = d.ctr->n_cand[parity ^ 1u];
+  const unsigned gwarp = (unsigned)tid >> 5, nwarps = (unsigned)stride >> 5;
+  if (tid == 0) d.ctr->n_cand[parity] = 0;
+  if (kFused) {
+    // the first F warps flip, all others sweep (a one-warp grid does both, one after the other)
+    const unsigned F = nwarps > 1 ? min(prev, nwarps / 2u) : 0u;
+    if (tid == 0 && prev) atomicAdd((unsigned long long*)&d.ctr->t1_candidates, (unsigned long long)prev);
+    if (gwarp < F) {
+      flipper_work(d, k, prev, lane);
+    } else {
+      if (nwarps == 1 && prev) flipper_work(d, k, prev, lane);
+      const int first = (int)(gwarp - F) * 32 + lane, step_v = (int)(nwarps - F) * 32;
+      if (prev && nwarps > 1) sweep<true>(d, k, first, step_v, lane);
+      else sweep<false>(d, k, first, step_v, lane);
+    }
+  } else {
+    // the previous step's T1 candidates are done: clear their cells' minimum keys (row a6)
+    for (unsigned i = tid; i < prev; i += stride) {
+      const Cand c = d.cand[i];
+      d.minkey[c.cL] = ~0ull; d.minkey[c.cR] = ~0ull; d.minkey[c.cE1] = ~0ull; d.minkey[c.cE2] = ~0ull;
+    }
+    sweep<false>(d, k, tid, stride, lane);
   }
 }
 
@@ -194,8 +320,9 @@ __device__ __noinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va,
   const int cR = d.vc[k2 * k.Vs + v2], cE2 = d.vc[((k2 + 1) % 3) * k.Vs + v2];
   const bool distinct = cL != cR && cL != cE1 && cL != cE2 && cR != cE1 && cR != cE2 && cE1 != cE2;
   if (!distinct) return;
-  if (!(d.cvn[cL] > 3 && d.cvn[cR] > 3)) return;               // no 2-gons (T2 absent)
-  if (!(d.cvn[cE1] < k.S && d.cvn[cE2] < k.S)) {               // row would exceed the stride
+  const int nq[4] = {d.cvn[cL], d.cvn[cR], d.cvn[cE1], d.cvn[cE2]};
+  if (!(nq[0] > 3 && nq[1] > 3)) return;                       // no 2-gons (T2 absent)
+  if (!(nq[2] < k.S && nq[3] < k.S)) {                         // row would exceed the stride
     if (count_stats) {
       atomicAdd((unsigned long long*)&d.ctr->overflow_rejects, 1ull);
       atomicOr((unsigned long long*)&d.ctr->error, 2ull);
@@ -221,6 +348,28 @@ __device__ __noinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va,
   atomicMin(&d.minkey[cR], cd.key);
   atomicMin(&d.minkey[cE1], cd.key);
   atomicMin(&d.minkey[cE2], cd.key);
+  // Everything a flip of this edge would write, and everything that reads it in the next
+  // force/move pass, belongs to a vertex of these four cells: flag them, so that the fused
+  // prologue of force_move can run the flips while the untouched vertices already move.
+#ifndef AVM_EXP_NOMARK
+  if (count_stats) {
+    const int quad[4] = {cL, cR, cE1, cE2};
+    // rows first (independent vector loads), then fire-and-forget reductions
+    int4 q[4][2];
+#pragma unroll
+    for (int t = 0; t < 4; ++t) { q[t][0] = d.cv[quad[t]]; q[t][1] = d.cv[(size_t)k.N + quad[t]]; }
+#pragma unroll
+    for (int t = 0; t < 4; ++t) {
+      const int e[8] = {q[t][0].x, q[t][0].y, q[t][0].z, q[t][0].w, q[t][1].x, q[t][1].y, q[t][1].z, q[t][1].w};
+#pragma unroll
+      for (int j = 0; j < 8; ++j) atomicOr(&d.dirty[e[j] >> 5], 1u << (e[j] & 31));   // padding repeats entry 0
+      for (int j = 8; j < nq[t]; ++j) {
+        const int u = row_entry(d.cv, k.N, quad[t], j);
+        atomicOr(&d.dirty[u >> 5], 1u << (u & 31));
+      }
+    }
+  }
+#endif
 }
 
 // The geometry pass flagged edges of cell c (bit j-1 = the edge ending at row entry j, j = n
@@ -253,12 +402,13 @@ __device__ __noinline__ void t1_report_cell(const Dev& d, const Consts& k, int c
 // so each pass starts on the lines the previous pass touched last (L2 recency).
 // ---------------------------------------------------------------------------------------------
 template <bool kStep>
-__global__ void __launch_bounds__(kCellBlock)
+__global__ void __launch_bounds__(kCellBlock, AVM_CU_MINB)
 cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, const unsigned long long step,
                    const unsigned parity) {
   pdl_launch_dependents();
   pdl_wait();
   const int gid = blockIdx.x * kCellBlock + threadIdx.x;
+  if (kStep && gid == 0) { d.ctr->flip_done = 0; d.ctr->next_cand = 0; d.ctr->next_quad = 0; }   // the previous list is long done
   const bool valid = gid < k.N;
   const int c = valid ? k.N - 1 - gid : 0;
   const double2* __restrict__ pos = d.pos;
@@ -357,8 +507,132 @@ __global__ void detect_mark_kernel(const __grid_constant__ Dev d, const __grid_c
 // therefore own disjoint cell quadruples and every word written below belongs to a vertex or row
 // inside the winner's own quadruple.  minkey is only read here (cleared by the next force_move).
 // ---------------------------------------------------------------------------------------------
+// One candidate, one warp: decide (R11) and, if it wins, flip and rewrite (R9, R12).  Returns
+// whether the edge flipped.  Used by the stand-alone T1 kernel and by force_move's fused prologue.
+__device__ __noinline__ bool t1_try_flip(const Dev& d, const Consts& k, const Cand& c, const int lane) {
+  const int cells[4] = {c.cL, c.cR, c.cE1, c.cE2};
+  const int l4 = lane & 3;
+  // ---- everything is read before anything is written; the loads below are independent of
+  // one another (the marking thread decoded the neighbourhood), so the minimum-key test
+  // costs no extra round trip ----
+  const unsigned long long mk = d.minkey[l4 == 0 ? c.cL : l4 == 1 ? c.cR : l4 == 2 ? c.cE1 : c.cE2];
+  const int v1 = c.v1, v2 = c.v2, k1 = c.k1, k2 = c.k2;
+  const int a1 = (k1 + 1) % 3, b1 = (k1 + 2) % 3, a2 = (k2 + 1) % 3, b2 = (k2 + 2) % 3;
+  const double2 h1 = d.pos[v1], h2 = d.pos[v2];
+  const int x1 = c.x1, y1 = c.y1, x2 = c.x2, y2 = c.y2;
+  int row[4], nrow[4];
+#pragma unroll
+  for (int t = 0; t < 4; ++t) {
+    nrow[t] = d.cvn[cells[t]];
+    row[t] = row_entry(d.cv, k.N, cells[t], lane < k.S ? lane : 0);
+  }
+  if (!__all_sync(kFull, mk == c.key)) return false;
+  // ---- geometry: rigid counter-clockwise quarter turn about the midpoint, new length 1.5 l_c (R9)
+  const double dx = min_image(h2.x - h1.x, k.Lx, k.hLx), dy = min_image(h2.y - h1.y, k.Ly, k.hLy);
+  const double l = sqrt(dx * dx + dy * dy);
+  const double mx = h1.x + 0.5 * dx, my = h1.y + 0.5 * dy;
+  double px = 0.0, py = 1.0;
+  if (l > 0.0) { px = -dy / l; py = dx / l; }
+  const double half = 0.75 * k.lc;
+  const double2 n2 = make_double2(wrap_box(mx + half * px, k.Lx), wrap_box(my + half * py, k.Ly));
+  const double2 n1 = make_double2(wrap_box(mx - half * px, k.Lx), wrap_box(my - half * py, k.Ly));
+  if (lane == 0) {
+    d.pos[v2] = n2;
+    d.pos[v1] = n1;
+    // lists: u = ([w, x, y]; [C0, C1, C2]) cyclic from the partner slot
+    //     -> ([w, y, z]; [C1, C2, C']), z = partner's old x, C' = partner's old C1 (R12)
+    d.vn[a1 * k.Vs + v1] = y1; d.vn[b1 * k.Vs + v1] = x2;
+    d.vc[k1 * k.Vs + v1] = c.cE1; d.vc[a1 * k.Vs + v1] = c.cR; d.vc[b1 * k.Vs + v1] = c.cE2;
+    d.vn[a2 * k.Vs + v2] = y2; d.vn[b2 * k.Vs + v2] = x1;
+    d.vc[k2 * k.Vs + v2] = c.cE2; d.vc[a2 * k.Vs + v2] = c.cL; d.vc[b2 * k.Vs + v2] = c.cE1;
+  }
+  // outer vertices: x1 was joined to v1 and is now joined to v2 (same slot); x2 likewise
+  if (lane == 1) d.vn[c.sx1 * k.Vs + x1] = v2;
+  if (lane == 2) d.vn[c.sx2 * k.Vs + x2] = v1;
+  // rows (lane = row entry): L deletes v1, R deletes v2 (later entries shift down); E1 inserts
+  // v2 immediately after v1, E2 inserts v1 immediately after v2 (later entries shift up).
+  // The new rows are formed in registers, written back, and reused by the refresh below.
+  int nnew[4];
+#pragma unroll
+  for (int t = 0; t < 4; ++t) {
+    int r = row[t];
+    if (t < 2) {
+      const int victim = t == 0 ? v1 : v2;
+      const int p = __ffs(__ballot_sync(kFull, lane < nrow[t] && r == victim)) - 1;
+      const int nxt = __shfl_down_sync(kFull, r, 1);
+      nnew[t] = nrow[t] - 1;
+      if (lane >= p) r = nxt;
+    } else {
+      const int after = t == 2 ? v1 : v2, ins = t == 2 ? v2 : v1;
+      const int p = __ffs(__ballot_sync(kFull, lane < nrow[t] && r == after)) - 1;
+      const int prv = __shfl_up_sync(kFull, r, 1);
+      nnew[t] = nrow[t] + 1;
+      if (lane > p) r = lane == p + 1 ? ins : prv;
+    }
+    const int r0 = __shfl_sync(kFull, r, 0);
+    if (lane >= nnew[t]) r = r0;                         // padding repeats entry 0
+    if (lane < k.S && r != row[t]) row_entry(d.cv, k.N, cells[t], lane) = r;
+    if (lane == 0) d.cvn[cells[t]] = nnew[t];
+    row[t] = r;
+  }
+  // refresh the cached geometry of the four cells (directors unchanged): every lane fetches
+  // the position of "its" entry of each row (v1 and v2 take their new positions from
+  // registers), then the warp runs the same serial sum as the per-step pass, so that a resumed
+  // run reproduces these records bit for bit.  Lane t keeps cell t's result.
+  double2 hr[4];
+#pragma unroll
+  for (int t = 0; t < 4; ++t) {
+    hr[t] = make_double2(0.0, 0.0);
+    const int v = row[t];
+    if (lane < nnew[t]) hr[t] = v == v1 ? n1 : v == v2 ? n2 : d.pos[v];
+  }
+  // lane j holds entry j of each row: unwrapped position (ux, uy) and the length of the edge
+  // that ENDS at entry j (lane 0: the closing edge), computed in parallel with geom_edge's
+  // arithmetic; the order-dependent sums then run as four interleaved serial chains.
+  double ux[4], uy[4], sl[4];
+  int nmax = 0;
+#pragma unroll
+  for (int t = 0; t < 4; ++t) {
+    const double h0x = __shfl_sync(kFull, hr[t].x, 0), h0y = __shfl_sync(kFull, hr[t].y, 0);
+    ux[t] = min_image(__dsub_rn(hr[t].x, h0x), k.Lx, k.hLx);
+    uy[t] = min_image(__dsub_rn(hr[t].y, h0y), k.Ly, k.hLy);
+    const int prev = lane == 0 ? nnew[t] - 1 : lane - 1;
+    const double pxv = __shfl_sync(kFull, ux[t], prev), pyv = __shfl_sync(kFull, uy[t], prev);
+    const double dx = __dsub_rn(ux[t], pxv), dy = __dsub_rn(uy[t], pyv);
+    sl[t] = sqrt_pos(__fma_rn(dx, dx, __fma_rn(dy, dy, kTiny)));
+    nmax = max(nmax, nnew[t]);
+  }
+  double rxp[4] = {0.0, 0.0, 0.0, 0.0}, ryp[4] = {0.0, 0.0, 0.0, 0.0}, acc[4] = {0.0, 0.0, 0.0, 0.0},
+         per[4] = {0.0, 0.0, 0.0, 0.0};
+  for (int j = 1; j <= nmax; ++j) {
+#pragma unroll
+    for (int t = 0; t < 4; ++t) {
+      if (j <= nnew[t]) {                          // warp-uniform
+        const int src = j < nnew[t] ? j : 0;       // j == n: the closing edge back to entry 0 (r = 0)
+        const double x = __shfl_sync(kFull, ux[t], src), y = __shfl_sync(kFull, uy[t], src);
+        const double l = __shfl_sync(kFull, sl[t], src);
+        acc[t] = __fma_rn(rxp[t], y, acc[t]);
+        acc[t] = __fma_rn(-ryp[t], x, acc[t]);
+        per[t] = __dadd_rn(per[t], l);
+        rxp[t] = x; ryp[t] = y;
+      }
+    }
+  }
+  double myA = 0.0, myP = 0.0;
+#pragma unroll
+  for (int t = 0; t < 4; ++t)
+    if (lane == t) { myA = __dmul_rn(0.5, acc[t]); myP = per[t]; }
+  if (lane < 4) {
+    const int cc = cells[lane == 0 ? 0 : lane == 1 ? 1 : lane == 2 ? 2 : 3];
+    d.rec[cc].a = k.KA2 * (myA - k.A0);
+    d.rec[cc].p = k.KP2 * (myP - k.P0);
+  }
+  __syncwarp();
+  return true;
+}
+
 __global__ void __launch_bounds__(kT1Block)
-t1_flip_kernel(const Dev d, const Consts k, const unsigned parity, const bool count_stats) {
+t1_flip_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, const unsigned parity, const bool count_stats) {
   pdl_launch_dependents();
   pdl_wait();
   const unsigned int n_cand = d.ctr->n_cand[parity];
@@ -368,125 +642,7 @@ t1_flip_kernel(const Dev d, const Consts k, const unsigned parity, const bool co
   unsigned int flips = 0, blocked = 0;
   for (unsigned int i = gwarp; i < n_cand; i += nwarps) {
     const Cand c = d.cand[i];
-    const int cells[4] = {c.cL, c.cR, c.cE1, c.cE2};
-    const int l4 = lane & 3;
-    // ---- everything is read before anything is written; the loads below are independent of
-    // one another (the marking thread decoded the neighbourhood), so the minimum-key test
-    // costs no extra round trip ----
-    const unsigned long long mk = d.minkey[l4 == 0 ? c.cL : l4 == 1 ? c.cR : l4 == 2 ? c.cE1 : c.cE2];
-    const int v1 = c.v1, v2 = c.v2, k1 = c.k1, k2 = c.k2;
-    const int a1 = (k1 + 1) % 3, b1 = (k1 + 2) % 3, a2 = (k2 + 1) % 3, b2 = (k2 + 2) % 3;
-    const double2 h1 = d.pos[v1], h2 = d.pos[v2];
-    const int x1 = c.x1, y1 = c.y1, x2 = c.x2, y2 = c.y2;
-    int row[4], nrow[4];
-#pragma unroll
-    for (int t = 0; t < 4; ++t) {
-      nrow[t] = d.cvn[cells[t]];
-      row[t] = row_entry(d.cv, k.N, cells[t], lane < k.S ? lane : 0);
-    }
-    if (!__all_sync(kFull, mk == c.key)) { ++blocked; continue; }
-    ++flips;
-    // ---- geometry: rigid counter-clockwise quarter turn about the midpoint, new length 1.5 l_c (R9)
-    const double dx = min_image(h2.x - h1.x, k.Lx, k.hLx), dy = min_image(h2.y - h1.y, k.Ly, k.hLy);
-    const double l = sqrt(dx * dx + dy * dy);
-    const double mx = h1.x + 0.5 * dx, my = h1.y + 0.5 * dy;
-    double px = 0.0, py = 1.0;
-    if (l > 0.0) { px = -dy / l; py = dx / l; }
-    const double half = 0.75 * k.lc;
-    const double2 n2 = make_double2(wrap_box(mx + half * px, k.Lx), wrap_box(my + half * py, k.Ly));
-    const double2 n1 = make_double2(wrap_box(mx - half * px, k.Lx), wrap_box(my - half * py, k.Ly));
-    if (lane == 0) {
-      d.pos[v2] = n2;
-      d.pos[v1] = n1;
-      // lists: u = ([w, x, y]; [C0, C1, C2]) cyclic from the partner slot
-      //     -> ([w, y, z]; [C1, C2, C']), z = partner's old x, C' = partner's old C1 (R12)
-      d.vn[a1 * k.Vs + v1] = y1; d.vn[b1 * k.Vs + v1] = x2;
-      d.vc[k1 * k.Vs + v1] = c.cE1; d.vc[a1 * k.Vs + v1] = c.cR; d.vc[b1 * k.Vs + v1] = c.cE2;
-      d.vn[a2 * k.Vs + v2] = y2; d.vn[b2 * k.Vs + v2] = x1;
-      d.vc[k2 * k.Vs + v2] = c.cE2; d.vc[a2 * k.Vs + v2] = c.cL; d.vc[b2 * k.Vs + v2] = c.cE1;
-    }
-    // outer vertices: x1 was joined to v1 and is now joined to v2 (same slot); x2 likewise
-    if (lane == 1) d.vn[c.sx1 * k.Vs + x1] = v2;
-    if (lane == 2) d.vn[c.sx2 * k.Vs + x2] = v1;
-    // rows (lane = row entry): L deletes v1, R deletes v2 (later entries shift down); E1 inserts
-    // v2 immediately after v1, E2 inserts v1 immediately after v2 (later entries shift up).
-    // The new rows are formed in registers, written back, and reused by the refresh below.
-    int nnew[4];
-#pragma unroll
-    for (int t = 0; t < 4; ++t) {
-      int r = row[t];
-      if (t < 2) {
-        const int victim = t == 0 ? v1 : v2;
-        const int p = __ffs(__ballot_sync(kFull, lane < nrow[t] && r == victim)) - 1;
-        const int nxt = __shfl_down_sync(kFull, r, 1);
-        nnew[t] = nrow[t] - 1;
-        if (lane >= p) r = nxt;
-      } else {
-        const int after = t == 2 ? v1 : v2, ins = t == 2 ? v2 : v1;
-        const int p = __ffs(__ballot_sync(kFull, lane < nrow[t] && r == after)) - 1;
-        const int prv = __shfl_up_sync(kFull, r, 1);
-        nnew[t] = nrow[t] + 1;
-        if (lane > p) r = lane == p + 1 ? ins : prv;
-      }
-      const int r0 = __shfl_sync(kFull, r, 0);
-      if (lane >= nnew[t]) r = r0;                         // padding repeats entry 0
-      if (lane < k.S && r != row[t]) row_entry(d.cv, k.N, cells[t], lane) = r;
-      if (lane == 0) d.cvn[cells[t]] = nnew[t];
-      row[t] = r;
-    }
-    // refresh the cached geometry of the four cells (directors unchanged): every lane fetches
-    // the position of "its" entry of each row (v1 and v2 take their new positions from
-    // registers), then the warp runs the same serial sum as the per-step pass, so that a resumed
-    // run reproduces these records bit for bit.  Lane t keeps cell t's result.
-    double2 hr[4];
-#pragma unroll
-    for (int t = 0; t < 4; ++t) {
-      hr[t] = make_double2(0.0, 0.0);
-      const int v = row[t];
-      if (lane < nnew[t]) hr[t] = v == v1 ? n1 : v == v2 ? n2 : d.pos[v];
-    }
-    // lane j holds entry j of each row: unwrapped position (ux, uy) and the length of the edge
-    // that ENDS at entry j (lane 0: the closing edge), computed in parallel with geom_edge's
-    // arithmetic; the order-dependent sums then run as four interleaved serial chains.
-    double ux[4], uy[4], sl[4];
-    int nmax = 0;
-#pragma unroll
-    for (int t = 0; t < 4; ++t) {
-      const double h0x = __shfl_sync(kFull, hr[t].x, 0), h0y = __shfl_sync(kFull, hr[t].y, 0);
-      ux[t] = min_image(__dsub_rn(hr[t].x, h0x), k.Lx, k.hLx);
-      uy[t] = min_image(__dsub_rn(hr[t].y, h0y), k.Ly, k.hLy);
-      const int prev = lane == 0 ? nnew[t] - 1 : lane - 1;
-      const double pxv = __shfl_sync(kFull, ux[t], prev), pyv = __shfl_sync(kFull, uy[t], prev);
-      const double dx = __dsub_rn(ux[t], pxv), dy = __dsub_rn(uy[t], pyv);
-      sl[t] = sqrt_pos(__fma_rn(dx, dx, __fma_rn(dy, dy, kTiny)));
-      nmax = max(nmax, nnew[t]);
-    }
-    double rxp[4] = {0.0, 0.0, 0.0, 0.0}, ryp[4] = {0.0, 0.0, 0.0, 0.0}, acc[4] = {0.0, 0.0, 0.0, 0.0},
-           per[4] = {0.0, 0.0, 0.0, 0.0};
-    for (int j = 1; j <= nmax; ++j) {
-#pragma unroll
-      for (int t = 0; t < 4; ++t) {
-        if (j <= nnew[t]) {                          // warp-uniform
-          const int src = j < nnew[t] ? j : 0;       // j == n: the closing edge back to entry 0 (r = 0)
-          const double x = __shfl_sync(kFull, ux[t], src), y = __shfl_sync(kFull, uy[t], src);
-          const double l = __shfl_sync(kFull, sl[t], src);
-          acc[t] = __fma_rn(rxp[t], y, acc[t]);
-          acc[t] = __fma_rn(-ryp[t], x, acc[t]);
-          per[t] = __dadd_rn(per[t], l);
-          rxp[t] = x; ryp[t] = y;
-        }
-      }
-    }
-    double myA = 0.0, myP = 0.0;
-#pragma unroll
-    for (int t = 0; t < 4; ++t)
-      if (lane == t) { myA = __dmul_rn(0.5, acc[t]); myP = per[t]; }
-    if (lane < 4) {
-      const int cc = cells[lane == 0 ? 0 : lane == 1 ? 1 : lane == 2 ? 2 : 3];
-      d.rec[cc].a = k.KA2 * (myA - k.A0);
-      d.rec[cc].p = k.KP2 * (myP - k.P0);
-    }
-    __syncwarp();
+    if (t1_try_flip(d, k, c, lane)) ++flips; else ++blocked;
   }
   if (count_stats && lane == 0) {
     if (flips) atomicAdd((unsigned long long*)&d.ctr->t1_flips, (unsigned long long)flips);
@@ -505,7 +661,7 @@ t1_reset_kernel(const Dev d) {
     d.minkey[c.cL] = ~0ull; d.minkey[c.cR] = ~0ull; d.minkey[c.cE1] = ~0ull; d.minkey[c.cE2] = ~0ull;
   }
 }
-__global__ void zero_counts_kernel(const Dev d) { d.ctr->n_cand[0] = 0; d.ctr->n_cand[1] = 0; d.ctr->n_win = 0; }
+__global__ void zero_counts_kernel(const Dev d) { d.ctr->n_cand[0] = 0; d.ctr->n_cand[1] = 0; d.ctr->n_win = 0; d.ctr->flip_done = 0; d.ctr->next_cand = 0; d.ctr->next_quad = 0; }
 
 // debug hook: winners without flipping; (tag_min, tag_max) pairs out
 __global__ void t1_debug_kernel(const Dev d, int* cand_pairs, int* win_pairs, long long capacity) {
@@ -608,7 +764,10 @@ static int force_move_grid(const Consts& k) {
   // persistent: a whole number of CTAs per SM (148 SMs), never more CTAs than there is work
   static int per_sm = 0;
   if (!per_sm) {
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, force_move_kernel, kVertexBlock, 0);
+    int a = 0, b = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, force_move_kernel<true>, kVertexBlock, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, force_move_kernel<false>, kVertexBlock, 0);
+    per_sm = a < b ? a : b;
     if (per_sm < 1) per_sm = 1;
   }
   const int want = cdiv(k.V, kVertexBlock);
@@ -616,34 +775,59 @@ static int force_move_grid(const Consts& k) {
   return want < cap ? want : cap;
 }
 
-// Launch with the programmatic-stream-serialization attribute (see pdl_wait above).
+// Launch with the programmatic-stream-serialization attribute (see pdl_wait above) and,
+// optionally, as a cooperative grid (every CTA resident: force_move<true> spins on a counter
+// that other CTAs advance).
 template <typename... KArgs, typename... Args>
-static void launch_chained(void (*kernel)(KArgs...), int grid, int block, cudaStream_t s, bool pdl, Args... args) {
+static cudaError_t launch_chained(void (*kernel)(KArgs...), int grid, int block, cudaStream_t s, bool pdl, bool coop,
+                                  Args... args) {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block); cfg.dynamicSmemBytes = 0; cfg.stream = s;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
-  cfg.attrs = attr; cfg.numAttrs = 1;
-  cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+  cudaLaunchAttribute attr[2];
+  int na = 0;
+  if (pdl) { attr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization; attr[na].val.programmaticStreamSerializationAllowed = 1; ++na; }
+  if (coop) { attr[na].id = cudaLaunchAttributeCooperative; attr[na].val.cooperative = 1; ++na; }
+  cfg.attrs = attr; cfg.numAttrs = (unsigned)na;
+  return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
 // One timestep.  d.pos = positions at the start of the step, d.pos_next = buffer for the moved
 // positions (the caller swaps them afterwards).
+//   fused = true : two launches; the T1 flips of the PREVIOUS step ride in force_move's
+//                  prologue, those of this step stay pending (launch_t1_flush applies them).
+//   fused = false: three launches, each step complete on return (also the per-kernel timing mode).
 // ev (optional, AVM_K_COUNT+1 events): recorded before/after each kernel by avm_step_profile.
-int launch_step(const Dev& d, const Consts& k, unsigned long long step, cudaStream_t s, cudaEvent_t* ev) {
+int launch_step(const Dev& d, const Consts& k, unsigned long long step, cudaStream_t s, cudaEvent_t* ev, bool fused) {
   const unsigned parity = (unsigned)(step & 1ull);
   if (ev) cudaEventRecord(ev[0], s);
   const bool pdl = AVM_PDL && ev == nullptr;   // events between the kernels would break the chain anyway
-  launch_chained(force_move_kernel, force_move_grid(k), kVertexBlock, s, pdl, d, k, parity);
+  static int coop_pdl_ok = 1;                  // cooperative + programmatic launch accepted by this driver?
+  if (fused) {
+    cudaError_t e = cudaErrorUnknown;
+    if (pdl && coop_pdl_ok) {
+      e = launch_chained(force_move_kernel<true>, force_move_grid(k), kVertexBlock, s, true, AVM_FM_COOP != 0, d, k, parity);
+      if (e != cudaSuccess) { coop_pdl_ok = 0; cudaGetLastError(); if (getenv("AVM_B200_DEBUG")) fprintf(stderr, "avm: cooperative+programmatic launch rejected\n"); }
+    }
+    if (e != cudaSuccess) e = launch_chained(force_move_kernel<true>, force_move_grid(k), kVertexBlock, s, false, AVM_FM_COOP != 0, d, k, parity);
+    if (e != cudaSuccess) return -1;           // the caller falls back to the unfused schedule
+  } else {
+    launch_chained(force_move_kernel<false>, force_move_grid(k), kVertexBlock, s, pdl, false, d, k, parity);
+  }
   if (ev) cudaEventRecord(ev[1], s);
   Dev m = d;                      // from here on the moved positions are "the" positions
   m.pos = d.pos_next; m.pos_next = d.pos;
-  launch_chained(cell_update_kernel<true>, cdiv(k.N, kCellBlock), kCellBlock, s, pdl, m, k, step, parity);
+  launch_chained(cell_update_kernel<true>, cdiv(k.N, kCellBlock), kCellBlock, s, pdl, false, m, k, step, parity);
   if (ev) cudaEventRecord(ev[2], s);
-  launch_chained(t1_flip_kernel, kT1Grid, kT1Block, s, pdl, m, k, parity, true);
+  if (!fused) launch_chained(t1_flip_kernel, kT1Grid, kT1Block, s, pdl, false, m, k, parity, true);
   if (ev) cudaEventRecord(ev[3], s);
-  return 3;
+  return fused ? 2 : 3;
+}
+
+// Applies the flips a fused step left pending (d = the state after that step) and leaves the T1
+// work lists idle, so that any other entry point sees a complete step.
+int launch_t1_flush(const Dev& d, const Consts& k, unsigned long long last_step, cudaStream_t s) {
+  t1_flip_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, k, (unsigned)(last_step & 1ull), true);
+  return 1 + launch_t1_reset(d, k, s);
 }
 
 int launch_refresh_cells(const Dev& d, const Consts& k, cudaStream_t s) {
@@ -655,6 +839,7 @@ int launch_refresh_cells(const Dev& d, const Consts& k, cudaStream_t s) {
 int launch_t1_reset(const Dev& d, const Consts& k, cudaStream_t s) {
   t1_reset_kernel<<<kT1Grid, kT1Block, 0, s>>>(d);
   zero_counts_kernel<<<1, 1, 0, s>>>(d);
+  cudaMemsetAsync(d.dirty, 0, sizeof(unsigned int) * (size_t)((k.V + 31) / 32), s);
   return 2;
 }
 
