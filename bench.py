@@ -84,6 +84,23 @@ class ClockSampler:
                 "samples": len(self.sm)}
 
 
+def max_over_ranks(ms: float, dist, device: str) -> float:
+    """Replicas only: ranks share nothing but the clock.  The job's time is the
+    slowest rank's device time; this all-reduce of one scalar is the only collective in bench.py
+    (never on the data path).  `dist` is torch.distributed or None (single process)."""
+    if dist is None:
+        return float(ms)
+    import torch
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(units_per_rank: float, steps: int, ms: float, world: int) -> float:
+    """whole-job throughput: every rank advances its own replica of the workload (weak scaling)"""
+    return world * units_per_rank * steps / (ms * 1e-3)
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle as it stands, rank 0 only, on a bounded sample of the
     workload (a smaller tiling of the same recipe and density) so that K+W steps end in minutes."""
@@ -177,11 +194,8 @@ def main():
     barrier()
     ms = e0.elapsed_time(e1)
     st1 = sim.stats()
-    if dist is not None:
-        tms = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-        ms = float(tms.item())
-    value = world * V * args.steps / (ms * 1e-3)
+    ms = max_over_ranks(ms, dist, "cuda")
+    value = aggregate_value(V, args.steps, ms, world)
 
     # ---------------- per-kernel device time (CUDA events inside the library) --------------------
     prof = sim.step_profile(args.profile_steps)
@@ -228,11 +242,8 @@ def main():
             s2.close()
             del s2
         e2e_t = e2e_ms[-1]
-        if dist is not None:
-            tms = torch.tensor([e2e_t], device="cuda", dtype=torch.float64)
-            dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-            e2e_t = float(tms.item())
-        e2e = {"value": world * V * args.steps / (e2e_t * 1e-3), "unit": UNIT,
+        e2e_t = max_over_ranks(e2e_t, dist, "cuda")
+        e2e = {"value": aggregate_value(V, args.steps, e2e_t, world), "unit": UNIT,
                "h2d_bytes_per_step": h2d / args.steps, "d2h_bytes_per_step": d2h / args.steps,
                "job": "avm_create_host + avm_step(K) + avm_get_state_host, pinned host buffers", "ms": e2e_t}
 

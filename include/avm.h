@@ -111,10 +111,12 @@ int avm_create_host(const avm_params* params, const double* pos_xy, const int32_
  * Conditions arising inside a step set avm_stats.error; they do not stop the run. */
 int avm_step(avm_sim* sim, int64_t n_steps);
 
-/* Same steps as avm_step, but every kernel of the step is bracketed by CUDA events on the stream
- * and the call synchronises after each step: ms_per_kernel (HOST pointer, [AVM_K_COUNT]) receives
- * the summed device time of each kernel class over the n_steps.  Measurement aid for the roofline
- * figures of bench.py; not the timed path. */
+/* Same steps and same schedule as avm_step, but every kernel of the step is bracketed by CUDA
+ * events on the stream and the call synchronises after each step: ms_per_kernel (HOST pointer,
+ * [AVM_K_COUNT]) receives the summed device time of each kernel class over the n_steps.  In the
+ * default two-launch schedule the T1 flips of a step run inside the next force/move launch, so
+ * AVM_K_T1_FLIP only holds the stand-alone T1 kernel that completes the last step.  Measurement
+ * aid for the roofline figures of bench.py; not the timed path. */
 enum { AVM_K_FORCE_MOVE = 0, AVM_K_CELL_UPDATE = 1, AVM_K_T1_FLIP = 2, AVM_K_COUNT = 3 };
 int avm_step_profile(avm_sim* sim, int64_t n_steps, double* ms_per_kernel);
 

@@ -411,17 +411,38 @@ int avm_step_profile(avm_sim* s, int64_t n_steps, double* ms_per_kernel) {
   cudaEvent_t ev[AVM_K_COUNT + 1];
   for (int i = 0; i <= AVM_K_COUNT; ++i) AVM_CUDA(cudaEventCreate(&ev[i]));
   for (int i = 0; i < AVM_K_COUNT; ++i) ms_per_kernel[i] = 0.0;
+  // same schedule as avm_step (fused: the flips of step i ride in the force/move launch of step
+  // i+1, so the third slot only sees the final flush); the events serialise the launches
+  bool pending = false;
   for (int64_t i = 0; i < n_steps; ++i) {
-    s->launches += launch_step(s->dev(), s->k, s->step, s->stream, ev);
+    int n = -1;
+    if (s->fused) {
+      n = launch_step(s->dev(), s->k, s->step, s->stream, ev, true);
+      if (n < 0) s->fused = false; else pending = true;
+    }
+    if (n < 0) n = launch_step(s->dev(), s->k, s->step, s->stream, ev, false);
+    s->launches += n;
     s->cur_pos = 1 - s->cur_pos;
     ++s->step;
     AVM_CUDA(cudaEventSynchronize(ev[AVM_K_COUNT]));
     for (int j = 0; j < AVM_K_COUNT; ++j) {
       float ms = 0.f;
       AVM_CUDA(cudaEventElapsedTime(&ms, ev[j], ev[j + 1]));
-      ms_per_kernel[j] += ms;
+      if (!(pending && j == AVM_K_T1_FLIP)) ms_per_kernel[j] += ms;   // fused: nothing ran in that slot
     }
-    if (s->p.sort_every > 0 && (s->step - s->p.step0) % (unsigned long long)s->p.sort_every == 0) do_sort(s);
+    if (s->p.sort_every > 0 && (s->step - s->p.step0) % (unsigned long long)s->p.sort_every == 0) {
+      if (pending) { s->launches += launch_t1_flush(s->dev(), s->k, s->step - 1, s->stream); pending = false; }
+      do_sort(s);
+    }
+  }
+  if (pending) {
+    AVM_CUDA(cudaEventRecord(ev[0], s->stream));
+    s->launches += launch_t1_flush(s->dev(), s->k, s->step - 1, s->stream);
+    AVM_CUDA(cudaEventRecord(ev[1], s->stream));
+    AVM_CUDA(cudaEventSynchronize(ev[1]));
+    float ms = 0.f;
+    AVM_CUDA(cudaEventElapsedTime(&ms, ev[0], ev[1]));
+    ms_per_kernel[AVM_K_T1_FLIP] += ms;
   }
   for (int i = 0; i <= AVM_K_COUNT; ++i) cudaEventDestroy(ev[i]);
   AVM_CUDA(cudaGetLastError());

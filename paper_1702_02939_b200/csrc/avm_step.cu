@@ -38,7 +38,7 @@ static constexpr unsigned kFull = 0xffffffffu;
 #define AVM_PDL 1          // chain the step's kernels with programmatic dependent launch
 #endif
 #ifndef AVM_CU_MINB
-#define AVM_CU_MINB 9      // cell pass: resident CTAs per SM asked of the compiler (56 registers)
+#define AVM_CU_MINB 8      // cell pass: resident CTAs per SM asked of the compiler (64 registers; measured best of 7..11)
 #endif
 #ifndef AVM_FM_COOP
 #define AVM_FM_COOP 0       // launch the fused force_move as a cooperative grid (not needed: work is claimed, see flipper_work)
@@ -90,7 +90,11 @@ __device__ __forceinline__ unsigned may_wrap(double d, unsigned hi_half) { retur
 __device__ __forceinline__ double2 vertex_force(const double2 h, const double2 q0, const double2 q1,
                                                 const double2 q2, const CellRec& c0, const CellRec& c1,
                                                 const CellRec& c2, const Consts& k) {
-  double r0x = q0.x - h.x, r0y = q0.y - h.y, r1x = q1.x - h.x, r1y = q1.y - h.y, r2x = q2.x - h.x, r2y = q2.y - h.y;
+  // Explicit rounding intrinsics throughout: the function is instantiated in several kernels
+  // (sweep, post-flip move, avm_compute_forces) and must give the same bits in each, so no
+  // contraction is left to the compiler.
+  double r0x = __dsub_rn(q0.x, h.x), r0y = __dsub_rn(q0.y, h.y), r1x = __dsub_rn(q1.x, h.x), r1y = __dsub_rn(q1.y, h.y),
+         r2x = __dsub_rn(q2.x, h.x), r2y = __dsub_rn(q2.y, h.y);
   const unsigned hx = hi_word(k.hLx), hy = hi_word(k.hLy);
   if (may_wrap(r0x, hx) | may_wrap(r1x, hx) | may_wrap(r2x, hx) | may_wrap(r0y, hy) | may_wrap(r1y, hy) | may_wrap(r2y, hy)) {
     r0x = min_image(r0x, k.Lx, k.hLx); r1x = min_image(r1x, k.Lx, k.hLx); r2x = min_image(r2x, k.Lx, k.hLx);
@@ -100,12 +104,18 @@ __device__ __forceinline__ double2 vertex_force(const double2 h, const double2 q
   const double i0 = rsqrt_pos(__fma_rn(r0x, r0x, __fma_rn(r0y, r0y, kTiny)));
   const double i1 = rsqrt_pos(__fma_rn(r1x, r1x, __fma_rn(r1y, r1y, kTiny)));
   const double i2 = rsqrt_pos(__fma_rn(r2x, r2x, __fma_rn(r2y, r2y, kTiny)));
-  const double u0x = r0x * i0, u0y = r0y * i0, u1x = r1x * i1, u1y = r1y * i1, u2x = r2x * i2, u2y = r2y * i2;
+  const double u0x = __dmul_rn(r0x, i0), u0y = __dmul_rn(r0y, i0), u1x = __dmul_rn(r1x, i1), u1y = __dmul_rn(r1y, i1),
+               u2x = __dmul_rn(r2x, i2), u2y = __dmul_rn(r2y, i2);
   // cell k uses (next, prev) = (r_k, r_{k+1})
-  double fx = -0.5 * (c0.a * (r0y - r1y) + c1.a * (r1y - r2y) + c2.a * (r2y - r0y));
-  double fy = -0.5 * (c0.a * (r1x - r0x) + c1.a * (r2x - r1x) + c2.a * (r0x - r2x));
-  fx += c0.p * (u0x + u1x) + c1.p * (u1x + u2x) + c2.p * (u2x + u0x);
-  fy += c0.p * (u0y + u1y) + c1.p * (u1y + u2y) + c2.p * (u2y + u0y);
+  double sx = __dmul_rn(c0.a, __dsub_rn(r0y, r1y));
+  sx = __fma_rn(c1.a, __dsub_rn(r1y, r2y), sx);
+  sx = __fma_rn(c2.a, __dsub_rn(r2y, r0y), sx);
+  double sy = __dmul_rn(c0.a, __dsub_rn(r1x, r0x));
+  sy = __fma_rn(c1.a, __dsub_rn(r2x, r1x), sy);
+  sy = __fma_rn(c2.a, __dsub_rn(r0x, r2x), sy);
+  double fx = __dmul_rn(-0.5, sx), fy = __dmul_rn(-0.5, sy);
+  fx = __fma_rn(c0.p, __dadd_rn(u0x, u1x), fx); fx = __fma_rn(c1.p, __dadd_rn(u1x, u2x), fx); fx = __fma_rn(c2.p, __dadd_rn(u2x, u0x), fx);
+  fy = __fma_rn(c0.p, __dadd_rn(u0y, u1y), fy); fy = __fma_rn(c1.p, __dadd_rn(u1y, u2y), fy); fy = __fma_rn(c2.p, __dadd_rn(u2y, u0y), fy);
   return make_double2(fx, fy);
 }
 
@@ -124,9 +134,9 @@ __device__ __forceinline__ void move_vertex(const Dev& d, const Consts& k, int v
                                             const double2 q1, const double2 q2, const CellRec& c0, const CellRec& c1,
                                             const CellRec& c2) {
   const double2 f = vertex_force(h, q0, q1, q2, c0, c1, c2, k);
-  const double vx = k.mu * f.x + k.v0_3 * (c0.nx + c1.nx + c2.nx);
-  const double vy = k.mu * f.y + k.v0_3 * (c0.ny + c1.ny + c2.ny);
-  double x = h.x + k.dt * vx, y = h.y + k.dt * vy;
+  const double vx = __fma_rn(k.mu, f.x, __dmul_rn(k.v0_3, __dadd_rn(__dadd_rn(c0.nx, c1.nx), c2.nx)));
+  const double vy = __fma_rn(k.mu, f.y, __dmul_rn(k.v0_3, __dadd_rn(__dadd_rn(c0.ny, c1.ny), c2.ny)));
+  double x = __fma_rn(k.dt, vx, h.x), y = __fma_rn(k.dt, vy, h.y);
   // negative, >= L (conservatively) and non-finite values all have a large unsigned high word
   if ((hi_word(x) >= hi_word(k.Lx)) | (hi_word(y) >= hi_word(k.Ly))) {
     x = wrap_box(x, k.Lx); y = wrap_box(y, k.Ly);
@@ -274,15 +284,14 @@ force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts 
   const unsigned gwarp = (unsigned)tid >> 5, nwarps = (unsigned)stride >> 5;
   if (tid == 0) d.ctr->n_cand[parity] = 0;
   if (kFused) {
-    // the first F warps flip, all others sweep (a one-warp grid does both, one after the other)
-    const unsigned F = nwarps > 1 ? min(prev, nwarps / 2u) : 0u;
+    // the first F warps flip, all others sweep (a grid has at least kVertexBlock / 32 = 8 warps)
+    const unsigned F = min(prev, nwarps / 2u);
     if (tid == 0 && prev) atomicAdd((unsigned long long*)&d.ctr->t1_candidates, (unsigned long long)prev);
     if (gwarp < F) {
       flipper_work(d, k, prev, lane);
     } else {
-      if (nwarps == 1 && prev) flipper_work(d, k, prev, lane);
       const int first = (int)(gwarp - F) * 32 + lane, step_v = (int)(nwarps - F) * 32;
-      if (prev && nwarps > 1) sweep<true>(d, k, first, step_v, lane);
+      if (prev) sweep<true>(d, k, first, step_v, lane);
       else sweep<false>(d, k, first, step_v, lane);
     }
   } else {
@@ -351,7 +360,6 @@ __device__ __noinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va,
   // Everything a flip of this edge would write, and everything that reads it in the next
   // force/move pass, belongs to a vertex of these four cells: flag them, so that the fused
   // prologue of force_move can run the flips while the untouched vertices already move.
-#ifndef AVM_EXP_NOMARK
   if (count_stats) {
     const int quad[4] = {cL, cR, cE1, cE2};
     // rows first (independent vector loads), then fire-and-forget reductions
@@ -369,7 +377,6 @@ __device__ __noinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va,
       }
     }
   }
-#endif
 }
 
 // The geometry pass flagged edges of cell c (bit j-1 = the edge ending at row entry j, j = n

@@ -341,3 +341,52 @@ def test_full_size_configs_against_oracle(B, k, steps):
     apg = g.compute_forces()[1].cpu().numpy()
     assert abs(apg[:, 0].sum() - L2) <= 1e-12 * L2
     _TILINGS.pop(k, None)
+
+
+def test_two_launch_schedule_equals_three_launch_schedule(B, monkeypatch):
+    """The default schedule applies the T1 flips of a step inside the next force/move launch
+    (flagged vertices are moved after the flips); the plain schedule runs a third kernel per
+    step.  Both must give the same bits, whatever the chunking of avm_step calls, including the
+    step-0 burst (thousands of candidates: more candidates than flipper warps) and a re-sort."""
+    t = tiling(1)
+    p = dict(w.config_params(1), sort_every=7)
+    keys = ("pos", "theta", "cell_vertices", "vertex_neighbors", "vertex_cell_neighbors", "cell_vertex_num")
+    a = B.from_tiling(t, **p)
+    a.step(40)
+    sa = to_np(a.get_state())
+    b = B.from_tiling(t, **p)
+    for n in (1, 1, 3, 5, 13, 17):
+        b.step(n)
+    sb = to_np(b.get_state())
+    monkeypatch.setenv("AVM_B200_UNFUSED", "1")
+    c = B.from_tiling(t, **p)
+    c.step(40)
+    sc = to_np(c.get_state())
+    monkeypatch.delenv("AVM_B200_UNFUSED")
+    assert sa["stats"]["kernel_launches"] < sc["stats"]["kernel_launches"]
+    for key in keys:
+        assert np.array_equal(sa[key], sb[key]), f"chunking changes {key}: max diff {np.abs(sa[key] - sb[key]).max()}"
+        assert np.array_equal(sa[key], sc[key]), \
+            f"two-launch and three-launch schedules differ in {key}: max diff {np.abs(sa[key] - sc[key]).max()}"
+    for key in ("t1_short", "t1_candidates", "t1_flips", "t1_blocked", "overflow_rejects", "error"):
+        assert sa["stats"][key] == sb["stats"][key] == sc["stats"][key], key
+    assert sa["stats"]["t1_flips"] > 100
+
+
+def test_golden_trace_on_gpu(B):
+    """the stored oracle trace of configs[0] (tests/golden/) reproduced by the CUDA path"""
+    import json
+    import os
+    stored = json.load(open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "cfg0_oracle_trace.json")))
+    t = tiling(0)
+    g = B.from_tiling(t, **w.config_params(0))
+    for r in stored["rows"]:
+        g.step(r["step"] - g.stats()["step"])
+        s = to_np(g.get_state())
+        F, ap = g.compute_forces()
+        ap = ap.cpu().numpy()
+        assert s["stats"]["t1_flips"] == r["t1_flips"] and s["stats"]["t1_candidates"] == r["t1_candidates"]
+        assert np.bincount(s["cell_vertex_num"], minlength=17).tolist() == r["cell_vertex_num_hist"]
+        assert abs(ap[:, 0].sum() - r["sum_area"]) <= 1e-10 and abs(ap[:, 1].sum() - r["sum_perimeter"]) <= 1e-7
+        assert abs(g.energy() - r["energy"]) <= 1e-7 * max(1.0, r["energy"])
+        assert abs(s["theta"].sum() - r["theta_sum"]) <= 1e-8
