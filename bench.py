@@ -84,6 +84,20 @@ class ClockSampler:
                 "samples": len(self.sm)}
 
 
+def ncu_traffic(kernel: str, workload: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed ncu
+    capture (profiles/r1_v3_dram_traffic.csv; the command is in profiles/r1_v3_two_launch.md)."""
+    path = os.path.join(ROOT, "profiles", "r1_v3_dram_traffic.csv")
+    try:
+        import csv
+        for row in csv.DictReader(open(path)):
+            if row["kernel"] == kernel and row["workload"] == workload:
+                return float(row["dram_bytes_read_per_launch"]) + float(row["dram_bytes_write_per_launch"])
+    except Exception:
+        pass
+    return None
+
+
 def max_over_ranks(ms: float, dist, device: str) -> float:
     """Replicas only: ranks share nothing but the clock.  The job's time is the
     slowest rank's device time; this all-reduce of one scalar is the only collective in bench.py
@@ -206,7 +220,9 @@ def main():
     ach = kbytes[dom] / (per_launch_ms[dom] * 1e-3) / 1e9
     step_bytes = sum(kbytes.values())
     roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": None, "peak_source": peak_src,
+                "traffic": ncu_traffic(dom, cfg["name"]), "peak_source": peak_src,
+                "timing": "CUDA events on the library's stream around every launch of a separate pass of "
+                          f"{args.profile_steps} steps (same schedule as the timed region, launches serialised by the events)",
                 "bytes_per_launch": kbytes[dom], "ms_per_launch": per_launch_ms[dom],
                 "kernels_ms_per_launch": per_launch_ms,
                 "step": {"algorithmic_bytes": step_bytes, "achieved_GBps": step_bytes / (ms / args.steps * 1e-3) / 1e9,
