@@ -272,7 +272,10 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   s->cur_pos = 0; s->cur_set = 0;
   s->step = params->step0;
   s->n_sorts = 0; s->launches = 0;
-  s->fused = AVM_FUSED_T1 && !getenv("AVM_B200_UNFUSED");
+  // Two-launch schedule (flips inside the next force/move launch) pays when the sweep is longer
+  // than the flippers' chain of dependent loads (~15 us): from about a million vertices.  Smaller
+  // systems run the plain three-launch schedule.  AVM_B200_FUSED / AVM_B200_UNFUSED override.
+  s->fused = AVM_FUSED_T1 && (V >= (1 << 20) || getenv("AVM_B200_FUSED")) && !getenv("AVM_B200_UNFUSED");
 
   cudaStream_t st = s->stream;
   const cudaMemcpyKind kind = host_inputs ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;

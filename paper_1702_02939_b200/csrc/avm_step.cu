@@ -219,7 +219,7 @@ __device__ __forceinline__ void sweep(const Dev& d, const Consts& k, const int f
 //   3. claim candidates again: move the flagged vertices of the candidate's four cells with
 //      loads that bypass L1 (whoever clears a vertex's bit moves it) and release the cells'
 //      minimum keys (row a6).
-__device__ __noinline__ void flipper_work(const Dev& d, const Consts& k, const unsigned prev, const int lane) {
+__device__ __noinline__ void flipper_flips(const Dev& d, const Consts& k, const unsigned prev, const int lane) {
   unsigned mine = 0, flips = 0;
   for (;;) {
     unsigned i = 0;
@@ -239,8 +239,14 @@ __device__ __noinline__ void flipper_work(const Dev& d, const Consts& k, const u
       atomicAdd(&d.ctr->flip_done, mine);
     }
   }
+}
+
+__device__ __noinline__ void flipper_moves(const Dev& d, const Consts& k, const unsigned prev, const int lane) {
   while (ld_volatile(&d.ctr->flip_done) < prev) __nanosleep(64);
   __threadfence();
+  // rows of up to 16 entries: two rows per pass (half a warp each), else one row per pass
+  const bool two = k.S <= 16;
+  const int half = two ? lane >> 4 : 0, j = two ? lane & 15 : lane;
   for (;;) {
     unsigned i = 0;
     if (lane == 0) i = atomicAdd(&d.ctr->next_quad, 1u);
@@ -249,10 +255,12 @@ __device__ __noinline__ void flipper_work(const Dev& d, const Consts& k, const u
     const Cand c = d.cand[i];
     const int quad[4] = {c.cL, c.cR, c.cE1, c.cE2};
 #pragma unroll 1
-    for (int t = 0; t < 4; ++t) {
-      const int n = __ldcg(d.cvn + quad[t]);
-      if (lane < n) {
-        const int u = __ldcg(reinterpret_cast<const int*>(d.cv + (size_t)(lane >> 2) * k.N + quad[t]) + (lane & 3));
+    for (int t0 = 0; t0 < 4; t0 += (two ? 2 : 1)) {
+      const int cell = quad[t0 + half];
+      // the entry is loaded whatever the row length is (padding repeats entry 0): no dependent load
+      const int n = __ldcg(d.cvn + cell);
+      const int u = __ldcg(reinterpret_cast<const int*>(d.cv + (size_t)(j >> 2) * k.N + cell) + (j & 3));
+      if (j < n) {
         const unsigned bit = 1u << (u & 31);
         if (atomicAnd(&d.dirty[u >> 5], ~bit) & bit) move_vertex_coherent(d, k, u);
       }
@@ -264,14 +272,12 @@ __device__ __noinline__ void flipper_work(const Dev& d, const Consts& k, const u
 // Persistent grid-stride kernel: each thread keeps the streaming loads of its NEXT vertex in
 // flight while it gathers and computes the current one.
 //
-// kFused (cooperative launch: every CTA is resident) also carries rows a6 + a7 of the PREVIOUS
-// step: warp i of the grid decides and flips candidate i of the previous step's list first
-// (t1_try_flip), while all other warps start moving vertices at once.  A vertex whose inputs a
-// flip may rewrite has its bit set in d.dirty (the marking thread flagged every vertex of the
-// candidate's four cells); such vertices are skipped in the main sweep and moved in a short
-// second sweep, after the grid-wide counter flip_done shows that every candidate has been
-// decided, with loads that bypass L1.  The latency-bound flips thus overlap the bandwidth-bound
-// sweep and the step needs no third launch.
+// kFused also carries rows a6 + a7 of the PREVIOUS step (flipper_flips / flipper_moves above):
+// a few warps decide and flip that step's candidates while all other warps already move
+// vertices.  A vertex whose inputs a flip may rewrite has its bit set in d.dirty (the marking
+// thread flagged every vertex of the candidate's four cells); the sweep skips it and a flipper
+// moves it once every candidate has been decided.  The latency-bound flips thus overlap the
+// gather-bound sweep and the step needs no third launch.
 template <bool kFused>
 __global__ void __launch_bounds__(kVertexBlock, AVM_FM_MINB)
 force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, const unsigned parity) {
@@ -284,15 +290,24 @@ force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts 
   const unsigned gwarp = (unsigned)tid >> 5, nwarps = (unsigned)stride >> 5;
   if (tid == 0) d.ctr->n_cand[parity] = 0;
   if (kFused) {
-    // the first F warps flip, all others sweep (a grid has at least kVertexBlock / 32 = 8 warps)
-    const unsigned F = min(prev, nwarps / 2u);
     if (tid == 0 && prev) atomicAdd((unsigned long long*)&d.ctr->t1_candidates, (unsigned long long)prev);
-    if (gwarp < F) {
-      flipper_work(d, k, prev, lane);
+    if (2u * prev <= nwarps) {
+      // few candidates: the first `prev` warps only flip (they would start the sweep late and
+      // finish it last), all others only sweep
+      if (gwarp < prev) {
+        flipper_flips(d, k, prev, lane);
+        flipper_moves(d, k, prev, lane);
+      } else {
+        const int first = (int)(gwarp - prev) * 32 + lane, step_v = (int)(nwarps - prev) * 32;
+        if (prev) sweep<true>(d, k, first, step_v, lane);
+        else sweep<false>(d, k, first, step_v, lane);
+      }
     } else {
-      const int first = (int)(gwarp - F) * 32 + lane, step_v = (int)(nwarps - F) * 32;
-      if (prev) sweep<true>(d, k, first, step_v, lane);
-      else sweep<false>(d, k, first, step_v, lane);
+      // many candidates (the burst after a random start, T1-heavy regimes): every warp flips,
+      // then sweeps its share, then moves flagged vertices
+      flipper_flips(d, k, prev, lane);
+      sweep<true>(d, k, tid, stride, lane);
+      flipper_moves(d, k, prev, lane);
     }
   } else {
     // the previous step's T1 candidates are done: clear their cells' minimum keys (row a6)

@@ -351,6 +351,7 @@ def test_two_launch_schedule_equals_three_launch_schedule(B, monkeypatch):
     t = tiling(1)
     p = dict(w.config_params(1), sort_every=7)
     keys = ("pos", "theta", "cell_vertices", "vertex_neighbors", "vertex_cell_neighbors", "cell_vertex_num")
+    monkeypatch.setenv("AVM_B200_FUSED", "1")      # small systems default to the three-launch schedule
     a = B.from_tiling(t, **p)
     a.step(40)
     sa = to_np(a.get_state())
@@ -358,6 +359,7 @@ def test_two_launch_schedule_equals_three_launch_schedule(B, monkeypatch):
     for n in (1, 1, 3, 5, 13, 17):
         b.step(n)
     sb = to_np(b.get_state())
+    monkeypatch.delenv("AVM_B200_FUSED")
     monkeypatch.setenv("AVM_B200_UNFUSED", "1")
     c = B.from_tiling(t, **p)
     c.step(40)
