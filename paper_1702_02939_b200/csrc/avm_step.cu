@@ -324,27 +324,43 @@ force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts 
 // run by the thread that found it.  (va, vb) are current vertex indices.  Cold path.
 // ---------------------------------------------------------------------------------------------
 __device__ __noinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va, int vb, unsigned parity, bool count_stats) {
-  // canonical test (R9): strict l < l_c on the minimum-image separation of the two endpoints
+  // The marking thread delays the end of the cell pass when it sits in the last wave, so its
+  // loads are issued in two batches of independent loads instead of a chain of five.
+  // ---- batch 1: everything known from (va, vb) ----
   const double2 ha = d.pos[va], hb = d.pos[vb];
+  const unsigned int ta = (unsigned int)d.vtag[va], tb = (unsigned int)d.vtag[vb];
+  int na[3], nb[3], ca[3], cb[3];
+#pragma unroll
+  for (int s = 0; s < 3; ++s) {
+    na[s] = d.vn[s * k.Vs + va]; nb[s] = d.vn[s * k.Vs + vb];
+    ca[s] = d.vc[s * k.Vs + va]; cb[s] = d.vc[s * k.Vs + vb];
+  }
+  // canonical test (R9): strict l < l_c on the minimum-image separation of the two endpoints
   const double dx = min_image(hb.x - ha.x, k.Lx, k.hLx), dy = min_image(hb.y - ha.y, k.Ly, k.hLy);
   if (!(dx * dx + dy * dy < k.lc2)) return;
   if (count_stats) atomicAdd((unsigned long long*)&d.ctr->t1_short, 1ull);
-  int v1 = va, v2 = vb;
-  unsigned int t1 = (unsigned int)d.vtag[v1], t2 = (unsigned int)d.vtag[v2];
-  if (t1 > t2) { int tv = v1; v1 = v2; v2 = tv; unsigned int tt = t1; t1 = t2; t2 = tt; }
-  int k1 = 0, k2 = 0, nb1[3], nb2[3];
+  const bool sw = ta > tb;                    // v1 = endpoint with the smaller tag
+  const int v1 = sw ? vb : va, v2 = sw ? va : vb;
+  const unsigned int t1 = sw ? tb : ta, t2 = sw ? ta : tb;
+  int nb1[3], nb2[3], vc1[3], vc2[3];
 #pragma unroll
-  for (int s = 0; s < 3; ++s) {
-    nb1[s] = d.vn[s * k.Vs + v1]; nb2[s] = d.vn[s * k.Vs + v2];
-    if (nb1[s] == v2) k1 = s;
-    if (nb2[s] == v1) k2 = s;
-  }
+  for (int s = 0; s < 3; ++s) { nb1[s] = sw ? nb[s] : na[s]; nb2[s] = sw ? na[s] : nb[s]; vc1[s] = sw ? cb[s] : ca[s]; vc2[s] = sw ? ca[s] : cb[s]; }
+  const int k1 = nb1[0] == v2 ? 0 : nb1[1] == v2 ? 1 : 2, k2 = nb2[0] == v1 ? 0 : nb2[1] == v1 ? 1 : 2;
   // cyclic from the partner's slot the cells of u are (C0, C1, C2); C0 is left of u -> partner
-  const int cL = d.vc[k1 * k.Vs + v1], cE1 = d.vc[((k1 + 1) % 3) * k.Vs + v1];
-  const int cR = d.vc[k2 * k.Vs + v2], cE2 = d.vc[((k2 + 1) % 3) * k.Vs + v2];
+  const int cL = k1 == 0 ? vc1[0] : k1 == 1 ? vc1[1] : vc1[2], cE1 = k1 == 0 ? vc1[1] : k1 == 1 ? vc1[2] : vc1[0];
+  const int cR = k2 == 0 ? vc2[0] : k2 == 1 ? vc2[1] : vc2[2], cE2 = k2 == 0 ? vc2[1] : k2 == 1 ? vc2[2] : vc2[0];
   const bool distinct = cL != cR && cL != cE1 && cL != cE2 && cR != cE1 && cR != cE2 && cE1 != cE2;
   if (!distinct) return;
-  const int nq[4] = {d.cvn[cL], d.cvn[cR], d.cvn[cE1], d.cvn[cE2]};
+  // the flip's outer vertices, decoded here so that the flip needs no dependent loads
+  const int x1 = k1 == 0 ? nb1[1] : k1 == 1 ? nb1[2] : nb1[0], y1 = k1 == 0 ? nb1[2] : k1 == 1 ? nb1[0] : nb1[1];
+  const int x2 = k2 == 0 ? nb2[1] : k2 == 1 ? nb2[2] : nb2[0], y2 = k2 == 0 ? nb2[2] : k2 == 1 ? nb2[0] : nb2[1];
+  // ---- batch 2: everything known from the four cells and the outer vertices ----
+  const int quad[4] = {cL, cR, cE1, cE2};
+  int nq[4];
+  int4 q[4][2];
+#pragma unroll
+  for (int t = 0; t < 4; ++t) { nq[t] = d.cvn[quad[t]]; q[t][0] = d.cv[quad[t]]; q[t][1] = d.cv[(size_t)k.N + quad[t]]; }
+  const int x1s1 = d.vn[k.Vs + x1], x1s2 = d.vn[2 * k.Vs + x1], x2s1 = d.vn[k.Vs + x2], x2s2 = d.vn[2 * k.Vs + x2];
   if (!(nq[0] > 3 && nq[1] > 3)) return;                       // no 2-gons (T2 absent)
   if (!(nq[2] < k.S && nq[3] < k.S)) {                         // row would exceed the stride
     if (count_stats) {
@@ -357,15 +373,9 @@ __device__ __noinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va,
   cd.v1 = v1; cd.v2 = v2; cd.k1 = k1; cd.k2 = k2;
   cd.cL = cL; cd.cR = cR; cd.cE1 = cE1; cd.cE2 = cE2;
   cd.key = ((unsigned long long)t1 << 32) | t2;
-  // the flip's outer vertices, decoded here so that the flip kernel needs no dependent loads
-  cd.x1 = k1 == 0 ? nb1[1] : k1 == 1 ? nb1[2] : nb1[0]; cd.y1 = k1 == 0 ? nb1[2] : k1 == 1 ? nb1[0] : nb1[1];
-  cd.x2 = k2 == 0 ? nb2[1] : k2 == 1 ? nb2[2] : nb2[0]; cd.y2 = k2 == 0 ? nb2[2] : k2 == 1 ? nb2[0] : nb2[1];
-  cd.sx1 = 0; cd.sx2 = 0;
-#pragma unroll
-  for (int s = 1; s < 3; ++s) {
-    if (d.vn[s * k.Vs + cd.x1] == v1) cd.sx1 = s;
-    if (d.vn[s * k.Vs + cd.x2] == v2) cd.sx2 = s;
-  }
+  cd.x1 = x1; cd.y1 = y1; cd.x2 = x2; cd.y2 = y2;
+  cd.sx1 = x1s1 == v1 ? 1 : x1s2 == v1 ? 2 : 0;
+  cd.sx2 = x2s1 == v2 ? 1 : x2s2 == v2 ? 2 : 0;
   const unsigned int slot = atomicAdd(&d.ctr->n_cand[parity], 1u);
   d.cand[slot] = cd;
   atomicMin(&d.minkey[cL], cd.key);
@@ -373,14 +383,9 @@ __device__ __noinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va,
   atomicMin(&d.minkey[cE1], cd.key);
   atomicMin(&d.minkey[cE2], cd.key);
   // Everything a flip of this edge would write, and everything that reads it in the next
-  // force/move pass, belongs to a vertex of these four cells: flag them, so that the fused
-  // prologue of force_move can run the flips while the untouched vertices already move.
+  // force/move pass, belongs to a vertex of these four cells: flag them, so that force_move can
+  // run the flips while the untouched vertices already move.
   if (count_stats) {
-    const int quad[4] = {cL, cR, cE1, cE2};
-    // rows first (independent vector loads), then fire-and-forget reductions
-    int4 q[4][2];
-#pragma unroll
-    for (int t = 0; t < 4; ++t) { q[t][0] = d.cv[quad[t]]; q[t][1] = d.cv[(size_t)k.N + quad[t]]; }
 #pragma unroll
     for (int t = 0; t < 4; ++t) {
       const int e[8] = {q[t][0].x, q[t][0].y, q[t][0].z, q[t][0].w, q[t][1].x, q[t][1].y, q[t][1].z, q[t][1].w};
