@@ -77,6 +77,22 @@ class ClockSampler:
         except Exception:
             pass
 
+    def start(self, period_s: float = 0.004):
+        """sample from a background thread while the caller enqueues and waits (ctypes releases the GIL)"""
+        import threading
+        self._stop = threading.Event()
+
+        def loop():
+            while not self._stop.is_set():
+                self.sample()
+                self._stop.wait(period_s)
+        self._thread = threading.Thread(target=loop, daemon=True)
+        self._thread.start()
+
+    def stop(self):
+        self._stop.set()
+        self._thread.join()
+
     def summary(self):
         if not self.sm:
             return {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": sorted(self.reasons), "samples": 0}
@@ -86,8 +102,8 @@ class ClockSampler:
 
 def ncu_traffic(kernel: str, workload: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed ncu
-    capture (profiles/r1_v3_dram_traffic.csv; the command is in profiles/r1_v3_two_launch.md)."""
-    path = os.path.join(ROOT, "profiles", "r1_v3_dram_traffic.csv")
+    capture (profiles/r1_v4_dram_traffic.csv; the command is in profiles/r1_v4_two_launch.md)."""
+    path = os.path.join(ROOT, "profiles", "r1_v4_dram_traffic.csv")
     try:
         import csv
         for row in csv.DictReader(open(path)):
@@ -199,12 +215,12 @@ def main():
     sampler = ClockSampler(local_rank)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
+    sampler.start()
     e0.record()
     sim.step(args.steps)
     e1.record()
-    while not e1.query():
-        sampler.sample()
-        time.sleep(0.002)
+    e1.synchronize()
+    sampler.stop()
     barrier()
     ms = e0.elapsed_time(e1)
     st1 = sim.stats()
