@@ -86,25 +86,86 @@ radix_hist_kernel(const unsigned int* __restrict__ key, int n, int shift, int n_
     for (int i = lane; i < 256; i += 32) hist[(size_t)i * n_seg + seg] = cnt[warp][i];
 }
 
-// exclusive scan of `len` counters by one block (len is at most a few million; off the hot path)
-__global__ void __launch_bounds__(1024)
-exclusive_scan_kernel(unsigned int* __restrict__ a, long long len) {
-  __shared__ unsigned int part[1024];
-  const long long chunk = (len + 1023) / 1024;
-  const long long beg = (long long)threadIdx.x * chunk, end = min(len, beg + chunk);
-  unsigned int s = 0;
-  for (long long i = beg; i < end; ++i) s += a[i];
-  part[threadIdx.x] = s;
+// ---- exclusive scan of the digit counters (digit-major, `len` = 256 * segments), three coalesced
+// kernels: per-chunk sums, scan of the chunk sums by one block, per-chunk scan with its offset ----
+static constexpr int kScanBlock = 1024;
+static constexpr int kScanChunk = 4 * kScanBlock;   // four consecutive counters per thread
+
+__device__ __forceinline__ unsigned int block_exclusive_scan(unsigned int x, unsigned int* warp_sums, unsigned int& total) {
+  // exclusive scan of one value per thread over a block of kScanBlock threads
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  unsigned int incl = x;
+#pragma unroll
+  for (int off = 1; off < 32; off <<= 1) {
+    const unsigned int y = __shfl_up_sync(0xffffffffu, incl, off);
+    if (lane >= off) incl += y;
+  }
+  if (lane == 31) warp_sums[warp] = incl;
   __syncthreads();
-  // Hillis-Steele inclusive scan of the 1024 partial sums
-  for (int off = 1; off < 1024; off <<= 1) {
-    unsigned int v = threadIdx.x >= off ? part[threadIdx.x - off] : 0u;
-    __syncthreads();
-    part[threadIdx.x] += v;
+  if (warp == 0) {
+    unsigned int w = warp_sums[lane], wi = w;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+      const unsigned int y = __shfl_up_sync(0xffffffffu, wi, off);
+      if (lane >= off) wi += y;
+    }
+    warp_sums[lane] = wi - w;          // exclusive prefix of the warp sums
+    if (lane == 31) warp_sums[32] = wi;
+  }
+  __syncthreads();
+  total = warp_sums[32];
+  return warp_sums[warp] + incl - x;
+}
+
+__global__ void __launch_bounds__(kScanBlock)
+scan_chunk_sums_kernel(const unsigned int* __restrict__ a, long long len, unsigned int* __restrict__ sums) {
+  __shared__ unsigned int ws[33];
+  const long long i = (long long)blockIdx.x * kScanChunk + 4 * threadIdx.x;
+  unsigned int s = 0;
+  if (i + 3 < len) { const uint4 v = *reinterpret_cast<const uint4*>(a + i); s = v.x + v.y + v.z + v.w; }
+  else for (int j = 0; j < 4; ++j) if (i + j < len) s += a[i + j];
+  unsigned int total;
+  block_exclusive_scan(s, ws, total);
+  if (threadIdx.x == 0) sums[blockIdx.x] = total;
+}
+
+__global__ void __launch_bounds__(kScanBlock)
+scan_top_kernel(unsigned int* __restrict__ sums, int n) {
+  __shared__ unsigned int ws[33];
+  unsigned int run = 0;
+  for (int base = 0; base < n; base += kScanBlock) {
+    const int i = base + threadIdx.x;
+    const unsigned int x = i < n ? sums[i] : 0u;
+    unsigned int total;
+    const unsigned int ex = block_exclusive_scan(x, ws, total);
+    if (i < n) sums[i] = run + ex;
+    run += total;
     __syncthreads();
   }
-  unsigned int run = threadIdx.x ? part[threadIdx.x - 1] : 0u;
-  for (long long i = beg; i < end; ++i) { const unsigned int t = a[i]; a[i] = run; run += t; }
+}
+
+__global__ void __launch_bounds__(kScanBlock)
+scan_apply_kernel(unsigned int* __restrict__ a, long long len, const unsigned int* __restrict__ sums) {
+  __shared__ unsigned int ws[33];
+  const long long i = (long long)blockIdx.x * kScanChunk + 4 * threadIdx.x;
+  uint4 v = make_uint4(0, 0, 0, 0);
+  const bool full = i + 3 < len;
+  if (full) v = *reinterpret_cast<const uint4*>(a + i);
+  else { if (i < len) v.x = a[i]; if (i + 1 < len) v.y = a[i + 1]; if (i + 2 < len) v.z = a[i + 2]; }
+  unsigned int total;
+  const unsigned int ex = sums[blockIdx.x] + block_exclusive_scan(v.x + v.y + v.z + v.w, ws, total);
+  const uint4 o = make_uint4(ex, ex + v.x, ex + v.x + v.y, ex + v.x + v.y + v.z);
+  if (full) *reinterpret_cast<uint4*>(a + i) = o;
+  else { if (i < len) a[i] = o.x; if (i + 1 < len) a[i + 1] = o.y; if (i + 2 < len) a[i + 2] = o.z; }
+}
+
+static int launch_exclusive_scan(unsigned int* a, long long len, cudaStream_t s) {
+  const int nb = (int)((len + kScanChunk - 1) / kScanChunk);
+  unsigned int* sums = a + ((len + 3) & ~3ll);      // chunk sums live behind the counters (sort_hist_entries)
+  scan_chunk_sums_kernel<<<nb, kScanBlock, 0, s>>>(a, len, sums);
+  scan_top_kernel<<<1, kScanBlock, 0, s>>>(sums, nb);
+  scan_apply_kernel<<<nb, kScanBlock, 0, s>>>(a, len, sums);
+  return 3;
 }
 
 __global__ void __launch_bounds__(32 * kWarpsPerBlock)
@@ -176,7 +237,10 @@ __global__ void permute_cells_kernel(const Dev a, const Dev b, const Consts k, c
   }
 }
 
-size_t sort_hist_entries(int n) { return (size_t)256 * (size_t)((n + kSeg - 1) / kSeg); }
+size_t sort_hist_entries(int n) {
+  const size_t len = (size_t)256 * (size_t)((n + kSeg - 1) / kSeg);
+  return ((len + 3) & ~(size_t)3) + (len + kScanChunk - 1) / kScanChunk + 4;   // counters + their chunk sums
+}
 
 static inline int cdiv(long long a, int b) { return (int)((a + b - 1) / b); }
 
@@ -186,7 +250,7 @@ static int radix_sort_pairs(const SortScratch& sc, int n, int key_bits, cudaStre
   int cur = 0;
   for (int shift = 0; shift < key_bits; shift += 8) {
     radix_hist_kernel<<<cdiv(n_seg, kWarpsPerBlock), 32 * kWarpsPerBlock, 0, s>>>(sc.key[cur], n, shift, n_seg, sc.hist);
-    exclusive_scan_kernel<<<1, 1024, 0, s>>>(sc.hist, (long long)256 * n_seg);
+    *launches += launch_exclusive_scan(sc.hist, (long long)256 * n_seg, s) - 1;
     radix_scatter_kernel<<<cdiv(n_seg, kWarpsPerBlock), 32 * kWarpsPerBlock, 0, s>>>(
         sc.key[cur], sc.val[cur], n, shift, n_seg, sc.hist, sc.key[1 - cur], sc.val[1 - cur]);
     cur = 1 - cur;
