@@ -22,7 +22,7 @@ _lib: Optional[ctypes.CDLL] = None
 
 class OracleParams(ctypes.Structure):
     _fields_ = [("n_cells", ctypes.c_int32), ("n_vertices", ctypes.c_int32),
-                ("max_cell_vertices", ctypes.c_int32), ("reserved", ctypes.c_int32),
+                ("max_cell_vertices", ctypes.c_int32), ("t1_max_passes", ctypes.c_int32),
                 ("Lx", ctypes.c_double), ("Ly", ctypes.c_double),
                 ("KA", ctypes.c_double), ("KP", ctypes.c_double), ("A0", ctypes.c_double), ("P0", ctypes.c_double),
                 ("v0", ctypes.c_double), ("Dr", ctypes.c_double), ("mu", ctypes.c_double),
@@ -107,7 +107,7 @@ class OracleSim:
 
     def __init__(self, pos, cell_vertex_num, cell_vertices, vertex_neighbors, vertex_cell_neighbors, theta, *,
                  Lx, Ly, KA=1.0, KP=1.0, A0=1.0, P0=3.8, v0=0.0, Dr=0.0, mu=1.0, dt=0.01, l_c=0.0,
-                 seed=0, step0=0, **_ignored):
+                 seed=0, step0=0, t1_max_passes=1, **_ignored):
         lib = _load()
         pos = np.ascontiguousarray(pos, dtype=np.float64)
         cvn = np.ascontiguousarray(cell_vertex_num, dtype=np.int32)
@@ -117,7 +117,7 @@ class OracleSim:
         th = np.ascontiguousarray(theta, dtype=np.float64)
         self.N, self.S = cv.shape
         self.V = pos.shape[0]
-        self.params = OracleParams(self.N, self.V, self.S, 0, Lx, Ly, KA, KP, A0, P0, v0, Dr, mu, dt, l_c, seed, step0)
+        self.params = OracleParams(self.N, self.V, self.S, int(t1_max_passes), Lx, Ly, KA, KP, A0, P0, v0, Dr, mu, dt, l_c, seed, step0)
         self._h = lib.oracle_create(ctypes.byref(self.params), _ptr(pos), _ptr(cvn), _ptr(cv), _ptr(vn), _ptr(vc), _ptr(th))
         if not self._h:
             raise ValueError("oracle_create rejected the input")

@@ -29,7 +29,9 @@
 namespace {
 
 struct Params {
-  int32_t n_cells, n_vertices, max_cell_vertices, reserved;
+  int32_t n_cells, n_vertices, max_cell_vertices;
+  int32_t t1_max_passes;   // NEXT-1: T1 passes per step; <= 1 = one pass (north_star), P > 1 = repeat until a
+                           // pass finds no candidate, at most P passes
   double Lx, Ly;
   double KA, KP, A0, P0;      // Eq. A1: uniform moduli and preferred values (R17)
   double v0, Dr, mu, dt, l_c;
@@ -291,7 +293,8 @@ void t1_flip(Sim& s, const Cand& c) {
   row_insert_after(s, E2, v2, v1);
 }
 
-void t1_pass(Sim& s) {
+// returns the number of candidates of the pass (0 = the topology is at a fixed point of the rule)
+size_t t1_pass(Sim& s) {
   std::vector<Cand> cands;
   std::vector<char> win;
   t1_candidates(s, cands, true);
@@ -301,6 +304,7 @@ void t1_pass(Sim& s) {
     if (win[i]) { t1_flip(s, cands[i]); ++s.st.t1_flips; }
     else ++s.st.t1_blocked;
   }
+  return cands.size();
 }
 
 // ------------------------------------------------------------------------------------------
@@ -328,7 +332,11 @@ void step(Sim& s) {
   const double amp = std::sqrt(2.0 * s.p.Dr * s.p.dt);               // 4: Euler-Maruyama (R8)
   for (int64_t c = 0; c < s.N; ++c)
     s.theta[c] += amp * director_noise(s.p.seed, (uint64_t)s.st.step, (uint64_t)c);
-  t1_pass(s);                                                        // 5
+  // 5: one pass (north_star), or the paper's rule ("called repeatedly until no
+  // changes"): repeat until a pass finds no candidate, at most t1_max_passes passes
+  const int passes = s.p.t1_max_passes > 1 ? s.p.t1_max_passes : 1;
+  for (int pass = 0; pass < passes; ++pass)
+    if (t1_pass(s) == 0) break;
   ++s.st.step;                                                       // 6
 }
 

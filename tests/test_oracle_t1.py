@@ -261,3 +261,73 @@ def test_many_flips_keep_invariants_larger_system():
     ap = sim.geometry()
     assert abs(ap[:, 0].sum() - t.Lx * t.Ly) <= 1e-12 * t.Lx * t.Ly
     assert s["stats"]["t1_flips"] > 100
+
+
+# ---- NEXT-1: the paper's own rule, T1 passes repeated until no candidate remains ----
+
+def test_repeated_passes_resolve_a_conflict_chain_within_one_step():
+    """The chain e1 < e2 < e3 of test_conflict_chain...: one pass flips e1 only; with repeated
+    passes the blocked candidates flip in later passes of the SAME step, unless an earlier flip
+    has already lengthened them, and the step ends at a fixed point of the rule."""
+    l_c = 0.04
+    t = w.hex_tiling(8, 6, a=1.0)
+    row = t.cell_vertices[20, :6]
+    pos = t.pos.copy()
+    edges = [(int(row[0]), int(row[1])), (int(row[2]), int(row[3])), (int(row[4]), int(row[5]))]
+    tt = t.copy()
+    for a, b in edges:
+        tt.pos = pos
+        pos, _, _ = shrink_edge(tt, min(a, b), max(a, b), 0.5 * l_c)
+    # K_A = K_P = v0 = 0: the step moves nothing, it only runs the T1 stage
+    kw = dict(l_c=l_c, KA=0.0, KP=0.0, v0=0.0, Dr=0.0, dt=0.01)
+    one = oracle.from_tiling(t, **kw)
+    one.set_positions(pos)
+    one.step(1)
+    many = oracle.from_tiling(t, t1_max_passes=8, **kw)
+    many.set_positions(pos)
+    many.step(1)
+    s1, sm = one.get_state()["stats"], many.get_state()["stats"]
+    assert s1["t1_flips"] == 1 and s1["t1_blocked"] == 2
+    assert sm["t1_flips"] >= 2 and sm["t1_flips"] > s1["t1_flips"]
+    cand, _ = many.debug_t1()
+    assert len(cand) == 0, "repeat-until-none must end at a fixed point of the rule"
+    cand1, _ = one.debug_t1()
+    assert len(cand1) > 0, "the single pass leaves the blocked candidates short"
+    s = many.get_state()
+    h.check_topology(s["cell_vertex_num"], s["cell_vertices"], s["vertex_neighbors"], s["vertex_cell_neighbors"])
+
+
+def test_repeated_passes_on_a_voronoi_start():
+    """configs[0] and configs[1]: with enough passes no candidate survives any step, every
+    invariant of the single-pass rule still holds, and the first pass of every step is the
+    single-pass rule itself (same candidates, same winners from the same state)."""
+    for k, steps in ((0, 30), (1, 8)):
+        t = w.config_tiling(k)
+        p = w.config_params(k)
+        sim = oracle.from_tiling(t, t1_max_passes=50, **p)
+        ref = oracle.from_tiling(t, **p)
+        # step 0 from the identical state: the repeated rule flips at least the single-pass winners
+        sim.step(1)
+        ref.step(1)
+        assert sim.get_state()["stats"]["t1_flips"] >= ref.get_state()["stats"]["t1_flips"] > 0
+        for _ in range(steps):
+            sim.step(1)
+            s = sim.get_state()
+            cand, _ = sim.debug_t1()
+            assert len(cand) == 0
+            h.check_topology(s["cell_vertex_num"], s["cell_vertices"], s["vertex_neighbors"], s["vertex_cell_neighbors"])
+            ap = sim.geometry()
+            assert abs(ap[:, 0].sum() - t.Lx * t.Ly) <= 1e-12 * t.Lx * t.Ly
+        st = sim.get_state()["stats"]
+        assert st["t1_candidates"] == st["t1_flips"] + st["t1_blocked"] and st["error"] == 0
+
+
+def test_one_pass_is_the_default_and_equals_max_passes_one():
+    t = w.config_tiling(0)
+    p = w.config_params(0)
+    a = oracle.from_tiling(t, **p)
+    b = oracle.from_tiling(t, t1_max_passes=1, **p)
+    a.step(40)
+    b.step(40)
+    sa, sb = a.get_state(), b.get_state()
+    assert np.array_equal(sa["pos"], sb["pos"]) and np.array_equal(sa["cell_vertices"], sb["cell_vertices"])
