@@ -63,7 +63,14 @@ typedef struct avm_params {
 
 enum {
   AVM_FLAG_SORT_AT_CREATE = 1, /* Hilbert-order cells and vertices once inside avm_create       */
-  AVM_FLAG_NO_GRAPH = 2        /* launch kernels directly instead of through CUDA graphs        */
+  AVM_FLAG_NO_GRAPH = 2,       /* reserved, no effect (kernels are always launched directly)    */
+  /* bits 8..15: maximum number of T1 passes per step.  0 or 1 = one pass per step (the rule of
+   * BASELINE.json's north_star, the default and the timed path).  P > 1 = the paper's own rule
+   * (the T1 kernel is "called repeatedly until no changes"): after the first pass
+   * the detect / resolve / flip passes are repeated on the current state until a pass finds no
+   * candidate, at most P passes in total. */
+  AVM_FLAG_T1_PASSES_SHIFT = 8,
+  AVM_FLAG_T1_PASSES_MASK = 0xff00
 };
 
 /* Counters since creation.  error is a sticky bit set: 1 = a non-finite position was produced,

@@ -98,6 +98,7 @@ struct avm_sim {
   Cand* cand;
   Counters* ctr;
   unsigned int* dirty;
+  int t1_passes;         // T1 passes per step (1 = north_star's rule; > 1 = repeat until none, NEXT-1)
   bool fused;            // T1 flips ride in force_move's prologue (cooperative launch available)
   double2* ap;
   double* epart;
@@ -275,7 +276,9 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   // Two-launch schedule (flips inside the next force/move launch) pays when the sweep is longer
   // than the flippers' chain of dependent loads (~15 us): from about a million vertices.  Smaller
   // systems run the plain three-launch schedule.  AVM_B200_FUSED / AVM_B200_UNFUSED override.
-  s->fused = AVM_FUSED_T1 && (V >= (1 << 20) || getenv("AVM_B200_FUSED")) && !getenv("AVM_B200_UNFUSED");
+  s->t1_passes = (params->flags & AVM_FLAG_T1_PASSES_MASK) >> AVM_FLAG_T1_PASSES_SHIFT;
+  if (s->t1_passes < 1) s->t1_passes = 1;
+  s->fused = s->t1_passes == 1 && AVM_FUSED_T1 && (V >= (1 << 20) || getenv("AVM_B200_FUSED")) && !getenv("AVM_B200_UNFUSED");
 
   cudaStream_t st = s->stream;
   const cudaMemcpyKind kind = host_inputs ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
@@ -398,6 +401,8 @@ int avm_step(avm_sim* s, int64_t n_steps) {
     if (n < 0) n = launch_step(s->dev(), s->k, s->step, s->stream, nullptr, false);
     s->launches += n;
     s->cur_pos = 1 - s->cur_pos;
+    for (int pass = 1; pass < s->t1_passes; ++pass)
+      s->launches += launch_t1_extra_pass(s->dev(), s->k, (unsigned)(s->step & 1ull), s->stream);
     ++s->step;
     if (s->p.sort_every > 0 && (s->step - s->p.step0) % (unsigned long long)s->p.sort_every == 0) {
       if (pending) { s->launches += launch_t1_flush(s->dev(), s->k, s->step - 1, s->stream); pending = false; }
@@ -426,6 +431,8 @@ int avm_step_profile(avm_sim* s, int64_t n_steps, double* ms_per_kernel) {
     if (n < 0) n = launch_step(s->dev(), s->k, s->step, s->stream, ev, false);
     s->launches += n;
     s->cur_pos = 1 - s->cur_pos;
+    for (int pass = 1; pass < s->t1_passes; ++pass)     // outside the per-kernel slots
+      s->launches += launch_t1_extra_pass(s->dev(), s->k, (unsigned)(s->step & 1ull), s->stream);
     ++s->step;
     AVM_CUDA(cudaEventSynchronize(ev[AVM_K_COUNT]));
     for (int j = 0; j < AVM_K_COUNT; ++j) {

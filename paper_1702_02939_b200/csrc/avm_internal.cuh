@@ -35,7 +35,7 @@ struct Counters {
   unsigned int flip_done; // fused schedule: candidates decided so far          } zeroed by the
   unsigned int next_cand; // fused schedule: next candidate index to be claimed  } cell pass of
   unsigned int next_quad; // fused schedule: next candidate whose cells' flagged } every step
-  unsigned int pad;       //                 vertices are to be moved
+  unsigned int pass_cands; // candidates of the latest T1 pass (gates the repeated passes, NEXT-1)
   long long t1_short, t1_candidates, t1_flips, t1_blocked, overflow_rejects, error;
   double energy;
 };
@@ -209,6 +209,7 @@ int launch_t1_flush(const Dev& d, const Consts& k, unsigned long long last_step,
 int launch_refresh_cells(const Dev& d, const Consts& k, cudaStream_t s);
 int launch_t1_reset(const Dev& d, const Consts& k, cudaStream_t s);
 int launch_t1_pass_only(const Dev& d, const Consts& k, cudaStream_t s);
+int launch_t1_extra_pass(const Dev& d, const Consts& k, unsigned parity, cudaStream_t s);
 int launch_t1_debug(const Dev& d, const Consts& k, int* cand_pairs, int* win_pairs, long long capacity, cudaStream_t s);
 int launch_compute_forces(const Dev& d, const Consts& k, double2* ap_scratch, double* force_user, double* ap_user, cudaStream_t s);
 int launch_energy(const Dev& d, const Consts& k, double* partial, cudaStream_t s);

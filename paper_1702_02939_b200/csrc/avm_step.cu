@@ -518,14 +518,39 @@ cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts
 
 // Detection alone (test hooks avm_t1_pass / avm_debug_t1): thread per vertex, edge owned by the
 // smaller current index.
+// gated = true (repeated passes, NEXT-1): nothing to do once a pass has found no candidate.
 __global__ void detect_mark_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, const unsigned parity,
-                                   const bool count_stats) {
+                                   const bool count_stats, const bool gated) {
+  if (gated && d.ctr->pass_cands == 0) return;
   const int v = blockIdx.x * blockDim.x + threadIdx.x;
   if (v >= k.V) return;
+  const double2 h = d.pos[v];
   for (int s = 0; s < 3; ++s) {
     const int w = d.vn[s * k.Vs + v];
-    if (v < w) t1_mark_edge(d, k, v, w, parity, count_stats);
+    if (v < w) {
+      // cheap pre-test; t1_mark_edge repeats the canonical one
+      const double2 q = d.pos[w];
+      const double dx = min_image(q.x - h.x, k.Lx, k.hLx), dy = min_image(q.y - h.y, k.Ly, k.hLy);
+      if (dx * dx + dy * dy < k.lc2) t1_mark_edge(d, k, v, w, parity, count_stats);
+    }
   }
+}
+
+// Repeated passes (NEXT-1; "called repeatedly until no changes").  One more pass on
+// the current state = release the minimum keys of the previous pass's list, empty the list (its
+// length is kept in pass_cands), detect + mark again, flip.  Once a pass has found no candidate
+// the remaining passes of the step are no-ops: nothing to release, detection gated off, empty list.
+__global__ void __launch_bounds__(kT1Block)
+t1_release_kernel(const Dev d, const unsigned parity) {
+  const unsigned n = d.ctr->n_cand[parity];
+  for (unsigned int i = blockIdx.x * kT1Block + threadIdx.x; i < n; i += gridDim.x * kT1Block) {
+    const Cand c = d.cand[i];
+    d.minkey[c.cL] = ~0ull; d.minkey[c.cR] = ~0ull; d.minkey[c.cE1] = ~0ull; d.minkey[c.cE2] = ~0ull;
+  }
+}
+__global__ void t1_empty_kernel(const Dev d, const unsigned parity) {
+  d.ctr->pass_cands = d.ctr->n_cand[parity];
+  d.ctr->n_cand[parity] = 0;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -872,15 +897,23 @@ int launch_t1_reset(const Dev& d, const Consts& k, cudaStream_t s) {
 
 int launch_t1_pass_only(const Dev& d, const Consts& k, cudaStream_t s) {
   int n = launch_t1_reset(d, k, s);
-  detect_mark_kernel<<<cdiv(k.V, 256), 256, 0, s>>>(d, k, 0u, true);
+  detect_mark_kernel<<<cdiv(k.V, 256), 256, 0, s>>>(d, k, 0u, true, false);
   t1_flip_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, k, 0u, true);
   n += 2;
   return n + launch_t1_reset(d, k, s);
 }
 
+int launch_t1_extra_pass(const Dev& d, const Consts& k, unsigned parity, cudaStream_t s) {
+  t1_release_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, parity);
+  t1_empty_kernel<<<1, 1, 0, s>>>(d, parity);
+  detect_mark_kernel<<<cdiv(k.V, 256), 256, 0, s>>>(d, k, parity, true, true);
+  t1_flip_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, k, parity, true);
+  return 4;
+}
+
 int launch_t1_debug(const Dev& d, const Consts& k, int* cand_pairs, int* win_pairs, long long capacity, cudaStream_t s) {
   int n = launch_t1_reset(d, k, s);
-  detect_mark_kernel<<<cdiv(k.V, 256), 256, 0, s>>>(d, k, 0u, false);
+  detect_mark_kernel<<<cdiv(k.V, 256), 256, 0, s>>>(d, k, 0u, false, false);
   t1_debug_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, cand_pairs, win_pairs, capacity);
   return n + 2;   // the caller reads the counters, then calls launch_t1_reset
 }

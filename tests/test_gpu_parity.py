@@ -392,3 +392,33 @@ def test_golden_trace_on_gpu(B):
         assert abs(ap[:, 0].sum() - r["sum_area"]) <= 1e-10 and abs(ap[:, 1].sum() - r["sum_perimeter"]) <= 1e-7
         assert abs(g.energy() - r["energy"]) <= 1e-7 * max(1.0, r["energy"])
         assert abs(s["theta"].sum() - r["theta_sum"]) <= 1e-8
+
+
+@pytest.mark.parametrize("k,steps,sort_every", [(0, 100, 0), (1, 40, 9), (2, 6, 0)])
+def test_repeated_t1_passes_match_the_oracle(B, k, steps, sort_every):
+    """NEXT-1, the paper's own rule: T1 passes repeated within a step until none
+    finds a candidate.  Topology and counters bit-exact, positions within the trajectory
+    tolerance, and no candidate left after the last step."""
+    t = tiling(k)
+    p = dict(w.config_params(k), t1_max_passes=12)
+    g = B.from_tiling(t, **dict(p, sort_every=sort_every))
+    o = oracle.from_tiling(t, **p)
+    one = oracle.from_tiling(t, **w.config_params(k))
+    chunk = max(1, steps // 4)
+    done = 0
+    while done < steps:
+        n = min(chunk, steps - done)
+        g.step(n)
+        o.step(n)
+        done += n
+        assert_states_match(to_np(g.get_state()), o.get_state(), t.Lx, t.Ly)
+    one.step(steps)
+    so = o.get_state()
+    assert so["stats"]["t1_flips"] > 0
+    if k > 0:   # blocked candidates flip within the same step: fewer candidates seen again later
+        assert so["stats"]["t1_blocked"] != one.get_state()["stats"]["t1_blocked"] or \
+            so["stats"]["t1_candidates"] != one.get_state()["stats"]["t1_candidates"]
+    cand, _ = o.debug_t1()
+    assert len(cand) == 0
+    cg, wg = g.debug_t1()
+    assert len(cg) == 0 and len(wg) == 0
