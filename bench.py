@@ -177,6 +177,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (kernel experiments only)")
     ap.add_argument("--profile-steps", type=int, default=100)
+    ap.add_argument("--t1-passes", type=int, default=1,
+                    help="T1 passes per step: 1 = north_star's rule (default, the headline), P > 1 = repeat until none (NEXT-1)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
 
@@ -205,6 +207,8 @@ def main():
 
     cfg = w.CONFIGS[args.config]
     p = dict(w.config_params(args.config), device=local_rank)
+    if args.t1_passes > 1:
+        p["t1_max_passes"] = args.t1_passes
     t = w.config_tiling(args.config)
     N, V = t.N, t.V
 
@@ -302,6 +306,7 @@ def main():
                                    f"(seed {cfg['points_seed']}), p0={cfg['p0']}, v0={cfg['v0']}, Dr={cfg['Dr']}, dt={cfg['dt']}, "
                                    f"l_c={cfg['l_c']}, Hilbert-sorted at create={cfg['sort_at_create']}, sort_every={cfg['sort_every']}",
                        "parallelism": "replicas only" if world > 1 else "1 GPU",
+                       "t1_passes_per_step": args.t1_passes,
                        "l2": f"inputs larger than L2: resident state {224 * N / 1e6:.0f} MB vs 126 MB L2" if 224 * N > 126e6
                              else "state fits in L2 (latency/launch bound config); no flush",
                        "timed_region": f"steps {st0['step']}..{st1['step'] - 1} after {args.warmup} warm-up steps"},
