@@ -294,10 +294,12 @@ void t1_flip(Sim& s, const Cand& c) {
 }
 
 // returns the number of candidates of the pass (0 = the topology is at a fixed point of the rule)
-size_t t1_pass(Sim& s) {
+// count_detect: whether this pass adds to the t1_short / overflow_rejects counters (the first pass
+// of a step does; repeated passes re-see the same ineligible edges and do not count them again)
+size_t t1_pass(Sim& s, bool count_detect = true) {
   std::vector<Cand> cands;
   std::vector<char> win;
-  t1_candidates(s, cands, true);
+  t1_candidates(s, cands, count_detect);
   t1_winners(s, cands, win);
   s.st.t1_candidates += (int64_t)cands.size();
   for (size_t i = 0; i < cands.size(); ++i) {
@@ -336,7 +338,7 @@ void step(Sim& s) {
   // changes"): repeat until a pass finds no candidate, at most t1_max_passes passes
   const int passes = s.p.t1_max_passes > 1 ? s.p.t1_max_passes : 1;
   for (int pass = 0; pass < passes; ++pass)
-    if (t1_pass(s) == 0) break;
+    if (t1_pass(s, pass == 0) == 0) break;
   ++s.st.step;                                                       // 6
 }
 

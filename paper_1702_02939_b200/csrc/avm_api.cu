@@ -46,7 +46,7 @@ struct BufferSet {
 
 struct Layout {
   size_t pos[2], vn[2], vc[2], cv[2], cvn[2], theta[2], rec[2], vtag[2], ctag[2];
-  size_t minkey, cand, ctr, dirty, ap, epart, key[2], val[2], hist, newidx_v, newidx_c, order_v, order_c;
+  size_t minkey, cand, ctr, dirty, estamp, ap, epart, key[2], val[2], hist, newidx_v, newidx_c, order_v, order_c;
   size_t total;
 };
 
@@ -65,6 +65,7 @@ Layout make_layout(const avm_params& p) {
   L.cand = take(sizeof(Cand) * 3 * N);
   L.ctr = take(sizeof(Counters));
   L.dirty = take(4 * ((V + 31) / 32));
+  L.estamp = take(12 * Vs);
   L.ap = take(16 * N);
   L.epart = take(8 * 1024);
   for (int i = 0; i < 2; ++i) { L.key[i] = take(4 * V); L.val[i] = take(4 * V); }
@@ -98,6 +99,8 @@ struct avm_sim {
   Cand* cand;
   Counters* ctr;
   unsigned int* dirty;
+  unsigned int* estamp;
+  unsigned int stamp;    // id of the latest repeated T1 pass (estamp entries equal to it were tested in that pass)
   int t1_passes;         // T1 passes per step (1 = north_star's rule; > 1 = repeat until none, NEXT-1)
   bool fused;            // T1 flips ride in force_move's prologue (cooperative launch available)
   double2* ap;
@@ -113,7 +116,7 @@ struct avm_sim {
     const BufferSet& b = set[cur_set];
     d.vn = b.vn; d.vc = b.vc; d.cv = b.cv; d.cvn = b.cvn; d.theta = b.theta; d.rec = b.rec;
     d.vtag = b.vtag; d.ctag = b.ctag;
-    d.minkey = minkey; d.cand = cand; d.ctr = ctr; d.dirty = dirty;
+    d.minkey = minkey; d.cand = cand; d.ctr = ctr; d.dirty = dirty; d.estamp = estamp;
     return d;
   }
   Dev dev_alt() const {   // the other buffer set, target of a re-sort / staging area
@@ -220,6 +223,24 @@ int do_sort(avm_sim* s) {
   return AVM_OK;
 }
 
+// NEXT-1: the repeated T1 passes of the step just taken (s->step is still that step's index; the
+// position buffers have been swapped already).  Lists alternate between ids 3 and 2.
+int extra_t1_passes(avm_sim* s) {
+  if (s->t1_passes <= 1) return 0;
+  int n = 0;
+  unsigned prev = (unsigned)(s->step & 1ull);
+  for (int pass = 1; pass < s->t1_passes; ++pass) {
+    const unsigned next = 2u + (unsigned)(pass & 1);
+    if (++s->stamp == 0u) {               // wrapped: forget all stamps
+      cudaMemsetAsync(s->estamp, 0, 12 * (size_t)s->k.Vs, s->stream);
+      s->stamp = 1u;
+    }
+    n += launch_t1_extra_pass(s->dev(), s->k, prev, next, s->stamp, s->stream);
+    prev = next;
+  }
+  return n + launch_t1_release(s->dev(), s->k, prev, s->stream);
+}
+
 int read_counters(avm_sim* s, Counters* out) {
   AVM_CUDA(cudaMemcpyAsync(out, s->ctr, sizeof(Counters), cudaMemcpyDeviceToHost, s->stream));
   AVM_CUDA(cudaStreamSynchronize(s->stream));
@@ -251,6 +272,7 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   k.amp = sqrt(2.0 * params->Dr * params->dt);
   k.lc = params->l_c; k.lc2 = params->l_c * params->l_c;
   k.seed = params->seed;
+  k.cap_a = ((params->flags & AVM_FLAG_T1_PASSES_MASK) >> AVM_FLAG_T1_PASSES_SHIFT) > 1 ? N : 3 * N;
   for (int r = 0; r < 10; ++r) k.rkey[r] = philox_round_key(params->seed, r);
   char* w = s->ws;
   for (int i = 0; i < 2; ++i) {
@@ -265,6 +287,8 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   s->cand = (Cand*)(w + L.cand);
   s->ctr = (Counters*)(w + L.ctr);
   s->dirty = (unsigned int*)(w + L.dirty);
+  s->estamp = (unsigned int*)(w + L.estamp);
+  s->stamp = 0;
   s->ap = (double2*)(w + L.ap);
   s->epart = (double*)(w + L.epart);
   s->sc.hist = (unsigned int*)(w + L.hist);
@@ -301,6 +325,7 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   AVM_CUDA_F(cudaMemcpyAsync(b.theta, theta, 8 * (size_t)N, kind, st));
   AVM_CUDA_F(cudaMemsetAsync(s->ctr, 0, sizeof(Counters), st));
   AVM_CUDA_F(cudaMemsetAsync(s->dirty, 0, 4 * (((size_t)V + 31) / 32), st));
+  AVM_CUDA_F(cudaMemsetAsync(s->estamp, 0, 12 * (size_t)k.Vs, st));
   const Dev d = s->dev();
   import_kernel<<<cdiv(V, 256), 256, 0, st>>>(d, k, stage.vn, stage.vc, (const int*)stage.cv);
   validate_kernel<<<cdiv(V, 256), 256, 0, st>>>(d, k);
@@ -401,8 +426,7 @@ int avm_step(avm_sim* s, int64_t n_steps) {
     if (n < 0) n = launch_step(s->dev(), s->k, s->step, s->stream, nullptr, false);
     s->launches += n;
     s->cur_pos = 1 - s->cur_pos;
-    for (int pass = 1; pass < s->t1_passes; ++pass)
-      s->launches += launch_t1_extra_pass(s->dev(), s->k, (unsigned)(s->step & 1ull), s->stream);
+    s->launches += extra_t1_passes(s);
     ++s->step;
     if (s->p.sort_every > 0 && (s->step - s->p.step0) % (unsigned long long)s->p.sort_every == 0) {
       if (pending) { s->launches += launch_t1_flush(s->dev(), s->k, s->step - 1, s->stream); pending = false; }
@@ -431,8 +455,7 @@ int avm_step_profile(avm_sim* s, int64_t n_steps, double* ms_per_kernel) {
     if (n < 0) n = launch_step(s->dev(), s->k, s->step, s->stream, ev, false);
     s->launches += n;
     s->cur_pos = 1 - s->cur_pos;
-    for (int pass = 1; pass < s->t1_passes; ++pass)     // outside the per-kernel slots
-      s->launches += launch_t1_extra_pass(s->dev(), s->k, (unsigned)(s->step & 1ull), s->stream);
+    s->launches += extra_t1_passes(s);                  // outside the per-kernel slots
     ++s->step;
     AVM_CUDA(cudaEventSynchronize(ev[AVM_K_COUNT]));
     for (int j = 0; j < AVM_K_COUNT; ++j) {

@@ -30,12 +30,11 @@ struct __align__(16) Cand {
 struct Counters {
   // candidate list length, double-buffered by step parity: the list of step s is flipped by
   // t1_flip(s) and its per-cell minimum keys are cleared by the prologue of force_move(s+1)
-  unsigned int n_cand[2];
+  unsigned int n_cand[4];   // [0], [1]: the step's list by step parity; [2], [3]: lists of repeated passes (NEXT-1)
   unsigned int n_win;     // winners (debug hook only)
   unsigned int flip_done; // fused schedule: candidates decided so far          } zeroed by the
   unsigned int next_cand; // fused schedule: next candidate index to be claimed  } cell pass of
   unsigned int next_quad; // fused schedule: next candidate whose cells' flagged } every step
-  unsigned int pass_cands; // candidates of the latest T1 pass (gates the repeated passes, NEXT-1)
   long long t1_short, t1_candidates, t1_flips, t1_blocked, overflow_rejects, error;
   double energy;
 };
@@ -50,6 +49,7 @@ struct Consts {
   double v0_3, mu, dt;       // v0_3 = v0 / 3 (Eq. 4 with n = 3, R5)
   double amp;                // sqrt(2 Dr dt) (R8)
   double lc, lc2;
+  int cap_a;                 // capacity of the step's candidate list (3N, or N when repeated passes use the rest)
   unsigned long long seed;
   uint2 rkey[10];            // Philox round keys of `seed` (the key schedule is uniform: done once on the host)
 };
@@ -76,6 +76,7 @@ struct Dev {
   unsigned long long* minkey;  // [N] per-cell minimum candidate key, ~0 when idle
   Cand* cand;         // [3N]
   unsigned int* dirty; // [ceil(V/32)] bit v: vertex v belongs to a cell of some pending T1 candidate
+  unsigned int* estamp; // [3*Vs] per directed half-edge (slot plane, owner vertex): id of the repeated pass that tested it last
   Counters* ctr;
 };
 
@@ -200,6 +201,13 @@ __device__ __forceinline__ void cell_area_perimeter(const double2* pos, const in
   A = __dmul_rn(0.5, acc); P = per;
 }
 
+// Candidate lists.  List 0 / 1 (the step's list, by step parity) starts at d.cand and holds up to
+// k.cap_a entries; lists 2 / 3 (repeated passes, NEXT-1) hold up to N entries each behind it.
+__device__ __forceinline__ Cand* list_base(const Dev& d, const Consts& k, unsigned list) {
+  return d.cand + (list < 2u ? (size_t)0 : (size_t)(list - 1u) * (size_t)k.N);
+}
+__device__ __forceinline__ unsigned list_cap(const Consts& k, unsigned list) { return list < 2u ? (unsigned)k.cap_a : (unsigned)k.N; }
+
 // ---------------------------------------------------------------------------------------------
 // host-side launchers (defined in the .cu files); every launcher returns the number of kernels
 // it enqueued so that the API can keep avm_stats.kernel_launches honest.
@@ -209,7 +217,8 @@ int launch_t1_flush(const Dev& d, const Consts& k, unsigned long long last_step,
 int launch_refresh_cells(const Dev& d, const Consts& k, cudaStream_t s);
 int launch_t1_reset(const Dev& d, const Consts& k, cudaStream_t s);
 int launch_t1_pass_only(const Dev& d, const Consts& k, cudaStream_t s);
-int launch_t1_extra_pass(const Dev& d, const Consts& k, unsigned parity, cudaStream_t s);
+int launch_t1_extra_pass(const Dev& d, const Consts& k, unsigned list_prev, unsigned list_new, unsigned stamp, cudaStream_t s);
+int launch_t1_release(const Dev& d, const Consts& k, unsigned list, cudaStream_t s);
 int launch_t1_debug(const Dev& d, const Consts& k, int* cand_pairs, int* win_pairs, long long capacity, cudaStream_t s);
 int launch_compute_forces(const Dev& d, const Consts& k, double2* ap_scratch, double* force_user, double* ap_user, cudaStream_t s);
 int launch_energy(const Dev& d, const Consts& k, double* partial, cudaStream_t s);

@@ -286,7 +286,7 @@ force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts 
   const int tid = blockIdx.x * kVertexBlock + threadIdx.x;
   const int stride = gridDim.x * kVertexBlock;
   const int lane = threadIdx.x & 31;
-  const unsigned prev = d.ctr->n_cand[parity ^ 1u];
+  const unsigned prev = min(d.ctr->n_cand[parity ^ 1u], (unsigned)k.cap_a);
   const unsigned gwarp = (unsigned)tid >> 5, nwarps = (unsigned)stride >> 5;
   if (tid == 0) d.ctr->n_cand[parity] = 0;
   if (kFused) {
@@ -377,7 +377,11 @@ __device__ __noinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va,
   cd.sx1 = x1s1 == v1 ? 1 : x1s2 == v1 ? 2 : 0;
   cd.sx2 = x2s1 == v2 ? 1 : x2s2 == v2 ? 2 : 0;
   const unsigned int slot = atomicAdd(&d.ctr->n_cand[parity], 1u);
-  d.cand[slot] = cd;
+  if (slot >= list_cap(k, parity)) {          // cannot happen for a tiling (<= 3N edges; N per repeated pass)
+    atomicOr((unsigned long long*)&d.ctr->error, 8ull);
+    return;
+  }
+  list_base(d, k, parity)[slot] = cd;
   atomicMin(&d.minkey[cL], cd.key);
   atomicMin(&d.minkey[cR], cd.key);
   atomicMin(&d.minkey[cE1], cd.key);
@@ -518,10 +522,8 @@ cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts
 
 // Detection alone (test hooks avm_t1_pass / avm_debug_t1): thread per vertex, edge owned by the
 // smaller current index.
-// gated = true (repeated passes, NEXT-1): nothing to do once a pass has found no candidate.
 __global__ void detect_mark_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, const unsigned parity,
-                                   const bool count_stats, const bool gated) {
-  if (gated && d.ctr->pass_cands == 0) return;
+                                   const bool count_stats) {
   const int v = blockIdx.x * blockDim.x + threadIdx.x;
   if (v >= k.V) return;
   const double2 h = d.pos[v];
@@ -536,21 +538,59 @@ __global__ void detect_mark_kernel(const __grid_constant__ Dev d, const __grid_c
   }
 }
 
-// Repeated passes (NEXT-1; "called repeatedly until no changes").  One more pass on
-// the current state = release the minimum keys of the previous pass's list, empty the list (its
-// length is kept in pass_cands), detect + mark again, flip.  Once a pass has found no candidate
-// the remaining passes of the step are no-ops: nothing to release, detection gated off, empty list.
+// Repeated passes (NEXT-1; "called repeatedly until no changes").  A further pass
+// on the current state can only find candidates among the edges that have an endpoint in a cell
+// of a candidate of the previous pass: lengths changed only at flipped vertices, eligibility
+// (R10) only through the vertex counts of a flipped candidate's four cells, and blocked
+// candidates are such edges themselves.  So one more pass =
+//   release : clear the minimum keys of the previous pass's list, empty the new list;
+//   detect  : one warp per previous candidate tests the edges of every vertex of its four cells
+//             (each edge once per pass: stamp on the half-edge of its smaller endpoint) and marks;
+//   flip    : t1_flip_kernel on the new list.
+// When a pass found nothing, the following ones have nothing to release, test or flip.
 __global__ void __launch_bounds__(kT1Block)
-t1_release_kernel(const Dev d, const unsigned parity) {
-  const unsigned n = d.ctr->n_cand[parity];
+t1_release_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, const unsigned list, const int empty_list) {
+  const unsigned n = min(d.ctr->n_cand[list], list_cap(k, list));
+  const Cand* __restrict__ l = list_base(d, k, list);
   for (unsigned int i = blockIdx.x * kT1Block + threadIdx.x; i < n; i += gridDim.x * kT1Block) {
-    const Cand c = d.cand[i];
+    const Cand c = l[i];
     d.minkey[c.cL] = ~0ull; d.minkey[c.cR] = ~0ull; d.minkey[c.cE1] = ~0ull; d.minkey[c.cE2] = ~0ull;
   }
+  if (empty_list >= 0 && blockIdx.x == 0 && threadIdx.x == 0) d.ctr->n_cand[empty_list] = 0;
 }
-__global__ void t1_empty_kernel(const Dev d, const unsigned parity) {
-  d.ctr->pass_cands = d.ctr->n_cand[parity];
-  d.ctr->n_cand[parity] = 0;
+
+__global__ void __launch_bounds__(kT1Block)
+t1_local_detect_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, const unsigned list_prev,
+                       const unsigned list_new, const unsigned stamp) {
+  const unsigned n = min(d.ctr->n_cand[list_prev], list_cap(k, list_prev));
+  const Cand* __restrict__ l = list_base(d, k, list_prev);
+  const int lane = threadIdx.x & 31;
+  const unsigned gwarp = (blockIdx.x * kT1Block + threadIdx.x) >> 5, nwarps = (gridDim.x * kT1Block) >> 5;
+  for (unsigned int i = gwarp; i < n; i += nwarps) {
+    const Cand c = l[i];
+    const int quad[4] = {c.cL, c.cR, c.cE1, c.cE2};
+#pragma unroll 1
+    for (int t = 0; t < 4; ++t) {
+      const int nrow = d.cvn[quad[t]];
+      if (lane >= nrow) continue;
+      const int u = row_entry(d.cv, k.N, quad[t], lane);
+      const double2 hu = d.pos[u];
+#pragma unroll 1
+      for (int sl = 0; sl < 3; ++sl) {
+        const int wv = d.vn[sl * k.Vs + u];
+        // the half-edge of the smaller endpoint identifies the edge
+        int owner = u, other = wv, oslot = sl;
+        if (wv < u) {
+          owner = wv; other = u;
+          oslot = d.vn[wv] == u ? 0 : d.vn[k.Vs + wv] == u ? 1 : 2;
+        }
+        if (atomicExch(&d.estamp[(size_t)oslot * k.Vs + owner], stamp) == stamp) continue;   // tested in this pass already
+        const double2 hw = d.pos[wv];
+        const double dx = min_image(hw.x - hu.x, k.Lx, k.hLx), dy = min_image(hw.y - hu.y, k.Ly, k.hLy);
+        if (dx * dx + dy * dy < k.lc2) t1_mark_edge(d, k, owner, other, list_new, false);
+      }
+    }
+  }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -687,13 +727,14 @@ __global__ void __launch_bounds__(kT1Block)
 t1_flip_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, const unsigned parity, const bool count_stats) {
   pdl_launch_dependents();
   pdl_wait();
-  const unsigned int n_cand = d.ctr->n_cand[parity];
+  const unsigned int n_cand = min(d.ctr->n_cand[parity], list_cap(k, parity));
+  const Cand* __restrict__ list = list_base(d, k, parity);
   const int lane = threadIdx.x & 31;
   const unsigned gwarp = (blockIdx.x * kT1Block + threadIdx.x) >> 5, nwarps = (gridDim.x * kT1Block) >> 5;
   if (count_stats && gwarp == 0 && lane == 0 && n_cand) atomicAdd((unsigned long long*)&d.ctr->t1_candidates, (unsigned long long)n_cand);
   unsigned int flips = 0, blocked = 0;
   for (unsigned int i = gwarp; i < n_cand; i += nwarps) {
-    const Cand c = d.cand[i];
+    const Cand c = list[i];
     if (t1_try_flip(d, k, c, lane)) ++flips; else ++blocked;
   }
   if (count_stats && lane == 0) {
@@ -705,15 +746,15 @@ t1_flip_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, 
 // Clears the minimum keys of both candidate lists and empties them (before a re-sort, around the
 // test hooks).  Inside avm_step this work rides in force_move's prologue instead.
 __global__ void __launch_bounds__(kT1Block)
-t1_reset_kernel(const Dev d) {
+t1_reset_kernel(const Dev d, const unsigned cap) {
   const unsigned n0 = d.ctr->n_cand[0], n1 = d.ctr->n_cand[1];
-  const unsigned n = n0 > n1 ? n0 : n1;
+  const unsigned n = min(n0 > n1 ? n0 : n1, cap);
   for (unsigned int i = blockIdx.x * kT1Block + threadIdx.x; i < n; i += gridDim.x * kT1Block) {
     const Cand c = d.cand[i];
     d.minkey[c.cL] = ~0ull; d.minkey[c.cR] = ~0ull; d.minkey[c.cE1] = ~0ull; d.minkey[c.cE2] = ~0ull;
   }
 }
-__global__ void zero_counts_kernel(const Dev d) { d.ctr->n_cand[0] = 0; d.ctr->n_cand[1] = 0; d.ctr->n_win = 0; d.ctr->flip_done = 0; d.ctr->next_cand = 0; d.ctr->next_quad = 0; }
+__global__ void zero_counts_kernel(const Dev d) { d.ctr->n_cand[0] = 0; d.ctr->n_cand[1] = 0; d.ctr->n_cand[2] = 0; d.ctr->n_cand[3] = 0; d.ctr->n_win = 0; d.ctr->flip_done = 0; d.ctr->next_cand = 0; d.ctr->next_quad = 0; }
 
 // debug hook: winners without flipping; (tag_min, tag_max) pairs out
 __global__ void t1_debug_kernel(const Dev d, int* cand_pairs, int* win_pairs, long long capacity) {
@@ -889,7 +930,7 @@ int launch_refresh_cells(const Dev& d, const Consts& k, cudaStream_t s) {
 
 // leaves minkey all-idle and both candidate lists empty
 int launch_t1_reset(const Dev& d, const Consts& k, cudaStream_t s) {
-  t1_reset_kernel<<<kT1Grid, kT1Block, 0, s>>>(d);
+  t1_reset_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, (unsigned)k.cap_a);
   zero_counts_kernel<<<1, 1, 0, s>>>(d);
   cudaMemsetAsync(d.dirty, 0, sizeof(unsigned int) * (size_t)((k.V + 31) / 32), s);
   return 2;
@@ -897,23 +938,27 @@ int launch_t1_reset(const Dev& d, const Consts& k, cudaStream_t s) {
 
 int launch_t1_pass_only(const Dev& d, const Consts& k, cudaStream_t s) {
   int n = launch_t1_reset(d, k, s);
-  detect_mark_kernel<<<cdiv(k.V, 256), 256, 0, s>>>(d, k, 0u, true, false);
+  detect_mark_kernel<<<cdiv(k.V, 256), 256, 0, s>>>(d, k, 0u, true);
   t1_flip_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, k, 0u, true);
   n += 2;
   return n + launch_t1_reset(d, k, s);
 }
 
-int launch_t1_extra_pass(const Dev& d, const Consts& k, unsigned parity, cudaStream_t s) {
-  t1_release_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, parity);
-  t1_empty_kernel<<<1, 1, 0, s>>>(d, parity);
-  detect_mark_kernel<<<cdiv(k.V, 256), 256, 0, s>>>(d, k, parity, true, true);
-  t1_flip_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, k, parity, true);
-  return 4;
+int launch_t1_release(const Dev& d, const Consts& k, unsigned list, cudaStream_t s) {
+  t1_release_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, k, list, (int)list);
+  return 1;
+}
+
+int launch_t1_extra_pass(const Dev& d, const Consts& k, unsigned list_prev, unsigned list_new, unsigned stamp, cudaStream_t s) {
+  t1_release_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, k, list_prev, (int)list_new);
+  t1_local_detect_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, k, list_prev, list_new, stamp);
+  t1_flip_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, k, list_new, true);
+  return 3;
 }
 
 int launch_t1_debug(const Dev& d, const Consts& k, int* cand_pairs, int* win_pairs, long long capacity, cudaStream_t s) {
   int n = launch_t1_reset(d, k, s);
-  detect_mark_kernel<<<cdiv(k.V, 256), 256, 0, s>>>(d, k, 0u, false, false);
+  detect_mark_kernel<<<cdiv(k.V, 256), 256, 0, s>>>(d, k, 0u, false);
   t1_debug_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, cand_pairs, win_pairs, capacity);
   return n + 2;   // the caller reads the counters, then calls launch_t1_reset
 }
