@@ -2,19 +2,21 @@
 //
 // Paper order of one step (PAPER.md:62-64 §II.B, :104-108 §II.D; R6):
 //   geometry -> forces -> move vertices -> rotate directors -> T1 test/update.
-// Kernel schedule used here, three launches per step:
+// Kernel schedule used here:
 //   force_move   (thread/vertex)  rows a2+a3: F_v from the 3 incident cells' cached (a,p) records
 //                                  and the 3 neighbour positions, Euler step of Eq. 4, wrap.
-//                                  Prologue: clears the per-cell minimum keys the previous step's
-//                                  T1 candidates left behind.
 //   cell_update  (thread/cell)    rows a4+a1+a5+a6: director noise, then area/perimeter of the MOVED
 //                                  tiling (= the geometry the next step's forces need); edges found
 //                                  shorter than l_c are tested for eligibility by the detecting
 //                                  thread, appended to the candidate list and their key is
 //                                  atomicMin-ed into the four cells (conflict rule, marking half).
-//   t1_flip      (warp/candidate) rows a6+a7: a candidate whose key is the minimum on all four of
-//                                  its cells flips; the warp rewrites the four lists cooperatively
-//                                  and refreshes the four cells' cached geometry.
+//   T1 flips     (warp/candidate) rows a6+a7 (t1_try_flip): a candidate whose key is the minimum on
+//                                  all four of its cells flips; the warp rewrites the four lists
+//                                  cooperatively and refreshes the four cells' cached geometry.
+//                                  Two-launch schedule (large systems): run by a few "flipper"
+//                                  warps inside the NEXT step's force_move launch while the other
+//                                  warps sweep.  Three-launch schedule: t1_flip_kernel.
+//   repeated T1 passes (NEXT-1)    t1_release / t1_local_detect / t1_flip per extra pass.
 // Geometry is thus evaluated once per step on the positions the forces of the following step
 // act on; after a flip the records of its four cells are refreshed in place, so every force is
 // computed from the geometry of the current topology exactly as in the paper's cycle.
@@ -550,6 +552,8 @@ __global__ void detect_mark_kernel(const __grid_constant__ Dev d, const __grid_c
 // When a pass found nothing, the following ones have nothing to release, test or flip.
 __global__ void __launch_bounds__(kT1Block)
 t1_release_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, const unsigned list, const int empty_list) {
+  pdl_launch_dependents();
+  pdl_wait();
   const unsigned n = min(d.ctr->n_cand[list], list_cap(k, list));
   const Cand* __restrict__ l = list_base(d, k, list);
   for (unsigned int i = blockIdx.x * kT1Block + threadIdx.x; i < n; i += gridDim.x * kT1Block) {
@@ -562,6 +566,8 @@ t1_release_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts 
 __global__ void __launch_bounds__(kT1Block)
 t1_local_detect_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, const unsigned list_prev,
                        const unsigned list_new, const unsigned stamp) {
+  pdl_launch_dependents();
+  pdl_wait();
   const unsigned n = min(d.ctr->n_cand[list_prev], list_cap(k, list_prev));
   const Cand* __restrict__ l = list_base(d, k, list_prev);
   const int lane = threadIdx.x & 31;
@@ -945,14 +951,15 @@ int launch_t1_pass_only(const Dev& d, const Consts& k, cudaStream_t s) {
 }
 
 int launch_t1_release(const Dev& d, const Consts& k, unsigned list, cudaStream_t s) {
-  t1_release_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, k, list, (int)list);
+  launch_chained(t1_release_kernel, kT1Grid, kT1Block, s, AVM_PDL != 0, false, d, k, list, (int)list);
   return 1;
 }
 
 int launch_t1_extra_pass(const Dev& d, const Consts& k, unsigned list_prev, unsigned list_new, unsigned stamp, cudaStream_t s) {
-  t1_release_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, k, list_prev, (int)list_new);
-  t1_local_detect_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, k, list_prev, list_new, stamp);
-  t1_flip_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, k, list_new, true);
+  const bool pdl = AVM_PDL != 0;     // part of the step's chain of dependent launches
+  launch_chained(t1_release_kernel, kT1Grid, kT1Block, s, pdl, false, d, k, list_prev, (int)list_new);
+  launch_chained(t1_local_detect_kernel, kT1Grid, kT1Block, s, pdl, false, d, k, list_prev, list_new, stamp);
+  launch_chained(t1_flip_kernel, kT1Grid, kT1Block, s, pdl, false, d, k, list_new, true);
   return 3;
 }
 
