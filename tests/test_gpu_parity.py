@@ -422,3 +422,61 @@ def test_repeated_t1_passes_match_the_oracle(B, k, steps, sort_every):
     assert len(cand) == 0
     cg, wg = g.debug_t1()
     assert len(cg) == 0 and len(wg) == 0
+
+
+def test_long_run_at_the_config_length_keeps_every_invariant(B):
+    """configs[2] for its full 10^4 steps (fluid regime, ~60 flips per step, a re-sort every 500):
+    far beyond what the oracle can follow, so what is checked is what holds at any length —
+    a valid 3-coordinated tiling of the torus with the slot convention intact, areas tiling the
+    box, a clean error word, and the create-validation accepting the exported state again."""
+    t = tiling(2)
+    p = dict(w.config_params(2), sort_every=500)
+    g = B.from_tiling(t, **p)
+    g.step(10000)
+    s = to_np(g.get_state())
+    assert s["stats"]["error"] == 0 and s["stats"]["n_sorts"] >= 20
+    assert s["stats"]["t1_flips"] > 100000
+    assert s["stats"]["t1_flips"] + s["stats"]["t1_blocked"] == s["stats"]["t1_candidates"]
+    assert np.isfinite(s["pos"]).all() and (s["pos"] >= 0).all() and (s["pos"][:, 0] < t.Lx).all()
+    h.check_topology(s["cell_vertex_num"], s["cell_vertices"], s["vertex_neighbors"], s["vertex_cell_neighbors"], S=t.S)
+    ap = g.compute_forces()[1].cpu().numpy()
+    L2 = t.Lx * t.Ly
+    assert abs(ap[:, 0].sum() - L2) <= 1e-12 * L2
+    assert (ap[:, 1] > 0).all()
+    # the exported state is a consistent input (avm_create validates lists against each other)
+    tt = w.Tiling(t.Lx, t.Ly, t.S, s["pos"], s["cell_vertex_num"], s["cell_vertices"], s["vertex_neighbors"],
+                  s["vertex_cell_neighbors"], s["theta"])
+    g2 = B.from_tiling(tt, **dict(p, step0=10000))
+    g2.step(1)
+    g.step(1)
+    s1, s2 = to_np(g.get_state()), to_np(g2.get_state())
+    assert np.array_equal(s1["pos"], s2["pos"]) and np.array_equal(s1["theta"], s2["theta"])
+
+
+def test_two_launch_schedule_at_full_size_equals_three_launch_schedule(B, monkeypatch):
+    """configs[3] (N = 1,048,576, the bench workload) for 300 steps with a re-sort every 100: the
+    default two-launch schedule — ~96 000 simultaneous candidates in step 0 (every warp flips),
+    then a few dozen per step (a few flipper warps) — against the three-launch schedule, bit for bit."""
+    t = tiling(3)
+    p = dict(w.config_params(3), sort_every=100)
+    a = B.from_tiling(t, **p)
+    a.step(300)
+    sa = to_np(a.get_state())
+    area = a.compute_forces()[1][:, 0].sum().item()
+    a.close()
+    del a
+    monkeypatch.setenv("AVM_B200_UNFUSED", "1")
+    b = B.from_tiling(t, **p)
+    b.step(300)
+    sb = to_np(b.get_state())
+    b.close()
+    monkeypatch.delenv("AVM_B200_UNFUSED")
+    assert sa["stats"]["kernel_launches"] < sb["stats"]["kernel_launches"]
+    for key in ("pos", "theta", "cell_vertices", "vertex_neighbors", "vertex_cell_neighbors", "cell_vertex_num"):
+        assert np.array_equal(sa[key], sb[key]), key
+    for key in ("t1_short", "t1_candidates", "t1_flips", "t1_blocked", "overflow_rejects", "error"):
+        assert sa["stats"][key] == sb["stats"][key], key
+    assert sa["stats"]["error"] == 0 and sa["stats"]["t1_flips"] > 90000
+    L2 = t.Lx * t.Ly
+    assert abs(area - L2) <= 1e-12 * L2
+    _TILINGS.pop(3, None)
