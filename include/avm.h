@@ -137,6 +137,18 @@ int avm_compute_forces_host(avm_sim* sim, double* force_xy, double* area_perim);
  * fixed order (deterministic).  energy is a HOST pointer; synchronises the stream. */
 int avm_energy(avm_sim* sim, double* energy);
 
+/* Observables of the current state, reduced on the device in a
+ * fixed order (deterministic): the energy of Eq. 1, the area and perimeter totals, the mean shape
+ * index <P / sqrt(A)> over the cells with A > 0 (the order parameter of the rigidity transition
+ * the paper's model is used for), area extremes and variance, the number of cells
+ * with non-positive signed area (transiently possible, R14), and the running T1 count.
+ * out is a HOST pointer; synchronises the stream. */
+typedef struct avm_observables {
+  double energy, sum_area, sum_perimeter, mean_shape_index, area_min, area_max, area_variance;
+  int64_t n_nonpositive_area, step, t1_flips;
+} avm_observables;
+int avm_observe(avm_sim* sim, avm_observables* out);
+
 /* Copy the current state out in user order.  stats (HOST pointer, may be NULL) receives the
  * counters; when it is non-NULL, or for the host variant, the call synchronises the stream. */
 int avm_get_state(avm_sim* sim, double* pos_xy, int32_t* cell_vertex_num, int32_t* cell_vertices,

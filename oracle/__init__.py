@@ -135,6 +135,19 @@ class OracleSim:
     def energy(self) -> float:
         return float(_load().oracle_energy(self._h))
 
+    def observables(self) -> dict:
+        """NEXT-2: the definitions, written out with numpy on the oracle's own geometry: energy of
+        Eq. 1, totals, mean shape index <P / sqrt(A)> over cells with A > 0, area
+        extremes and (population) variance, number of cells with non-positive signed area."""
+        ap = self.geometry()
+        A, P = ap[:, 0], ap[:, 1]
+        pos = A > 0
+        return {"energy": self.energy(), "sum_area": float(A.sum()), "sum_perimeter": float(P.sum()),
+                "mean_shape_index": float((P[pos] / np.sqrt(A[pos])).mean()) if pos.any() else 0.0,
+                "area_min": float(A.min()), "area_max": float(A.max()),
+                "area_variance": float((A * A).mean() - A.mean() ** 2),
+                "n_nonpositive_area": int((~pos).sum())}
+
     def compute_forces(self):
         F = np.empty((self.V, 2), dtype=np.float64)
         ap = np.empty((self.N, 2), dtype=np.float64)

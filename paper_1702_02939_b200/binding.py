@@ -21,7 +21,7 @@ LIB_PATH = os.environ.get("AVM_B200_LIB") or os.path.join(_HERE, "libavm_b200.so
 # every symbol include/avm.h declares (tests check that the library exports all of them)
 ABI_SYMBOLS = [
     "avm_workspace_bytes", "avm_create", "avm_create_host", "avm_step", "avm_step_profile", "avm_compute_forces",
-    "avm_compute_forces_host", "avm_energy", "avm_get_state", "avm_get_state_host", "avm_debug_t1",
+    "avm_compute_forces_host", "avm_energy", "avm_observe", "avm_get_state", "avm_get_state_host", "avm_debug_t1",
     "avm_t1_pass", "avm_set_positions", "avm_resort", "avm_philox_words", "avm_hilbert_index",
     "avm_hilbert_index_host", "avm_destroy", "avm_strerror", "avm_last_cuda_error",
 ]
@@ -51,6 +51,15 @@ class AvmStats(ctypes.Structure):
         return {n: int(getattr(self, n)) for n, _ in self._fields_}
 
 
+class AvmObservables(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_double) for n in ("energy", "sum_area", "sum_perimeter", "mean_shape_index", "area_min",
+                                               "area_max", "area_variance")] + \
+               [(n, ctypes.c_int64) for n in ("n_nonpositive_area", "step", "t1_flips")]
+
+    def as_dict(self):
+        return {n: getattr(self, n) for n, _ in self._fields_}
+
+
 class AvmError(RuntimeError):
     pass
 
@@ -74,6 +83,7 @@ def _load() -> ctypes.CDLL:
     lib.avm_compute_forces.argtypes = [p, p, p]
     lib.avm_compute_forces_host.argtypes = [p, p, p]
     lib.avm_energy.argtypes = [p, ctypes.POINTER(ctypes.c_double)]
+    lib.avm_observe.argtypes = [p, ctypes.POINTER(AvmObservables)]
     for name in ("avm_get_state", "avm_get_state_host"):
         getattr(lib, name).argtypes = [p, p, p, p, p, p, p, ctypes.POINTER(AvmStats)]
     lib.avm_debug_t1.argtypes = [p, p, ctypes.POINTER(i64), p, ctypes.POINTER(i64), i64]
@@ -203,6 +213,11 @@ class AvmSim:
         e = ctypes.c_double(0.0)
         _check(lib.avm_energy(self._h, ctypes.byref(e)))
         return e.value
+
+    def observe(self) -> dict:
+        o = AvmObservables()
+        _check(lib.avm_observe(self._h, ctypes.byref(o)))
+        return o.as_dict()
 
     def get_state(self, stats: bool = True) -> dict:
         t = self.torch

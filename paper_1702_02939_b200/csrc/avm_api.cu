@@ -67,7 +67,7 @@ Layout make_layout(const avm_params& p) {
   L.dirty = take(4 * ((V + 31) / 32));
   L.estamp = take(12 * Vs);
   L.ap = take(16 * N);
-  L.epart = take(8 * 1024);
+  L.epart = take(8 * 8 * 512);   // block partials of the observables (8 slots x up to 512 blocks)
   for (int i = 0; i < 2; ++i) { L.key[i] = take(4 * V); L.val[i] = take(4 * V); }
   L.hist = take(4 * sort_hist_entries((int)V));
   L.newidx_v = take(4 * V); L.newidx_c = take(4 * N); L.order_v = take(4 * V); L.order_c = take(4 * N);
@@ -508,7 +508,28 @@ int avm_energy(avm_sim* s, double* energy) {
   Counters c;
   int rc = read_counters(s, &c);
   if (rc) return rc;
-  *energy = c.energy;
+  *energy = c.obs[0];
+  return AVM_OK;
+}
+
+int avm_observe(avm_sim* s, avm_observables* out) {
+  if (!s || !out) return AVM_EINVAL;
+  s->launches += launch_energy(s->dev(), s->k, s->epart, s->stream);
+  Counters c;
+  int rc = read_counters(s, &c);
+  if (rc) return rc;
+  const double N = (double)s->k.N;
+  out->energy = c.obs[0];
+  out->sum_area = c.obs[1];
+  out->sum_perimeter = c.obs[2];
+  out->n_nonpositive_area = (int64_t)c.obs[4];
+  const double npos = N - c.obs[4];
+  out->mean_shape_index = npos > 0.0 ? c.obs[3] / npos : 0.0;
+  out->area_variance = c.obs[5] / N - (c.obs[1] / N) * (c.obs[1] / N);
+  out->area_min = c.obs[6];
+  out->area_max = c.obs[7];
+  out->step = (int64_t)s->step;
+  out->t1_flips = c.t1_flips;
   return AVM_OK;
 }
 

@@ -36,7 +36,7 @@ struct Counters {
   unsigned int next_cand; // fused schedule: next candidate index to be claimed  } cell pass of
   unsigned int next_quad; // fused schedule: next candidate whose cells' flagged } every step
   long long t1_short, t1_candidates, t1_flips, t1_blocked, overflow_rejects, error;
-  double energy;
+  double obs[8];   // observables of the latest avm_energy / avm_observe call (slots: avm_step.cu)
 };
 
 // Model constants, passed by value to every kernel.

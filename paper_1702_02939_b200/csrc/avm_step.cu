@@ -817,35 +817,51 @@ __global__ void forces_kernel(const Dev d, const Consts k, const double2* __rest
   force_user[2 * t] = f.x; force_user[2 * t + 1] = f.y;
 }
 
-// Energy, Eq. 1 / A1: block partial sums in a fixed order, finished by one
-// block (deterministic, no floating-point atomics).
-__global__ void energy_partial_kernel(const Dev d, const Consts k, double* __restrict__ partial) {
-  __shared__ double sm[256];
-  double e = 0.0;
+// Observables of the current state (NEXT-2): energy, Eq. 1 / A1, and the
+// per-cell statistics a user of the model measures (shape index P / sqrt(A), area moments).
+// Slots: 0 energy, 1 sum A, 2 sum P, 3 sum P/sqrt(A) over cells with A > 0, 4 number of cells with
+// A <= 0, 5 sum A^2, 6 min A, 7 max A.  Block partials in a fixed order, finished by one block
+// (deterministic, no floating-point atomics).
+static constexpr int kObs = 8;
+__device__ __forceinline__ double obs_combine(int slot, double a, double b) {
+  return slot < 6 ? a + b : slot == 6 ? fmin(a, b) : fmax(a, b);
+}
+__device__ __forceinline__ void obs_block_reduce(double (&x)[kObs], double (*sm)[256]) {
+#pragma unroll
+  for (int q = 0; q < kObs; ++q) sm[q][threadIdx.x] = x[q];
+  __syncthreads();
+  for (int s = 128; s > 0; s >>= 1) {
+    if (threadIdx.x < s)
+#pragma unroll
+      for (int q = 0; q < kObs; ++q) sm[q][threadIdx.x] = obs_combine(q, sm[q][threadIdx.x], sm[q][threadIdx.x + s]);
+    __syncthreads();
+  }
+}
+__global__ void __launch_bounds__(256)
+observables_partial_kernel(const Dev d, const Consts k, double* __restrict__ partial) {
+  __shared__ double sm[kObs][256];
+  double x[kObs] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 1.0e300, -1.0e300};
   for (int c = blockIdx.x * 256 + threadIdx.x; c < k.N; c += gridDim.x * 256) {
     double A, P;
     cell_area_perimeter(d.pos, d.cv, c, d.cvn[c], k, A, P);
-    e += k.KA * (A - k.A0) * (A - k.A0) + k.KP * (P - k.P0) * (P - k.P0);
+    x[0] += k.KA * (A - k.A0) * (A - k.A0) + k.KP * (P - k.P0) * (P - k.P0);
+    x[1] += A; x[2] += P;
+    if (A > 0.0) x[3] += P / sqrt(A); else x[4] += 1.0;
+    x[5] += A * A;
+    x[6] = fmin(x[6], A); x[7] = fmax(x[7], A);
   }
-  sm[threadIdx.x] = e;
-  __syncthreads();
-  for (int s = 128; s > 0; s >>= 1) {
-    if (threadIdx.x < s) sm[threadIdx.x] += sm[threadIdx.x + s];
-    __syncthreads();
-  }
-  if (threadIdx.x == 0) partial[blockIdx.x] = sm[0];
+  obs_block_reduce(x, sm);
+  if (threadIdx.x < kObs) partial[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = sm[threadIdx.x][0];
 }
-__global__ void energy_final_kernel(const Dev d, const double* __restrict__ partial, int n) {
-  __shared__ double sm[256];
-  double e = 0.0;
-  for (int i = threadIdx.x; i < n; i += 256) e += partial[i];
-  sm[threadIdx.x] = e;
-  __syncthreads();
-  for (int s = 128; s > 0; s >>= 1) {
-    if (threadIdx.x < s) sm[threadIdx.x] += sm[threadIdx.x + s];
-    __syncthreads();
-  }
-  if (threadIdx.x == 0) d.ctr->energy = sm[0];
+__global__ void __launch_bounds__(256)
+observables_final_kernel(const Dev d, const double* __restrict__ partial, int n) {
+  __shared__ double sm[kObs][256];
+  double x[kObs] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 1.0e300, -1.0e300};
+  for (int i = threadIdx.x; i < n; i += 256)
+#pragma unroll
+    for (int q = 0; q < kObs; ++q) x[q] = obs_combine(q, x[q], partial[(size_t)q * n + i]);
+  obs_block_reduce(x, sm);
+  if (threadIdx.x < kObs) d.ctr->obs[threadIdx.x] = sm[threadIdx.x][0];
 }
 
 __global__ void philox_words_kernel(unsigned long long seed, unsigned long long step, unsigned long long cell0,
@@ -978,9 +994,9 @@ int launch_compute_forces(const Dev& d, const Consts& k, double2* ap_scratch, do
 }
 
 int launch_energy(const Dev& d, const Consts& k, double* partial, cudaStream_t s) {
-  const int nb = 148 * 2;
-  energy_partial_kernel<<<nb, 256, 0, s>>>(d, k, partial);
-  energy_final_kernel<<<1, 256, 0, s>>>(d, partial, nb);
+  const int nb = 148 * 2;      // partial holds kObs * nb doubles
+  observables_partial_kernel<<<nb, 256, 0, s>>>(d, k, partial);
+  observables_final_kernel<<<1, 256, 0, s>>>(d, partial, nb);
   return 2;
 }
 

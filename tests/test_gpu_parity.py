@@ -480,3 +480,23 @@ def test_two_launch_schedule_at_full_size_equals_three_launch_schedule(B, monkey
     L2 = t.Lx * t.Ly
     assert abs(area - L2) <= 1e-12 * L2
     _TILINGS.pop(3, None)
+
+
+@pytest.mark.parametrize("k,steps", [(0, 25), (1, 10)])
+def test_observables_match_the_oracle(B, k, steps):
+    """NEXT-2: avm_observe against the numpy definitions on the oracle's geometry, on the start
+    tiling and inside the step-0 burst (where some cells are transiently inverted)."""
+    t = tiling(k)
+    p = w.config_params(k)
+    g = B.from_tiling(t, **dict(p, sort_at_create=True))
+    o = oracle.from_tiling(t, **p)
+    for n in (0, 1, steps):
+        g.step(n)
+        o.step(n)
+        a, b = g.observe(), o.observables()
+        for key in ("energy", "sum_area", "sum_perimeter", "mean_shape_index", "area_min", "area_max", "area_variance"):
+            assert abs(a[key] - b[key]) <= 1e-9 * max(1.0, abs(b[key])), (n, key, a[key], b[key])
+        assert a["n_nonpositive_area"] == b["n_nonpositive_area"]
+        assert a["step"] == o.get_state()["stats"]["step"] and a["t1_flips"] == o.get_state()["stats"]["t1_flips"]
+        assert abs(a["energy"] - g.energy()) == 0.0
+    assert abs(a["sum_area"] - t.Lx * t.Ly) <= 1e-12 * t.Lx * t.Ly

@@ -3,6 +3,8 @@
 Nothing here compares the oracle with itself: closed forms for regular hexagons, central finite
 differences of Eq. A1 (the energy is a different code path from the force), conservation laws,
 and an independent numpy shoelace / scipy cross-check."""
+import math
+
 import numpy as np
 import pytest
 
@@ -163,3 +165,28 @@ def test_energy_definition_has_no_half():
     ap = h.polygon_areas_numpy(t.pos, t.cell_vertex_num, t.cell_vertices, t.Lx, t.Ly)
     E = np.sum(p["KA"] * (ap[:, 0] - p["A0"]) ** 2 + p["KP"] * (ap[:, 1] - p["P0"]) ** 2)
     assert abs(sim.energy() - E) <= 1e-12 * E
+
+
+def test_observables_closed_forms_on_hexagons_and_voronoi():
+    """NEXT-2 pins: regular hexagons of side a have shape index 6a / sqrt(3 sqrt(3)/2 a^2) =
+    3.72241943..., zero area variance and E = N [KA (A-A0)^2 + KP (P-P0)^2]; on a Voronoi tiling
+    the areas sum to L^2, so the mean area is L^2 / N and the variance follows from the cells."""
+    a = 0.8
+    t = w.hex_tiling(6, 4, a=a)
+    o = oracle.from_tiling(t, KA=1.3, KP=0.7, A0=1.0, P0=3.9)
+    ob = o.observables()
+    A, P = 1.5 * math.sqrt(3.0) * a * a, 6.0 * a
+    assert abs(ob["mean_shape_index"] - 6.0 / math.sqrt(1.5 * math.sqrt(3.0))) < 1e-13
+    assert abs(ob["mean_shape_index"] - 3.7224194364083982) < 1e-13
+    assert abs(ob["area_variance"]) < 1e-13 and ob["n_nonpositive_area"] == 0
+    assert abs(ob["area_min"] - A) < 1e-13 and abs(ob["area_max"] - A) < 1e-13
+    assert abs(ob["energy"] - 24 * (1.3 * (A - 1.0) ** 2 + 0.7 * (P - 3.9) ** 2)) < 1e-11
+    t = w.config_tiling(1)
+    o = oracle.from_tiling(t, **w.config_params(1))
+    ob = o.observables()
+    L2 = t.Lx * t.Ly
+    assert abs(ob["sum_area"] - L2) <= 1e-12 * L2
+    ref = h.polygon_areas_numpy(t.pos, t.cell_vertex_num, t.cell_vertices, t.Lx, t.Ly)   # independent shoelace
+    assert abs(ob["area_variance"] - ref[:, 0].var()) < 1e-12
+    assert abs(ob["mean_shape_index"] - (ref[:, 1] / np.sqrt(ref[:, 0])).mean()) < 1e-12
+    assert 0.2 < ob["area_variance"] < 0.35        # Poisson-Voronoi: var(A) / <A>^2 ~ 0.28
