@@ -298,11 +298,13 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   s->step = params->step0;
   s->n_sorts = 0; s->launches = 0;
   // Two-launch schedule (flips inside the next force/move launch) pays when the sweep is longer
-  // than the flippers' chain of dependent loads (~15 us): from about a million vertices.  Smaller
-  // systems run the plain three-launch schedule.  AVM_B200_FUSED / AVM_B200_UNFUSED override.
+  // than the flippers' chain of dependent loads (~15 us): from about a million vertices; and for
+  // tiny systems, which flip rarely and are bound by the number of launches.  In between the plain
+  // three-launch schedule is faster.  AVM_B200_FUSED / AVM_B200_UNFUSED override.
   s->t1_passes = (params->flags & AVM_FLAG_T1_PASSES_MASK) >> AVM_FLAG_T1_PASSES_SHIFT;
   if (s->t1_passes < 1) s->t1_passes = 1;
-  s->fused = s->t1_passes == 1 && AVM_FUSED_T1 && (V >= (1 << 20) || getenv("AVM_B200_FUSED")) && !getenv("AVM_B200_UNFUSED");
+  s->fused = s->t1_passes == 1 && AVM_FUSED_T1 && (V >= (1 << 20) || V <= 2048 || getenv("AVM_B200_FUSED")) &&
+             !getenv("AVM_B200_UNFUSED");
 
   cudaStream_t st = s->stream;
   const cudaMemcpyKind kind = host_inputs ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
