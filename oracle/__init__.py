@@ -64,6 +64,7 @@ def _load() -> ctypes.CDLL:
         lib.oracle_compute_forces.argtypes = [p, p, p]
         lib.oracle_step.argtypes = [p, i64]
         lib.oracle_t1_pass.argtypes = [p]
+        lib.oracle_set_cell_targets.argtypes = [p, p, p]
         lib.oracle_debug_t1.argtypes = [p, p, p, p, p, i64]
         lib.oracle_get_state.argtypes = [p, p, p, p, p, p, p, ctypes.POINTER(OracleStats)]
         lib.oracle_set_positions.argtypes = [p, p]
@@ -156,6 +157,13 @@ class OracleSim:
 
     def step(self, n: int = 1) -> None:
         _load().oracle_step(self._h, n)
+
+    def set_cell_targets(self, A0=None, P0=None) -> None:
+        """per-cell preferred area / perimeter of Eq. 1 (user order); None, None = uniform again"""
+        a = None if A0 is None else np.ascontiguousarray(A0, dtype=np.float64)
+        b = None if P0 is None else np.ascontiguousarray(P0, dtype=np.float64)
+        if _load().oracle_set_cell_targets(self._h, _ptr(a), _ptr(b)) != 0:
+            raise ValueError("oracle_set_cell_targets: give both arrays or neither")
 
     def t1_pass(self) -> None:
         _load().oracle_t1_pass(self._h)

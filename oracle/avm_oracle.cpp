@@ -51,7 +51,11 @@ struct Sim {
   std::vector<int32_t> cv;      // [N][S]        cellVertices, counter-clockwise
   std::vector<int32_t> vn;      // [V][3]        vertexNeighbors
   std::vector<int32_t> vc;      // [V][3]        vertexCellNeighbors
+  std::vector<double> A0c, P0c; // [N] per-cell preferred values A_{0,i}, P_{0,i} of Eq. 1 (
+                                // NEXT-4); empty = the uniform A0, P0 of Eq. A1 (R17)
   Stats st;
+  double A0(int64_t c) const { return A0c.empty() ? p.A0 : A0c[c]; }
+  double P0(int64_t c) const { return P0c.empty() ? p.P0 : P0c[c]; }
 };
 
 // ------------------------------------------------------------------------------------------
@@ -130,11 +134,11 @@ void geometry(const Sim& s, std::vector<double>& AP) {
   for (int64_t c = 0; c < s.N; ++c) cell_geometry(s, c, AP[2 * c], AP[2 * c + 1]);
 }
 
-// Eq. 1 / A1: E = sum_i K_A (A_i - A0)^2 + K_P (P_i - P0)^2, no 1/2 (R4).
+// Eq. 1 / A1: E = sum_i K_A (A_i - A0_i)^2 + K_P (P_i - P0_i)^2, no 1/2 (R4).
 double energy(const Sim& s, const std::vector<double>& AP) {
   double E = 0.0;
   for (int64_t c = 0; c < s.N; ++c) {
-    double dA = AP[2 * c] - s.p.A0, dP = AP[2 * c + 1] - s.p.P0;
+    double dA = AP[2 * c] - s.A0(c), dP = AP[2 * c + 1] - s.P0(c);
     E += s.p.KA * dA * dA + s.p.KP * dP * dP;
   }
   return E;
@@ -168,7 +172,7 @@ void vertex_force(const Sim& s, const std::vector<double>& AP, int64_t v, double
     if (lp > 0.0) { upx = rpx / lp; upy = rpy / lp; }
     if (ln > 0.0) { unx = rnx / ln; uny = rny / ln; }
     const double dPx = -(upx + unx), dPy = -(upy + uny);
-    const double ca = 2.0 * s.p.KA * (AP[2 * c] - s.p.A0), cp = 2.0 * s.p.KP * (AP[2 * c + 1] - s.p.P0);
+    const double ca = 2.0 * s.p.KA * (AP[2 * c] - s.A0(c)), cp = 2.0 * s.p.KP * (AP[2 * c + 1] - s.P0(c));
     Fx -= ca * dAx + cp * dPx;
     Fy -= ca * dAy + cp * dPy;
   }
@@ -404,6 +408,14 @@ int oracle_step(oracle_sim* s, int64_t n_steps) {
 }
 
 // one T1 pass on the current state without moving anything else (test hook)
+// NEXT-4: per-cell preferred values of Eq. 1, user order; NULL, NULL = uniform again
+int oracle_set_cell_targets(oracle_sim* s, const double* A0, const double* P0) {
+  if (!s || ((A0 == nullptr) != (P0 == nullptr))) return -1;
+  s->A0c.clear(); s->P0c.clear();
+  if (A0) { s->A0c.assign(A0, A0 + s->N); s->P0c.assign(P0, P0 + s->N); }
+  return 0;
+}
+
 int oracle_t1_pass(oracle_sim* s) { t1_pass(*s); return 0; }
 
 // detect + resolve on the current state without flipping: sorted (tag_min, tag_max) pairs

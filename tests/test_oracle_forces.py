@@ -190,3 +190,61 @@ def test_observables_closed_forms_on_hexagons_and_voronoi():
     assert abs(ob["area_variance"] - ref[:, 0].var()) < 1e-12
     assert abs(ob["mean_shape_index"] - (ref[:, 1] / np.sqrt(ref[:, 0])).mean()) < 1e-12
     assert 0.2 < ob["area_variance"] < 0.35        # Poisson-Voronoi: var(A) / <A>^2 ~ 0.28
+
+
+# ---- NEXT-4: per-cell preferred values A_{0,i}, P_{0,i} of Eq. 1 ----
+
+def test_per_cell_targets_match_finite_differences_of_eq1():
+    """heterogeneous A0_i, P0_i: F = -dE/dh against central differences of Eq. 1, whose energy
+    is written out here with numpy from the oracle's geometry"""
+    t = w.voronoi_tiling(64, 8.0, 5)
+    rng = np.random.default_rng(0)
+    A0 = rng.uniform(0.6, 1.4, t.N)
+    P0 = rng.uniform(3.2, 4.2, t.N)
+    sim = oracle.from_tiling(t, **PARAMS)
+    sim.set_cell_targets(A0, P0)
+    F, ap0 = sim.compute_forces()
+    assert abs(sim.energy() - np.sum(PARAMS["KA"] * (ap0[:, 0] - A0) ** 2 + PARAMS["KP"] * (ap0[:, 1] - P0) ** 2)) < 1e-10
+    rms = np.sqrt((F ** 2).sum(axis=1).mean())
+    worst = 0.0
+    for v in range(0, t.V, 3):
+        cells = t.vertex_cell_neighbors[v]
+        dn = t.pos[t.vertex_neighbors[v]] - t.pos[v]
+        lmin = np.hypot(h.min_image(dn[:, 0], t.Lx), h.min_image(dn[:, 1], t.Ly)).min()
+        delta = min(1e-5, 1e-2 * lmin)
+        g = np.zeros(2)
+        for ax in range(2):
+            e = {}
+            for m in (-2, -1, 1, 2):
+                pos = t.pos.copy()
+                pos[v, ax] += m * delta
+                pos[v, ax] %= (t.Lx, t.Ly)[ax]
+                sim.set_positions(pos)
+                ap = sim.geometry()
+                e[m] = np.sum(PARAMS["KA"] * (ap[cells, 0] - A0[cells]) ** 2 + PARAMS["KP"] * (ap[cells, 1] - P0[cells]) ** 2)
+            g[ax] = (8 * (e[1] - e[-1]) - (e[2] - e[-2])) / (12 * delta)
+        worst = max(worst, np.linalg.norm(F[v] + g) / max(np.linalg.norm(F[v]), rms))
+    assert worst < 1e-6, worst
+    # translation invariance survives heterogeneity
+    sim.set_positions(t.pos)
+    assert np.abs(sim.compute_forces()[0].sum(axis=0)).max() < 1e-10
+
+
+def test_per_cell_targets_special_cases():
+    """(i) arrays filled with the uniform values reproduce the uniform path bit for bit; (ii) with
+    each cell's targets set to its own area and perimeter every force vanishes and E = 0;
+    (iii) NULL, NULL restores the uniform values."""
+    t = w.config_tiling(0)
+    p = w.config_params(0)
+    a = oracle.from_tiling(t, **p)
+    b = oracle.from_tiling(t, **p)
+    b.set_cell_targets(np.full(t.N, p["A0"]), np.full(t.N, p["P0"]))
+    a.step(30)
+    b.step(30)
+    assert np.array_equal(a.get_state()["pos"], b.get_state()["pos"])
+    c = oracle.from_tiling(t, **p)
+    ap = c.geometry()
+    c.set_cell_targets(ap[:, 0], ap[:, 1])
+    assert np.abs(c.compute_forces()[0]).max() == 0.0 and c.energy() == 0.0
+    c.set_cell_targets(None, None)
+    assert np.array_equal(c.compute_forces()[0], oracle.from_tiling(t, **p).compute_forces()[0])
