@@ -137,6 +137,12 @@ int avm_compute_forces_host(avm_sim* sim, double* force_xy, double* area_perim);
  * fixed order (deterministic).  energy is a HOST pointer; synchronises the stream. */
 int avm_energy(avm_sim* sim, double* energy);
 
+/* Per-cell preferred area and perimeter A_{0,i}, P_{0,i} of Eq. 1 (SURVEY.md
+ * section 8(f), NEXT-4) instead of the uniform A0, P0 of Eq. A1.  area0, perimeter0: DEVICE
+ * pointers, [N] each, user order, copied; both NULL restores the uniform values of avm_params.
+ * Asynchronous.  The values are not part of avm_get_state: a resumed run sets them again. */
+int avm_set_cell_targets(avm_sim* sim, const double* area0, const double* perimeter0);
+
 /* Observables of the current state, reduced on the device in a
  * fixed order (deterministic): the energy of Eq. 1, the area and perimeter totals, the mean shape
  * index <P / sqrt(A)> over the cells with A > 0 (the order parameter of the rigidity transition

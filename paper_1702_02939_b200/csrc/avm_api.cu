@@ -42,10 +42,11 @@ struct BufferSet {
   int4* cv;
   double* theta;
   CellRec* rec;
+  double2* tgt;
 };
 
 struct Layout {
-  size_t pos[2], vn[2], vc[2], cv[2], cvn[2], theta[2], rec[2], vtag[2], ctag[2];
+  size_t pos[2], vn[2], vc[2], cv[2], cvn[2], theta[2], rec[2], tgt[2], vtag[2], ctag[2];
   size_t minkey, cand, ctr, dirty, estamp, ap, epart, key[2], val[2], hist, newidx_v, newidx_c, order_v, order_c;
   size_t total;
 };
@@ -59,7 +60,7 @@ Layout make_layout(const avm_params& p) {
   for (int i = 0; i < 2; ++i) L.pos[i] = take(16 * V);
   for (int i = 0; i < 2; ++i) {
     L.vn[i] = take(12 * Vs); L.vc[i] = take(12 * Vs); L.cv[i] = take(4 * N * S); L.cvn[i] = take(4 * N);
-    L.theta[i] = take(8 * N); L.rec[i] = take(32 * N); L.vtag[i] = take(4 * V); L.ctag[i] = take(4 * N);
+    L.theta[i] = take(8 * N); L.rec[i] = take(32 * N); L.tgt[i] = take(16 * N); L.vtag[i] = take(4 * V); L.ctag[i] = take(4 * N);
   }
   L.minkey = take(8 * N);
   L.cand = take(sizeof(Cand) * 3 * N);
@@ -114,7 +115,7 @@ struct avm_sim {
     Dev d;
     d.pos = pos[cur_pos]; d.pos_next = pos[1 - cur_pos];
     const BufferSet& b = set[cur_set];
-    d.vn = b.vn; d.vc = b.vc; d.cv = b.cv; d.cvn = b.cvn; d.theta = b.theta; d.rec = b.rec;
+    d.vn = b.vn; d.vc = b.vc; d.cv = b.cv; d.cvn = b.cvn; d.theta = b.theta; d.rec = b.rec; d.tgt = b.tgt;
     d.vtag = b.vtag; d.ctag = b.ctag;
     d.minkey = minkey; d.cand = cand; d.ctr = ctr; d.dirty = dirty; d.estamp = estamp;
     return d;
@@ -123,7 +124,7 @@ struct avm_sim {
     Dev d = dev();
     const BufferSet& b = set[1 - cur_set];
     d.pos = pos[1 - cur_pos]; d.pos_next = pos[cur_pos];
-    d.vn = b.vn; d.vc = b.vc; d.cv = b.cv; d.cvn = b.cvn; d.theta = b.theta; d.rec = b.rec;
+    d.vn = b.vn; d.vc = b.vc; d.cv = b.cv; d.cvn = b.cvn; d.theta = b.theta; d.rec = b.rec; d.tgt = b.tgt;
     d.vtag = b.vtag; d.ctag = b.ctag;
     return d;
   }
@@ -204,6 +205,12 @@ __global__ void export_cells_kernel(const Dev d, const Consts k, int* cvn, int* 
   if (cv)
     for (int j = 0; j < k.S; ++j) cv[(size_t)t * k.S + j] = j < n ? d.vtag[row_entry(d.cv, k.N, c, j)] : -1;
 }
+__global__ void import_targets_kernel(const Dev d, const Consts k, const double* __restrict__ A0, const double* __restrict__ P0) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= k.N) return;
+  const int t = d.ctag[c];
+  d.tgt[c] = make_double2(A0[t], P0[t]);
+}
 __global__ void import_positions_kernel(const Dev d, const Consts k, const double* pos) {
   const int v = blockIdx.x * blockDim.x + threadIdx.x;
   if (v >= k.V) return;
@@ -272,6 +279,7 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   k.amp = sqrt(2.0 * params->Dr * params->dt);
   k.lc = params->l_c; k.lc2 = params->l_c * params->l_c;
   k.seed = params->seed;
+  k.per_cell = 0;
   k.cap_a = ((params->flags & AVM_FLAG_T1_PASSES_MASK) >> AVM_FLAG_T1_PASSES_SHIFT) > 1 ? N : 3 * N;
   for (int r = 0; r < 10; ++r) k.rkey[r] = philox_round_key(params->seed, r);
   char* w = s->ws;
@@ -279,7 +287,7 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
     s->pos[i] = (double2*)(w + L.pos[i]);
     BufferSet& b = s->set[i];
     b.vn = (int*)(w + L.vn[i]); b.vc = (int*)(w + L.vc[i]); b.cv = (int4*)(w + L.cv[i]);
-    b.cvn = (int*)(w + L.cvn[i]); b.theta = (double*)(w + L.theta[i]); b.rec = (CellRec*)(w + L.rec[i]);
+    b.cvn = (int*)(w + L.cvn[i]); b.theta = (double*)(w + L.theta[i]); b.rec = (CellRec*)(w + L.rec[i]); b.tgt = (double2*)(w + L.tgt[i]);
     b.vtag = (int*)(w + L.vtag[i]); b.ctag = (int*)(w + L.ctag[i]);
     s->sc.key[i] = (unsigned int*)(w + L.key[i]); s->sc.val[i] = (int*)(w + L.val[i]);
   }
@@ -581,6 +589,16 @@ int avm_set_positions(avm_sim* s, const double* pos_xy) {
   import_positions_kernel<<<cdiv(s->k.V, 256), 256, 0, s->stream>>>(d, s->k, pos_xy);
   ++s->launches;
   s->launches += launch_refresh_cells(d, s->k, s->stream);
+  AVM_CUDA(cudaPeekAtLastError());
+  return AVM_OK;
+}
+
+int avm_set_cell_targets(avm_sim* s, const double* area0, const double* perimeter0) {
+  if (!s || ((area0 == nullptr) != (perimeter0 == nullptr))) return AVM_EINVAL;
+  s->k.per_cell = area0 ? 1 : 0;
+  const Dev d = s->dev();
+  if (area0) { import_targets_kernel<<<cdiv(s->k.N, 256), 256, 0, s->stream>>>(d, s->k, area0, perimeter0); ++s->launches; }
+  s->launches += launch_refresh_cells(d, s->k, s->stream);   // the cached records hold (A - A0_i), (P - P0_i)
   AVM_CUDA(cudaPeekAtLastError());
   return AVM_OK;
 }

@@ -49,6 +49,7 @@ struct Consts {
   double v0_3, mu, dt;       // v0_3 = v0 / 3 (Eq. 4 with n = 3, R5)
   double amp;                // sqrt(2 Dr dt) (R8)
   double lc, lc2;
+  int per_cell;              // 1: preferred values A0_i, P0_i per cell (Dev::tgt, Eq. 1), 0: uniform A0, P0 (Eq. A1)
   int cap_a;                 // capacity of the step's candidate list (3N, or N when repeated passes use the rest)
   unsigned long long seed;
   uint2 rkey[10];            // Philox round keys of `seed` (the key schedule is uniform: done once on the host)
@@ -76,6 +77,7 @@ struct Dev {
   unsigned long long* minkey;  // [N] per-cell minimum candidate key, ~0 when idle
   Cand* cand;         // [3N]
   unsigned int* dirty; // [ceil(V/32)] bit v: vertex v belongs to a cell of some pending T1 candidate
+  double2* tgt;       // [N] (A0_i, P0_i), internal order; read only when Consts::per_cell (NEXT-4)
   unsigned int* estamp; // [3*Vs] per directed half-edge (slot plane, owner vertex): id of the repeated pass that tested it last
   Counters* ctr;
 };
@@ -101,6 +103,11 @@ __device__ __forceinline__ int& row_entry(int4* cv, int N, int c, int j) {
 }
 __device__ __forceinline__ int row_entry(const int4* cv, int N, int c, int j) {
   return reinterpret_cast<const int*>(cv + (size_t)(j >> 2) * N + c)[j & 3];
+}
+
+// preferred (area, perimeter) of cell c: Eq. 1 per cell or the uniform pair of Eq. A1
+__device__ __forceinline__ double2 cell_targets(const Dev& d, const Consts& k, int c) {
+  return k.per_cell ? d.tgt[c] : make_double2(k.A0, k.P0);
 }
 
 // Square roots of squared lengths.  Every squared length in this library is formed as

@@ -514,8 +514,9 @@ cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts
   }
   if (!valid) return;
   CellRec r;
-  r.a = k.KA2 * (__dmul_rn(0.5, acc) - k.A0);
-  r.p = k.KP2 * (per - k.P0);
+  const double2 tg = cell_targets(d, k, c);
+  r.a = k.KA2 * (__dmul_rn(0.5, acc) - tg.x);
+  r.p = k.KP2 * (per - tg.y);
   r.nx = cs; r.ny = sn;
   st_rec(d.rec + c, r);
   smask &= n >= 32 ? ~0u : (1u << n) - 1u;     // edges beyond the closing one are padding
@@ -722,8 +723,9 @@ __device__ __noinline__ bool t1_try_flip(const Dev& d, const Consts& k, const Ca
     if (lane == t) { myA = __dmul_rn(0.5, acc[t]); myP = per[t]; }
   if (lane < 4) {
     const int cc = cells[lane == 0 ? 0 : lane == 1 ? 1 : lane == 2 ? 2 : 3];
-    d.rec[cc].a = k.KA2 * (myA - k.A0);
-    d.rec[cc].p = k.KP2 * (myP - k.P0);
+    const double2 tg = cell_targets(d, k, cc);
+    d.rec[cc].a = k.KA2 * (myA - tg.x);
+    d.rec[cc].p = k.KP2 * (myP - tg.y);
   }
   __syncwarp();
   return true;
@@ -809,8 +811,9 @@ __global__ void forces_kernel(const Dev d, const Consts k, const double2* __rest
 #pragma unroll
   for (int s = 0; s < 3; ++s) {
     q[s] = d.pos[d.vn[s * k.Vs + v]];
-    const double2 a = ap[d.vc[s * k.Vs + v]];
-    c[s].a = k.KA2 * (a.x - k.A0); c[s].p = k.KP2 * (a.y - k.P0); c[s].nx = 0.0; c[s].ny = 0.0;
+    const int cell = d.vc[s * k.Vs + v];
+    const double2 a = ap[cell], tg = cell_targets(d, k, cell);
+    c[s].a = k.KA2 * (a.x - tg.x); c[s].p = k.KP2 * (a.y - tg.y); c[s].nx = 0.0; c[s].ny = 0.0;
   }
   const double2 f = vertex_force(h, q[0], q[1], q[2], c[0], c[1], c[2], k);
   const int t = d.vtag[v];
@@ -844,7 +847,8 @@ observables_partial_kernel(const Dev d, const Consts k, double* __restrict__ par
   for (int c = blockIdx.x * 256 + threadIdx.x; c < k.N; c += gridDim.x * 256) {
     double A, P;
     cell_area_perimeter(d.pos, d.cv, c, d.cvn[c], k, A, P);
-    x[0] += k.KA * (A - k.A0) * (A - k.A0) + k.KP * (P - k.P0) * (P - k.P0);
+    const double2 tg = cell_targets(d, k, c);
+    x[0] += k.KA * (A - tg.x) * (A - tg.x) + k.KP * (P - tg.y) * (P - tg.y);
     x[1] += A; x[2] += P;
     if (A > 0.0) x[3] += P / sqrt(A); else x[4] += 1.0;
     x[5] += A * A;

@@ -500,3 +500,36 @@ def test_observables_match_the_oracle(B, k, steps):
         assert a["step"] == o.get_state()["stats"]["step"] and a["t1_flips"] == o.get_state()["stats"]["t1_flips"]
         assert abs(a["energy"] - g.energy()) == 0.0
     assert abs(a["sum_area"] - t.Lx * t.Ly) <= 1e-12 * t.Lx * t.Ly
+
+
+@pytest.mark.parametrize("k,steps,sort_every", [(0, 60, 0), (1, 24, 7)])
+def test_per_cell_targets_match_the_oracle(B, k, steps, sort_every):
+    """NEXT-4: per-cell preferred area and perimeter of Eq. 1 (a bidisperse mixture): forces within
+    1e-10, trajectory within 1e-8 with bit-exact topology (re-sorts included), energy, and
+    NULL, NULL restoring the uniform path."""
+    t = tiling(k)
+    p = w.config_params(k)
+    rng = np.random.default_rng(11)
+    big = rng.random(t.N) < 0.5
+    A0 = np.where(big, 1.25, 0.75)
+    P0 = np.where(big, 3.9 * np.sqrt(1.25), 3.7 * np.sqrt(0.75))
+    g = B.from_tiling(t, **dict(p, sort_every=sort_every, sort_at_create=True))
+    o = oracle.from_tiling(t, **p)
+    g.set_cell_targets(A0, P0)
+    o.set_cell_targets(A0, P0)
+    F, ap = g.compute_forces()
+    Fo, apo = o.compute_forces()
+    assert_forces_close(F.cpu().numpy(), Fo, ap.cpu().numpy(), apo)
+    assert abs(g.energy() - o.energy()) <= 1e-10 * abs(o.energy())
+    g.step(steps)
+    o.step(steps)
+    assert_states_match(to_np(g.get_state()), o.get_state(), t.Lx, t.Ly)
+    assert abs(g.energy() - o.energy()) <= 1e-8 * abs(o.energy())
+    uni = oracle.from_tiling(t, **p)
+    uni.step(steps)
+    assert np.abs(uni.get_state()["pos"] - o.get_state()["pos"]).max() > 1e-3      # the targets matter
+    g.set_cell_targets(None, None)
+    o.set_cell_targets(None, None)
+    F, ap = g.compute_forces()
+    Fo, apo = o.compute_forces()
+    assert_forces_close(F.cpu().numpy(), Fo, ap.cpu().numpy(), apo)
