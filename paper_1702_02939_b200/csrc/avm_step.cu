@@ -434,7 +434,7 @@ __device__ __noinline__ void t1_report_cell(const Dev& d, const Consts& k, int c
 // Cells are walked in DESCENDING index order while force_move walks vertices in ascending order,
 // so each pass starts on the lines the previous pass touched last (L2 recency).
 // ---------------------------------------------------------------------------------------------
-template <bool kStep>
+template <bool kStep, bool kPerCell>
 __global__ void __launch_bounds__(kCellBlock, AVM_CU_MINB)
 cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, const unsigned long long step,
                    const unsigned parity) {
@@ -514,7 +514,7 @@ cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts
   }
   if (!valid) return;
   CellRec r;
-  const double2 tg = cell_targets(d, k, c);
+  const double2 tg = kPerCell ? d.tgt[c] : make_double2(k.A0, k.P0);   // Eq. 1 per cell (NEXT-4) / Eq. A1
   r.a = k.KA2 * (__dmul_rn(0.5, acc) - tg.x);
   r.p = k.KP2 * (per - tg.y);
   r.nx = cs; r.ny = sn;
@@ -935,7 +935,8 @@ int launch_step(const Dev& d, const Consts& k, unsigned long long step, cudaStre
   if (ev) cudaEventRecord(ev[1], s);
   Dev m = d;                      // from here on the moved positions are "the" positions
   m.pos = d.pos_next; m.pos_next = d.pos;
-  launch_chained(cell_update_kernel<true>, cdiv(k.N, kCellBlock), kCellBlock, s, pdl, false, m, k, step, parity);
+  if (k.per_cell) launch_chained(cell_update_kernel<true, true>, cdiv(k.N, kCellBlock), kCellBlock, s, pdl, false, m, k, step, parity);
+  else launch_chained(cell_update_kernel<true, false>, cdiv(k.N, kCellBlock), kCellBlock, s, pdl, false, m, k, step, parity);
   if (ev) cudaEventRecord(ev[2], s);
   if (!fused) launch_chained(t1_flip_kernel, kT1Grid, kT1Block, s, pdl, false, m, k, parity, true);
   if (ev) cudaEventRecord(ev[3], s);
@@ -950,7 +951,8 @@ int launch_t1_flush(const Dev& d, const Consts& k, unsigned long long last_step,
 }
 
 int launch_refresh_cells(const Dev& d, const Consts& k, cudaStream_t s) {
-  cell_update_kernel<false><<<cdiv(k.N, kCellBlock), kCellBlock, 0, s>>>(d, k, 0ull, 0u);
+  if (k.per_cell) cell_update_kernel<false, true><<<cdiv(k.N, kCellBlock), kCellBlock, 0, s>>>(d, k, 0ull, 0u);
+  else cell_update_kernel<false, false><<<cdiv(k.N, kCellBlock), kCellBlock, 0, s>>>(d, k, 0ull, 0u);
   return 1;
 }
 
