@@ -313,6 +313,7 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   if (s->t1_passes < 1) s->t1_passes = 1;
   s->fused = s->t1_passes == 1 && AVM_FUSED_T1 && (V >= (1 << 20) || V <= 2048 || getenv("AVM_B200_FUSED")) &&
              !getenv("AVM_B200_UNFUSED");
+  k.flag_dirty = s->fused ? 1 : 0;
 
   cudaStream_t st = s->stream;
   const cudaMemcpyKind kind = host_inputs ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
@@ -431,7 +432,10 @@ int avm_step(avm_sim* s, int64_t n_steps) {
     int n = -1;
     if (s->fused) {
       n = launch_step(s->dev(), s->k, s->step, s->stream, nullptr, true);
-      if (n < 0) s->fused = false; else pending = true;
+      if (n < 0) {   // the launch was refused: complete the previous step, then go on with three launches per step
+        if (pending) { s->launches += launch_t1_flush(s->dev(), s->k, s->step - 1, s->stream); pending = false; }
+        s->fused = false; s->k.flag_dirty = 0;
+      } else pending = true;
     }
     if (n < 0) n = launch_step(s->dev(), s->k, s->step, s->stream, nullptr, false);
     s->launches += n;
@@ -460,7 +464,10 @@ int avm_step_profile(avm_sim* s, int64_t n_steps, double* ms_per_kernel) {
     int n = -1;
     if (s->fused) {
       n = launch_step(s->dev(), s->k, s->step, s->stream, ev, true);
-      if (n < 0) s->fused = false; else pending = true;
+      if (n < 0) {   // the launch was refused: complete the previous step, then go on with three launches per step
+        if (pending) { s->launches += launch_t1_flush(s->dev(), s->k, s->step - 1, s->stream); pending = false; }
+        s->fused = false; s->k.flag_dirty = 0;
+      } else pending = true;
     }
     if (n < 0) n = launch_step(s->dev(), s->k, s->step, s->stream, ev, false);
     s->launches += n;

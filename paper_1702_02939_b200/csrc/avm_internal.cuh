@@ -49,6 +49,7 @@ struct Consts {
   double v0_3, mu, dt;       // v0_3 = v0 / 3 (Eq. 4 with n = 3, R5)
   double amp;                // sqrt(2 Dr dt) (R8)
   double lc, lc2;
+  int flag_dirty;            // 1: the marking thread flags the vertices of a candidate's cells (two-launch schedule only)
   int per_cell;              // 1: preferred values A0_i, P0_i per cell (Dev::tgt, Eq. 1), 0: uniform A0, P0 (Eq. A1)
   int cap_a;                 // capacity of the step's candidate list (3N, or N when repeated passes use the rest)
   unsigned long long seed;

@@ -391,7 +391,7 @@ __device__ __noinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va,
   // Everything a flip of this edge would write, and everything that reads it in the next
   // force/move pass, belongs to a vertex of these four cells: flag them, so that force_move can
   // run the flips while the untouched vertices already move.
-  if (count_stats) {
+  if (count_stats && k.flag_dirty) {
 #pragma unroll
     for (int t = 0; t < 4; ++t) {
       const int e[8] = {q[t][0].x, q[t][0].y, q[t][0].z, q[t][0].w, q[t][1].x, q[t][1].y, q[t][1].z, q[t][1].w};
