@@ -74,7 +74,9 @@ enum {
 };
 
 /* Counters since creation.  error is a sticky bit set: 1 = a non-finite position was produced,
- * 2 = a flip was suppressed because a cell row would exceed S. */
+ * 2 = a flip was suppressed because a cell row would exceed S, 4 = the lists given to avm_create
+ * are out of range or inconsistent (avm_create then fails with AVM_EINCONSISTENT), 8 = a T1
+ * candidate list overflowed its capacity (cannot happen for a valid tiling). */
 typedef struct avm_stats {
   int64_t step;             /* current step counter (step0 + steps taken)                       */
   int64_t t1_short;         /* edges found shorter than l_c                                      */
