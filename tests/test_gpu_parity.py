@@ -533,3 +533,37 @@ def test_per_cell_targets_match_the_oracle(B, k, steps, sort_every):
     F, ap = g.compute_forces()
     Fo, apo = o.compute_forces()
     assert_forces_close(F.cpu().numpy(), Fo, ap.cpu().numpy(), apo)
+
+
+@pytest.mark.parametrize("S", [20, 32])
+@pytest.mark.parametrize("fused", [False, True])
+def test_other_row_strides_match_the_oracle(B, S, fused, monkeypatch):
+    """rows longer than 16 entries use different code (one row per pass in the flippers, planes
+    4..7 of the padded rows, bit 31 of the short-edge mask): configs[1] geometry with S = 20 and
+    the maximum S = 32, in both schedules, through the step-0 burst."""
+    monkeypatch.setenv("AVM_B200_FUSED" if fused else "AVM_B200_UNFUSED", "1")
+    t = w.voronoi_tiling(4096, 64.0, 2, S=S)
+    p = w.config_params(1)
+    g = B.from_tiling(t, **dict(p, sort_every=6, sort_at_create=True))
+    o = oracle.from_tiling(t, **p)
+    F, ap = g.compute_forces()
+    Fo, apo = o.compute_forces()
+    assert_forces_close(F.cpu().numpy(), Fo, ap.cpu().numpy(), apo)
+    g.step(25)
+    o.step(25)
+    assert_states_match(to_np(g.get_state()), o.get_state(), t.Lx, t.Ly)
+    assert o.get_state()["stats"]["t1_flips"] > 300
+
+
+def test_smallest_tori(B):
+    """the smallest tilings the generator builds with valid minimum-image unwrapping (3 x 4 and
+    4 x 4 hexagons: N = 12 and 16, a single CTA, more flipper warps than candidates), many steps
+    with strong noise and a large threshold so that flips keep happening"""
+    for nx, ny in ((3, 4), (4, 4)):
+        t = w.hex_tiling(nx, ny, a=1.0)
+        p = dict(KA=1.0, KP=1.0, A0=2.0, P0=6.5, v0=0.4, Dr=1.0, dt=0.01, l_c=0.3, seed=3)
+        g = B.from_tiling(t, **p)
+        o = oracle.from_tiling(t, **p)
+        g.step(200)
+        o.step(200)
+        assert_states_match(to_np(g.get_state()), o.get_state(), t.Lx, t.Ly, pos_tol=1e-7)
