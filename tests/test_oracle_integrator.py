@@ -99,3 +99,74 @@ def test_resume_is_bit_identical():
     sa, sc = a.get_state(), c.get_state()
     for k in ("pos", "theta", "cell_vertices", "vertex_neighbors", "vertex_cell_neighbors", "cell_vertex_num"):
         assert np.array_equal(sa[k], sc[k]), k
+
+
+def test_vertices_move_with_start_of_step_directors():
+    """R7 (PAPER.md:104 "first move the vertices and then update the cell directors"; Eq. 4, :56):
+    with K_A = K_P = 0, v0 > 0 and Dr > 0 the displacement of a step is dt*v0/3 * sum n(theta) with
+    theta taken at the START of that step, and the next step uses the rotated directors
+    theta1 = theta0 + sqrt(2 Dr dt) xi(seed, 0, c).  A swapped move/rotate order fails both halves."""
+    t = w.config_tiling(0)
+    v0, dt, Dr, seed = 0.7, 0.01, 2.0, 11
+    sim = oracle.from_tiling(t, KA=0.0, KP=0.0, v0=v0, Dr=Dr, dt=dt, l_c=0.0, seed=seed)
+    th0 = t.theta
+    th1 = th0 + np.sqrt(2 * Dr * dt) * oracle.director_noise(seed, 0, 0, t.N)
+    vc = t.vertex_cell_neighbors
+
+    def drift(th):
+        n = np.stack([np.cos(th), np.sin(th)], axis=1)
+        return dt * v0 / 3.0 * n[vc].sum(axis=1)
+
+    def mi_diff(a, b):
+        d = a - b
+        return np.stack([h.min_image(d[:, 0], t.Lx), h.min_image(d[:, 1], t.Ly)], axis=1)
+
+    sim.step(1)
+    s1 = sim.get_state()
+    assert np.abs(mi_diff(s1["pos"], t.pos) - drift(th0)).max() < 1e-14
+    assert np.abs(drift(th1) - drift(th0)).max() > 1e-4           # the two readings are far apart
+    assert np.abs(mi_diff(s1["pos"], t.pos) - drift(th1)).max() > 1e-4
+    assert np.array_equal(s1["theta"], th1)
+    sim.step(1)
+    s2 = sim.get_state()
+    assert np.abs(mi_diff(s2["pos"], s1["pos"]) - drift(th1)).max() < 1e-14
+    th2 = th1 + np.sqrt(2 * Dr * dt) * oracle.director_noise(seed, 1, 0, t.N)
+    assert np.abs(mi_diff(s2["pos"], s1["pos"]) - drift(th2)).max() > 1e-4
+
+
+def test_topology_is_tested_on_the_moved_positions():
+    """R6 ("with the forces in hand the degrees of freedom can be displaced ...
+    the next challenge is determining whether the cellular topology needs to be updated"; :104-108):
+    an edge that is longer than l_c at the start of the step and is brought below l_c by that
+    step's move flips in that very step; with the T1 pass before the move it would not."""
+    from tests.test_oracle_t1 import edge_cells_from_rows, shrink_edge
+    l_c, dt, v0 = 0.04, 0.01, 0.9
+    t = w.hex_tiling(6, 4, a=1.0)
+    v1 = 7
+    v2 = int(t.vertex_neighbors[v1, 1])
+    lo, hi = min(v1, v2), max(v1, v2)
+    L, R, E1, E2 = edge_cells_from_rows(t.cell_vertex_num, t.cell_vertices, t.vertex_cell_neighbors, lo, hi)
+    closing = dt * 2.0 * v0 / 3.0            # the end cells' directors point at each other along the edge
+    start_len = l_c + 0.5 * closing
+    pos, m, u = shrink_edge(t, lo, hi, start_len)
+    theta = np.zeros(t.N)
+    theta[E1] = np.arctan2(u[1], u[0])        # E1 holds lo: push lo towards hi
+    theta[E2] = np.arctan2(-u[1], -u[0])      # E2 holds hi: push hi towards lo
+    theta[L] = theta[R] = 0.3                 # shared by both endpoints: no relative motion
+    tt = w.Tiling(t.Lx, t.Ly, t.S, pos, t.cell_vertex_num, t.cell_vertices, t.vertex_neighbors,
+                  t.vertex_cell_neighbors, theta)
+    sim = oracle.from_tiling(tt, KA=0.0, KP=0.0, v0=v0, Dr=0.0, dt=dt, l_c=l_c)
+    cand, _ = sim.debug_t1()
+    assert len(cand) == 0                     # nothing is short before the move
+    sim.step(1)
+    s = sim.get_state()
+    assert s["stats"]["t1_short"] == 1 and s["stats"]["t1_flips"] == 1
+    assert h.cells_adjacent(s["cell_vertices"], s["cell_vertex_num"], E1, E2)
+    d = s["pos"][hi] - s["pos"][lo]
+    assert abs(np.hypot(h.min_image(d[0], t.Lx), h.min_image(d[1], t.Ly)) - 1.5 * l_c) < 1e-14
+    # the length the pass saw was start_len - closing < l_c: one more identical system, T1 off
+    ref = oracle.from_tiling(tt, KA=0.0, KP=0.0, v0=v0, Dr=0.0, dt=dt, l_c=0.0)
+    ref.step(1)
+    r = ref.get_state()["pos"]
+    d = r[hi] - r[lo]
+    assert abs(np.hypot(h.min_image(d[0], t.Lx), h.min_image(d[1], t.Ly)) - (start_len - closing)) < 1e-13
