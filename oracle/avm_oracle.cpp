@@ -188,7 +188,9 @@ struct Cand {
 };
 
 // Short edges, eligibility (R10), in ascending key order (v1, v2).
-void t1_candidates(Sim& s, std::vector<Cand>& cands, bool count) {
+// count: the pass adds to the t1_short / overflow_rejects statistics; raise: it may set the sticky
+// error bit (the debug hook does neither)
+void t1_candidates(Sim& s, std::vector<Cand>& cands, bool count, bool raise) {
   cands.clear();
   const double lc = s.p.l_c;
   for (int32_t v = 0; v < (int32_t)s.V; ++v) {
@@ -220,7 +222,11 @@ void t1_candidates(Sim& s, std::vector<Cand>& cands, bool count) {
       if (!distinct) continue;
       if (!(s.cvn[c.cL] > 3 && s.cvn[c.cR] > 3)) continue;          // no 2-gons; T2 not implemented
       if (!(s.cvn[c.cE1] < s.S && s.cvn[c.cE2] < s.S)) {            // row would exceed the stride
-        if (count) { ++s.st.overflow_rejects; s.st.error |= 2; }
+        // error bit 2 = "a flip was suppressed because a row would exceed S": raised whenever a
+        // pass sees it (a repeated pass can be the first to see it, when an earlier pass of the
+        // same step filled the end cell); the counter is a statistic of the step's first pass
+        if (count) ++s.st.overflow_rejects;
+        if (raise) s.st.error |= 2;
         continue;
       }
       cands.push_back(c);
@@ -298,12 +304,14 @@ void t1_flip(Sim& s, const Cand& c) {
 }
 
 // returns the number of candidates of the pass (0 = the topology is at a fixed point of the rule)
-// count_detect: whether this pass adds to the t1_short / overflow_rejects counters (the first pass
-// of a step does; repeated passes re-see the same ineligible edges and do not count them again)
+// count_detect: whether this pass adds to the t1_short / overflow_rejects counters.  Reading
+// (DESIGN.md section 9): both are statistics of the detection on the moved positions, i.e. of the
+// step's first pass; repeated passes re-see the same short-but-ineligible edges and
+// would count them once per pass.  The sticky error bit 2 is not a statistic: any pass raises it.
 size_t t1_pass(Sim& s, bool count_detect = true) {
   std::vector<Cand> cands;
   std::vector<char> win;
-  t1_candidates(s, cands, count_detect);
+  t1_candidates(s, cands, count_detect, true);
   t1_winners(s, cands, win);
   s.st.t1_candidates += (int64_t)cands.size();
   for (size_t i = 0; i < cands.size(); ++i) {
@@ -423,7 +431,7 @@ int oracle_debug_t1(oracle_sim* s, int32_t* cand_pairs, int64_t* n_cand, int32_t
                     int64_t* n_win, int64_t capacity) {
   std::vector<Cand> cands;
   std::vector<char> win;
-  t1_candidates(*s, cands, false);
+  t1_candidates(*s, cands, false, false);
   t1_winners(*s, cands, win);
   int64_t nc = 0, nw = 0;
   for (size_t i = 0; i < cands.size(); ++i) {

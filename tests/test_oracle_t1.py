@@ -331,3 +331,66 @@ def test_one_pass_is_the_default_and_equals_max_passes_one():
     b.step(40)
     sa, sb = a.get_state(), b.get_state()
     assert np.array_equal(sa["pos"], sb["pos"]) and np.array_equal(sa["cell_vertices"], sb["cell_vertices"])
+
+
+def pointing_edges(state, E):
+    """edges (u, w) that have cell E as an END cell: u runs over E's row, w is u's neighbour outside E
+    (slot convention R12: with vc[u][k] == E the row neighbours are vn[u][k], vn[u][k+1])"""
+    vn, vc = state["vertex_neighbors"], state["vertex_cell_neighbors"]
+    out = []
+    for u in state["cell_vertices"][E, :state["cell_vertex_num"][E]]:
+        k = vc[u].tolist().index(E)
+        out.append((int(u), int(vn[u][(k + 2) % 3])))
+    return out
+
+
+def overflow_on_a_later_pass_case(l_c=0.04):
+    """Hexagons with S = 8.  Cell E first gains a vertex (7 = S - 1); then two edges that both have E
+    as an end cell are short: they conflict through E, the smaller key flips in pass 1 (E reaches
+    S), and the other one is short, otherwise eligible, and rejected for overflow in pass 2."""
+    t = w.hex_tiling(6, 4, a=1.0, S=8)
+    E = 9
+    kw = dict(l_c=l_c, KA=0.0, KP=0.0, v0=0.0, Dr=0.0, dt=0.01)
+    sim = oracle.from_tiling(t, **kw)
+    e0 = pointing_edges(sim.get_state(), E)[2]
+    pos, _, _ = shrink_edge(t, min(e0), max(e0), 0.5 * l_c)
+    sim.set_positions(pos)
+    sim.t1_pass()
+    s = sim.get_state()
+    assert s["cell_vertex_num"][E] == 7
+    tt = w.Tiling(t.Lx, t.Ly, t.S, s["pos"], s["cell_vertex_num"], s["cell_vertices"], s["vertex_neighbors"],
+                  s["vertex_cell_neighbors"], s["theta"])
+    touched = set(e0) | set(s["vertex_neighbors"][list(e0)].ravel().tolist())   # the flipped edge and its star
+    far = [e for e in pointing_edges(s, E) if e[0] not in touched and e[1] not in touched]
+    assert len(far) >= 2
+    ea, eb = far[0], far[-1]
+    for a, b in (ea, eb):
+        tt.pos, _, _ = shrink_edge(tt, min(a, b), max(a, b), 0.5 * l_c)
+    return tt, kw, E, sorted([tuple(sorted(ea)), tuple(sorted(eb))])
+
+
+def test_repeated_passes_count_the_first_pass_and_raise_overflow_on_any_pass():
+    """Reading of DESIGN.md section 9: t1_short and overflow_rejects are statistics of the step's
+    first pass; the sticky error bit 2 ("a flip was suppressed because a row would exceed S") is
+    raised by whichever pass sees it first, also a repeated one."""
+    tt, kw, E, (first, second) = overflow_on_a_later_pass_case()
+    chk = oracle.from_tiling(tt, **kw)
+    cand, win = chk.debug_t1()
+    assert [tuple(x) for x in cand.tolist()] == [first, second] and [tuple(x) for x in win.tolist()] == [first]
+    many = oracle.from_tiling(tt, t1_max_passes=4, **kw)
+    many.step(1)
+    s = many.get_state()
+    st = s["stats"]
+    assert s["cell_vertex_num"][E] == 8
+    assert st["t1_short"] == 2 and st["t1_candidates"] == 2 and st["t1_flips"] == 1 and st["t1_blocked"] == 1
+    assert st["overflow_rejects"] == 0          # first-pass statistic: pass 1 rejected nothing
+    assert st["error"] == 2                      # pass 2 suppressed the second edge: E is full
+    cand, _ = many.debug_t1()
+    assert len(cand) == 0
+    # one pass per step: the overflow is seen (and counted) by the first pass of the NEXT step
+    one = oracle.from_tiling(tt, **kw)
+    one.step(1)
+    assert one.get_state()["stats"]["error"] == 0 and one.get_state()["stats"]["overflow_rejects"] == 0
+    one.step(1)
+    st = one.get_state()["stats"]
+    assert st["error"] == 2 and st["overflow_rejects"] == 1 and st["t1_short"] == 3 and st["t1_flips"] == 1
