@@ -49,7 +49,7 @@ typedef struct avm_sim avm_sim; /* opaque */
 typedef struct avm_params {
   int32_t n_cells;           /* N                                                               */
   int32_t n_vertices;        /* V, must equal 2N (3-coordinated tiling of the torus)            */
-  int32_t max_cell_vertices; /* S: row stride of cell_vertices, 4..32, multiple of 4            */
+  int32_t max_cell_vertices; /* S: row stride of cell_vertices, 8..32, multiple of 4            */
   int32_t sort_every;        /* 0 = never; k > 0 = Hilbert re-sort after every k-th step        */
   double Lx, Ly;             /* periodic box (R13); every cell must stay narrower than L/2      */
   double KA, KP, A0, P0;     /* Eq. A1: E = sum KA (A-A0)^2 + KP (P-P0)^2        */
@@ -63,7 +63,11 @@ typedef struct avm_params {
 
 enum {
   AVM_FLAG_SORT_AT_CREATE = 1, /* Hilbert-order cells and vertices once inside avm_create       */
-  AVM_FLAG_NO_GRAPH = 2,       /* reserved, no effect (kernels are always launched directly)    */
+  /* Kernel schedule of a step.  Default: chosen from the system size.  FUSED: two launches per
+   * step, the T1 flips of a step run inside the next force/move launch.  UNFUSED: three launches,
+   * a stand-alone T1 kernel.  Both give the same bits (tests); giving both flags is an error. */
+  AVM_FLAG_SCHEDULE_FUSED = 4,
+  AVM_FLAG_SCHEDULE_UNFUSED = 8,
   /* bits 8..15: maximum number of T1 passes per step.  0 or 1 = one pass per step (the rule of
    * BASELINE.json's north_star, the default and the timed path).  P > 1 = the paper's own rule
    * (the T1 kernel is "called repeatedly until no changes"): after the first pass

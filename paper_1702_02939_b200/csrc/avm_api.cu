@@ -37,6 +37,10 @@ inline size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
 inline int plane_stride(int V) { return (V + 63) & ~63; }
 
+inline size_t dirty_words(size_t V) { return ((V + 31) / 32 + 31) & ~(size_t)31; }   // per bitmap
+
+inline int t1_passes_of(const avm_params& p) { const int n = (p.flags & AVM_FLAG_T1_PASSES_MASK) >> AVM_FLAG_T1_PASSES_SHIFT; return n < 1 ? 1 : n; }
+
 struct BufferSet {
   int *vn, *vc, *cvn, *vtag, *ctag;
   int4* cv;
@@ -63,9 +67,9 @@ Layout make_layout(const avm_params& p) {
     L.theta[i] = take(8 * N); L.rec[i] = take(32 * N); L.tgt[i] = take(16 * N); L.vtag[i] = take(4 * V); L.ctag[i] = take(4 * N);
   }
   L.minkey = take(8 * N);
-  L.cand = take(sizeof(Cand) * 3 * N);
+  L.cand = take(sizeof(Cand) * (t1_passes_of(p) > 1 ? 5 : 3) * N);   // the step's list (3N = every edge) + two lists of N for repeated passes
   L.ctr = take(sizeof(Counters));
-  L.dirty = take(4 * ((V + 31) / 32));
+  L.dirty = take(4 * 2 * dirty_words(V));
   L.estamp = take(12 * Vs);
   L.ap = take(16 * N);
   L.epart = take(8 * 8 * 512);   // block partials of the observables (8 slots x up to 512 blocks)
@@ -80,7 +84,8 @@ bool params_ok(const avm_params* p) {
   if (!p) return false;
   if (p->n_cells < 4 || p->n_cells > (1 << 29)) return false;
   if (p->n_vertices != 2 * p->n_cells) return false;
-  if (p->max_cell_vertices < 4 || p->max_cell_vertices > 32 || (p->max_cell_vertices & 3)) return false;
+  if (p->max_cell_vertices < 8 || p->max_cell_vertices > 32 || (p->max_cell_vertices & 3)) return false;
+  if ((p->flags & AVM_FLAG_SCHEDULE_FUSED) && (p->flags & AVM_FLAG_SCHEDULE_UNFUSED)) return false;
   if (!(p->Lx > 0.0) || !(p->Ly > 0.0) || !(p->dt >= 0.0) || !(p->l_c >= 0.0) || !(p->Dr >= 0.0)) return false;
   if (p->sort_every < 0) return false;
   return true;
@@ -101,9 +106,14 @@ struct avm_sim {
   Counters* ctr;
   unsigned int* dirty;
   unsigned int* estamp;
+  unsigned int* d_feedback;   // device view of h_feedback (or a word of the counters)
   unsigned int stamp;    // id of the latest repeated T1 pass (estamp entries equal to it were tested in that pass)
   int t1_passes;         // T1 passes per step (1 = north_star's rule; > 1 = repeat until none, NEXT-1)
-  bool fused;            // T1 flips ride in force_move's prologue (cooperative launch available)
+  bool fused_ok;         // the two-launch schedule (T1 flips of a step ride in the next force/move launch) may be used
+  bool fused_forced;     // ... and is used whatever the T1 load is (AVM_FLAG_SCHEDULE_FUSED)
+  unsigned int* h_feedback;   // mapped host word (cudaHostAlloc): candidates of the latest completed step, written by
+                              // every force/move launch; NULL if the allocation failed (the guess of avm_create is kept)
+  unsigned int t1_guess;      // edges shorter than l_c at creation
   double2* ap;
   double* epart;
   SortScratch sc;
@@ -118,6 +128,7 @@ struct avm_sim {
     d.vn = b.vn; d.vc = b.vc; d.cv = b.cv; d.cvn = b.cvn; d.theta = b.theta; d.rec = b.rec; d.tgt = b.tgt;
     d.vtag = b.vtag; d.ctag = b.ctag;
     d.minkey = minkey; d.cand = cand; d.ctr = ctr; d.dirty = dirty; d.estamp = estamp;
+    d.feedback = d_feedback;
     return d;
   }
   Dev dev_alt() const {   // the other buffer set, target of a re-sort / staging area
@@ -280,7 +291,9 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   k.lc = params->l_c; k.lc2 = params->l_c * params->l_c;
   k.seed = params->seed;
   k.per_cell = 0;
-  k.cap_a = ((params->flags & AVM_FLAG_T1_PASSES_MASK) >> AVM_FLAG_T1_PASSES_SHIFT) > 1 ? N : 3 * N;
+  k.cap_a = 3 * N;
+  k.nw = (int)dirty_words((size_t)V);
+  k.fm_grid = force_move_grid(V);
   for (int r = 0; r < 10; ++r) k.rkey[r] = philox_round_key(params->seed, r);
   char* w = s->ws;
   for (int i = 0; i < 2; ++i) {
@@ -308,18 +321,32 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   // Two-launch schedule (flips inside the next force/move launch) pays when the sweep is longer
   // than the flippers' chain of dependent loads (~15 us): from about a million vertices; and for
   // tiny systems, which flip rarely and are bound by the number of launches.  In between the plain
-  // three-launch schedule is faster.  AVM_B200_FUSED / AVM_B200_UNFUSED override.
-  s->t1_passes = (params->flags & AVM_FLAG_T1_PASSES_MASK) >> AVM_FLAG_T1_PASSES_SHIFT;
-  if (s->t1_passes < 1) s->t1_passes = 1;
-  s->fused = s->t1_passes == 1 && AVM_FUSED_T1 && (V >= (1 << 20) || V <= 2048 || getenv("AVM_B200_FUSED")) &&
-             !getenv("AVM_B200_UNFUSED");
-  k.flag_dirty = s->fused ? 1 : 0;
+  // three-launch schedule is faster.  AVM_FLAG_SCHEDULE_FUSED / _UNFUSED override (both give the same bits).
+  s->t1_passes = t1_passes_of(*params);
+  s->fused_forced = (params->flags & AVM_FLAG_SCHEDULE_FUSED) != 0;
+  s->fused_ok = s->t1_passes == 1 && AVM_FUSED_T1 && (V >= (1 << 20) || V <= 2048 || s->fused_forced) &&
+                !(params->flags & AVM_FLAG_SCHEDULE_UNFUSED);
+  k.flag_dirty = 0; k.clear_dirty = 0;
+  s->h_feedback = nullptr;
+  s->d_feedback = &s->ctr->feedback_sink;
+  s->t1_guess = 0;
+  if (s->fused_ok && !s->fused_forced) {
+    void* h = nullptr;
+    void* dptr = nullptr;
+    if (cudaHostAlloc(&h, 64, cudaHostAllocMapped) == cudaSuccess && cudaHostGetDevicePointer(&dptr, h, 0) == cudaSuccess) {
+      s->h_feedback = (unsigned int*)h;
+      s->d_feedback = (unsigned int*)dptr;
+    } else {
+      if (h) cudaFreeHost(h);
+      cudaGetLastError();
+    }
+  }
 
   cudaStream_t st = s->stream;
   const cudaMemcpyKind kind = host_inputs ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
   const BufferSet& b = s->set[0];
   const BufferSet& stage = s->set[1];   // user-layout staging for the import kernel
-  auto fail = [&](int code) { delete s; return code; };
+  auto fail = [&](int code) { if (s->h_feedback) cudaFreeHost(s->h_feedback); delete s; return code; };
 #define AVM_CUDA_F(call)                                                                    \
   do {                                                                                      \
     cudaError_t e_ = (call);                                                                \
@@ -335,17 +362,20 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   AVM_CUDA_F(cudaMemcpyAsync(b.cvn, cvn, 4 * (size_t)N, kind, st));
   AVM_CUDA_F(cudaMemcpyAsync(b.theta, theta, 8 * (size_t)N, kind, st));
   AVM_CUDA_F(cudaMemsetAsync(s->ctr, 0, sizeof(Counters), st));
-  AVM_CUDA_F(cudaMemsetAsync(s->dirty, 0, 4 * (((size_t)V + 31) / 32), st));
+  AVM_CUDA_F(cudaMemsetAsync(s->dirty, 0, 4 * 2 * (size_t)k.nw, st));
   AVM_CUDA_F(cudaMemsetAsync(s->estamp, 0, 12 * (size_t)k.Vs, st));
   const Dev d = s->dev();
   import_kernel<<<cdiv(V, 256), 256, 0, st>>>(d, k, stage.vn, stage.vc, (const int*)stage.cv);
   validate_kernel<<<cdiv(V, 256), 256, 0, st>>>(d, k);
   s->launches += 2;
+  s->launches += launch_count_short_edges(d, k, st);      // first guess of the T1 load (into ctr->n_win)
   Counters c;
   AVM_CUDA_F(cudaMemcpyAsync(&c, s->ctr, sizeof(Counters), cudaMemcpyDeviceToHost, st));
   AVM_CUDA_F(cudaStreamSynchronize(st));
   AVM_CUDA_F(cudaGetLastError());
   if (c.error & 4) return fail(AVM_EINCONSISTENT);
+  s->t1_guess = c.n_win;
+  if (s->h_feedback) *s->h_feedback = s->t1_guess;
   s->launches += launch_refresh_cells(d, k, st);
   if (params->flags & AVM_FLAG_SORT_AT_CREATE) do_sort(s);
   AVM_CUDA_F(cudaGetLastError());
@@ -423,54 +453,72 @@ int avm_create_host(const avm_params* params, const double* pos_xy, const int32_
                        theta, workspace, workspace_bytes, cuda_stream, out, true);
 }
 
+// Schedule of one step.  Leaving the flips of a step pending (they then ride
+// in the next force/move launch: two launches per step) pays while there are few candidates: a few
+// dedicated warps handle them in the shadow of the sweep.  With many candidates the stand-alone T1
+// kernel is faster (more registers, quiet SMs).  The load is known from the count every force/move
+// launch reports through a mapped host word (read here without synchronising; it lags the device by
+// however far the host runs ahead, which is fine for a slowly varying load), before that from the
+// number of short edges at creation.  Both schedules give the same bits.
+#ifndef AVM_FUSED_MAX_CANDIDATES
+#define AVM_FUSED_MAX_CANDIDATES 96
+#endif
+static bool leave_flips_pending(const avm_sim* s, bool last_of_call) {
+  if (!s->fused_ok || last_of_call) return false;   // the last step of a call is completed inside the call
+  if (s->p.sort_every > 0 && (s->step + 1 - s->p.step0) % (unsigned long long)s->p.sort_every == 0) return false;   // so is the step before a re-sort
+  if (s->fused_forced) return true;
+  const unsigned load = s->h_feedback ? *(volatile unsigned int*)s->h_feedback : s->t1_guess;
+  return load <= AVM_FUSED_MAX_CANDIDATES;
+}
+
 int avm_step(avm_sim* s, int64_t n_steps) {
   if (!s || n_steps < 0) return AVM_EINVAL;
-  // Fused schedule: the flips of step i are applied by the force/move launch of step i+1, so
-  // the last step of this call (and the step before a re-sort) is completed by a flush.
-  bool pending = false;
+  bool pending = false;     // the previous step of this call left its flips pending
   for (int64_t i = 0; i < n_steps; ++i) {
-    int n = -1;
-    if (s->fused) {
-      n = launch_step(s->dev(), s->k, s->step, s->stream, nullptr, true);
-      if (n < 0) {   // the launch was refused: complete the previous step, then go on with three launches per step
-        if (pending) { s->launches += launch_t1_flush(s->dev(), s->k, s->step - 1, s->stream); pending = false; }
-        s->fused = false; s->k.flag_dirty = 0;
-      } else pending = true;
-    }
-    if (n < 0) n = launch_step(s->dev(), s->k, s->step, s->stream, nullptr, false);
-    s->launches += n;
+    const bool leave = leave_flips_pending(s, i == n_steps - 1);
+    s->launches += launch_step(s->dev(), s->k, s->step, s->stream, nullptr, pending, leave);
+    pending = leave;
     s->cur_pos = 1 - s->cur_pos;
     s->launches += extra_t1_passes(s);
     ++s->step;
-    if (s->p.sort_every > 0 && (s->step - s->p.step0) % (unsigned long long)s->p.sort_every == 0) {
-      if (pending) { s->launches += launch_t1_flush(s->dev(), s->k, s->step - 1, s->stream); pending = false; }
-      do_sort(s);
-    }
+    if (s->p.sort_every > 0 && (s->step - s->p.step0) % (unsigned long long)s->p.sort_every == 0) do_sort(s);
   }
-  if (pending) s->launches += launch_t1_flush(s->dev(), s->k, s->step - 1, s->stream);
   AVM_CUDA(cudaPeekAtLastError());
   return AVM_OK;
 }
+
+#ifdef AVM_TRACE
+// variant builds only: mean phase times (us) of the fused force/move launch since the last call
+extern "C" int avm_trace_read(avm_sim* s, double* out8) {
+  Counters c;
+  int rc = read_counters(s, &c);
+  if (rc) return rc;
+  for (int i = 1; i < 8; ++i) out8[i] = c.tr_acc[0] ? 1e-3 * (double)c.tr_acc[i] / (double)c.tr_acc[0] : 0.0;
+  out8[0] = (double)c.tr_acc[0];
+  // stamps of warp 0's first batch in the latest launch, relative to its entry into flipper_flips
+  fprintf(stderr, "w0 quads (us from entry): cand %.2f phase2 %.2f writes %.2f refresh %.2f rec %.2f | flipper_flips (us from entry): precheck %.2f claim %.2f quads %.2f loop_end %.2f fence %.2f signalled %.2f second_call_duration %.2f\n",
+          1e-3 * c.tr2[1], 1e-3 * c.tr2[2], 1e-3 * c.tr2[3], 1e-3 * c.tr2[4], 1e-3 * c.tr2[5],
+          1e-3 * c.tr2[9], 1e-3 * c.tr2[10], 1e-3 * c.tr2[11], 1e-3 * c.tr2[12], 1e-3 * c.tr2[13], 1e-3 * c.tr2[14], 1e-3 * c.tr2[15]);
+  fprintf(stderr, "   call: before_call->callee_entry %.2f, callee_entry->callee_end %.2f, callee_end->after_call %.2f\n", 1e-3 * (double)(long long)(c.tr2[7] - c.tr2[6]), 1e-3 * (double)(long long)(c.tr2[8] - c.tr2[7]), 1e-3 * (double)(long long)(c.tr2[0] - c.tr2[8]));
+  fprintf(stderr, "   per-lane phase2 / end (us): ");
+  for (int l = 0; l < 32; ++l) fprintf(stderr, "%.1f/%.1f ", 1e-3 * c.tr2[16 + l], 1e-3 * c.tr2[48 + l]);
+  fprintf(stderr, "\n");
+  cudaMemsetAsync(s->ctr->tr_acc, 0, sizeof(c.tr_acc), s->stream);
+  return AVM_OK;
+}
+#endif
 
 int avm_step_profile(avm_sim* s, int64_t n_steps, double* ms_per_kernel) {
   if (!s || n_steps < 0 || !ms_per_kernel) return AVM_EINVAL;
   cudaEvent_t ev[AVM_K_COUNT + 1];
   for (int i = 0; i <= AVM_K_COUNT; ++i) AVM_CUDA(cudaEventCreate(&ev[i]));
   for (int i = 0; i < AVM_K_COUNT; ++i) ms_per_kernel[i] = 0.0;
-  // same schedule as avm_step (fused: the flips of step i ride in the force/move launch of step
-  // i+1, so the third slot only sees the final flush); the events serialise the launches
+  // same schedule decisions as avm_step; the events serialise the launches
   bool pending = false;
   for (int64_t i = 0; i < n_steps; ++i) {
-    int n = -1;
-    if (s->fused) {
-      n = launch_step(s->dev(), s->k, s->step, s->stream, ev, true);
-      if (n < 0) {   // the launch was refused: complete the previous step, then go on with three launches per step
-        if (pending) { s->launches += launch_t1_flush(s->dev(), s->k, s->step - 1, s->stream); pending = false; }
-        s->fused = false; s->k.flag_dirty = 0;
-      } else pending = true;
-    }
-    if (n < 0) n = launch_step(s->dev(), s->k, s->step, s->stream, ev, false);
-    s->launches += n;
+    const bool leave = leave_flips_pending(s, i == n_steps - 1);
+    s->launches += launch_step(s->dev(), s->k, s->step, s->stream, ev, pending, leave);
+    pending = leave;
     s->cur_pos = 1 - s->cur_pos;
     s->launches += extra_t1_passes(s);                  // outside the per-kernel slots
     ++s->step;
@@ -478,21 +526,9 @@ int avm_step_profile(avm_sim* s, int64_t n_steps, double* ms_per_kernel) {
     for (int j = 0; j < AVM_K_COUNT; ++j) {
       float ms = 0.f;
       AVM_CUDA(cudaEventElapsedTime(&ms, ev[j], ev[j + 1]));
-      if (!(pending && j == AVM_K_T1_FLIP)) ms_per_kernel[j] += ms;   // fused: nothing ran in that slot
+      if (!(leave && j == AVM_K_T1_FLIP)) ms_per_kernel[j] += ms;   // two-launch step: nothing ran in that slot
     }
-    if (s->p.sort_every > 0 && (s->step - s->p.step0) % (unsigned long long)s->p.sort_every == 0) {
-      if (pending) { s->launches += launch_t1_flush(s->dev(), s->k, s->step - 1, s->stream); pending = false; }
-      do_sort(s);
-    }
-  }
-  if (pending) {
-    AVM_CUDA(cudaEventRecord(ev[0], s->stream));
-    s->launches += launch_t1_flush(s->dev(), s->k, s->step - 1, s->stream);
-    AVM_CUDA(cudaEventRecord(ev[1], s->stream));
-    AVM_CUDA(cudaEventSynchronize(ev[1]));
-    float ms = 0.f;
-    AVM_CUDA(cudaEventElapsedTime(&ms, ev[0], ev[1]));
-    ms_per_kernel[AVM_K_T1_FLIP] += ms;
+    if (s->p.sort_every > 0 && (s->step - s->p.step0) % (unsigned long long)s->p.sort_every == 0) do_sort(s);
   }
   for (int i = 0; i <= AVM_K_COUNT; ++i) cudaEventDestroy(ev[i]);
   AVM_CUDA(cudaGetLastError());
@@ -636,7 +672,11 @@ uint32_t avm_hilbert_index_host(int32_t m, uint32_t ix, uint32_t iy) {
   return hilbert_index_host(ix, iy, m);
 }
 
-void avm_destroy(avm_sim* s) { delete s; }
+void avm_destroy(avm_sim* s) {
+  if (!s) return;
+  if (s->h_feedback) cudaFreeHost(s->h_feedback);
+  delete s;
+}
 
 const char* avm_strerror(int code) {
   switch (code) {

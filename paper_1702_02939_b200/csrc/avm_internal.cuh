@@ -31,12 +31,20 @@ struct Counters {
   // candidate list length, double-buffered by step parity: the list of step s is flipped by
   // t1_flip(s) and its per-cell minimum keys are cleared by the prologue of force_move(s+1)
   unsigned int n_cand[4];   // [0], [1]: the step's list by step parity; [2], [3]: lists of repeated passes (NEXT-1)
-  unsigned int n_win;     // winners (debug hook only)
-  unsigned int flip_done; // fused schedule: candidates decided so far          } zeroed by the
-  unsigned int next_cand; // fused schedule: next candidate index to be claimed  } cell pass of
-  unsigned int next_quad; // fused schedule: next candidate whose cells' flagged } every step
+  unsigned int n_win;     // winners (debug hook); short edges at creation
+  unsigned int feedback_sink;   // target of Dev::feedback when no mapped host word is available
+  unsigned int pad0[26];
+  // fused schedule, zeroed by the cell pass of every step.  Each on a 128-byte line of its own: the
+  // first is hammered by claiming atomics while waiting warps poll the second.
+  unsigned int next_cand; // next candidate index to be claimed
+  unsigned int pad1[31];
+  unsigned int flip_done; // candidates decided so far
+  unsigned int pad2[31];
   long long t1_short, t1_candidates, t1_flips, t1_blocked, overflow_rejects, error;
   double obs[8];   // observables of the latest avm_energy / avm_observe call (slots: avm_step.cu)
+  // phase trace of the fused force/move launch (variant builds with -DAVM_TRACE only): tr = this launch's
+  // min start / max phase-end times (ns, %globaltimer), tr_acc = sums of (phase end - start) over launches
+  unsigned long long tr[8], tr_acc[8], tr2[80];
 };
 
 // Model constants, passed by value to every kernel.
@@ -50,8 +58,11 @@ struct Consts {
   double amp;                // sqrt(2 Dr dt) (R8)
   double lc, lc2;
   int flag_dirty;            // 1: the marking thread flags the vertices of a candidate's cells (two-launch schedule only)
+  int clear_dirty;           // 1: the cell pass clears the bitmap the force/move launch of this step swept with
+  int nw;                    // words per dirty bitmap (V/32 rounded up to a multiple of 32)
+  int fm_grid;               // CTAs of the persistent force/move grid (a whole number per SM, set at create)
   int per_cell;              // 1: preferred values A0_i, P0_i per cell (Dev::tgt, Eq. 1), 0: uniform A0, P0 (Eq. A1)
-  int cap_a;                 // capacity of the step's candidate list (3N, or N when repeated passes use the rest)
+  int cap_a;                 // capacity of the step's candidate list (3N: every edge of the tiling)
   unsigned long long seed;
   uint2 rkey[10];            // Philox round keys of `seed` (the key schedule is uniform: done once on the host)
 };
@@ -77,10 +88,14 @@ struct Dev {
   int* ctag;          // [N] user index of each cell
   unsigned long long* minkey;  // [N] per-cell minimum candidate key, ~0 when idle
   Cand* cand;         // [3N]
-  unsigned int* dirty; // [ceil(V/32)] bit v: vertex v belongs to a cell of some pending T1 candidate
+  unsigned int* dirty; // [2][nw] bit v of buffer (s & 1): vertex v belongs to a cell of a T1 candidate found in
+                       // step s.  Written only by the cell pass of step s, read only by the force/move launch
+                       // of step s+1 (read-only for that whole launch), cleared by the cell pass of step s+1.
   double2* tgt;       // [N] (A0_i, P0_i), internal order; read only when Consts::per_cell (NEXT-4)
   unsigned int* estamp; // [3*Vs] per directed half-edge (slot plane, owner vertex): id of the repeated pass that tested it last
   Counters* ctr;
+  unsigned int* feedback; // mapped HOST word: every force/move launch reports the candidate count of the previous step
+                          // (read by the host without synchronising, to choose the schedule of later steps)
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -210,9 +225,10 @@ __device__ __forceinline__ void cell_area_perimeter(const double2* pos, const in
 }
 
 // Candidate lists.  List 0 / 1 (the step's list, by step parity) starts at d.cand and holds up to
-// k.cap_a entries; lists 2 / 3 (repeated passes, NEXT-1) hold up to N entries each behind it.
+// k.cap_a = 3N entries; lists 2 / 3 (repeated passes, NEXT-1; allocated only when they are enabled)
+// hold up to N entries each behind it.
 __device__ __forceinline__ Cand* list_base(const Dev& d, const Consts& k, unsigned list) {
-  return d.cand + (list < 2u ? (size_t)0 : (size_t)(list - 1u) * (size_t)k.N);
+  return d.cand + (list < 2u ? (size_t)0 : (size_t)(list + 1u) * (size_t)k.N);
 }
 __device__ __forceinline__ unsigned list_cap(const Consts& k, unsigned list) { return list < 2u ? (unsigned)k.cap_a : (unsigned)k.N; }
 
@@ -220,8 +236,12 @@ __device__ __forceinline__ unsigned list_cap(const Consts& k, unsigned list) { r
 // host-side launchers (defined in the .cu files); every launcher returns the number of kernels
 // it enqueued so that the API can keep avm_stats.kernel_launches honest.
 // ---------------------------------------------------------------------------------------------
-int launch_step(const Dev& d, const Consts& k, unsigned long long step, cudaStream_t s, cudaEvent_t* ev = nullptr, bool fused = false);
-int launch_t1_flush(const Dev& d, const Consts& k, unsigned long long last_step, cudaStream_t s);
+int force_move_grid(int V);
+// One timestep.  consume_pending: the previous step left its T1 flips pending (they ride in this force/move
+// launch); leave_pending: this step leaves its own flips pending (two launches) instead of running t1_flip_kernel.
+int launch_step(const Dev& d, const Consts& k, unsigned long long step, cudaStream_t s, cudaEvent_t* ev, bool consume_pending,
+                bool leave_pending);
+int launch_count_short_edges(const Dev& d, const Consts& k, cudaStream_t s);
 int launch_refresh_cells(const Dev& d, const Consts& k, cudaStream_t s);
 int launch_t1_reset(const Dev& d, const Consts& k, cudaStream_t s);
 int launch_t1_pass_only(const Dev& d, const Consts& k, cudaStream_t s);

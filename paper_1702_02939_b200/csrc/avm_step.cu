@@ -10,9 +10,9 @@
 //                                  shorter than l_c are tested for eligibility by the detecting
 //                                  thread, appended to the candidate list and their key is
 //                                  atomicMin-ed into the four cells (conflict rule, marking half).
-//   T1 flips     (warp/candidate) rows a6+a7 (t1_try_flip): a candidate whose key is the minimum on
-//                                  all four of its cells flips; the warp rewrites the four lists
-//                                  cooperatively and refreshes the four cells' cached geometry.
+//   T1 flips     (4 lanes/candidate) rows a6+a7 (t1_flip_quads): a candidate whose key is the minimum
+//                                  on all four of its cells flips; each of the four lanes rewrites
+//                                  one cell row and refreshes that cell's cached geometry.
 //                                  Two-launch schedule (large systems): run by a few "flipper"
 //                                  warps inside the NEXT step's force_move launch while the other
 //                                  warps sweep.  Three-launch schedule: t1_flip_kernel.
@@ -42,9 +42,6 @@ static constexpr unsigned kFull = 0xffffffffu;
 #ifndef AVM_CU_MINB
 #define AVM_CU_MINB 8      // cell pass: resident CTAs per SM asked of the compiler (64 registers; measured best of 7..11)
 #endif
-#ifndef AVM_FM_COOP
-#define AVM_FM_COOP 0       // launch the fused force_move as a cooperative grid (not needed: work is claimed, see flipper_work)
-#endif
 #ifndef AVM_FM_MINB
 #define AVM_FM_MINB 3      // force_move: minimum resident CTAs per SM asked of the compiler
 #endif
@@ -60,6 +57,14 @@ static constexpr unsigned kFull = 0xffffffffu;
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
 
+#ifdef AVM_TRACE
+__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define AVM_TR_MAX(slot) do { if (lane == 0) atomicMax(&d.ctr->tr[slot], gtime()); } while (0)
+#define AVM_TR_W0(slot, dep) do { if (trq && blockIdx.x == 0 && threadIdx.x == 0) { if (slot == 0) tq0 = gtime(); else d.ctr->tr2[slot] = gtime() + ((dep) & 0) - tq0; } } while (0)
+#else
+#define AVM_TR_MAX(slot) do { } while (0)
+#define AVM_TR_W0(slot, dep) do { } while (0)
+#endif
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 // ---- cache-hinted loads -------------------------------------------------------------------------
@@ -169,16 +174,18 @@ __device__ __forceinline__ unsigned int ld_volatile(const unsigned int* p) {
   return x;
 }
 
-__device__ __noinline__ bool t1_try_flip(const Dev& d, const Consts& k, const Cand& c, const int lane);
+__device__ __noinline__ unsigned t1_flip_quads(const Dev& d, const Consts& k, const Cand* __restrict__ list, unsigned base,
+                                               unsigned n, const int lane);
 
-// The sweep of one thread over vertices first, first + step_v, ...  kSkipDirty: vertices
-// flagged in d.dirty are left to the flippers.
+// The sweep of one thread over vertices first, first + step_v, ...  kSkipDirty: vertices flagged
+// in `dirty` (read-only for this whole launch) are left to the dirty pass below.
 template <bool kSkipDirty>
-__device__ __forceinline__ void sweep(const Dev& d, const Consts& k, const int first, const int step_v, const int lane) {
+__device__ __forceinline__ void sweep(const Dev& d, const Consts& k, const unsigned int* __restrict__ dirty, const int first,
+                                      const int step_v, const int lane) {
   if (first >= k.V) return;
   int v = first;
   VertexIn in = load_vertex(d, k, v);
-  unsigned dw = kSkipDirty ? __ldg(d.dirty + (v >> 5)) : 0u;
+  unsigned dw = kSkipDirty ? __ldg(dirty + (v >> 5)) : 0u;
   for (;;) {
     if (AVM_FM_PF) {
       // pull the contiguous streams of a later sweep into L2: positions, both index lists and the
@@ -200,40 +207,80 @@ __device__ __forceinline__ void sweep(const Dev& d, const Consts& k, const int f
       const double2 q0 = __ldg(d.pos + in.n0), q1 = __ldg(d.pos + in.n1), q2 = __ldg(d.pos + in.n2);
       const CellRec c0 = ld_rec(d.rec + in.c0), c1 = ld_rec(d.rec + in.c1), c2 = ld_rec(d.rec + in.c2);
       const double2 h = in.h;
-      if (AVM_FM_REGPF && vnext < k.V) { in = load_vertex(d, k, vnext); if (kSkipDirty) dw = __ldg(d.dirty + (vnext >> 5)); }
+      if (AVM_FM_REGPF && vnext < k.V) { in = load_vertex(d, k, vnext); if (kSkipDirty) dw = __ldg(dirty + (vnext >> 5)); }
       move_vertex(d, k, v, h, q0, q1, q2, c0, c1, c2);
     } else if (AVM_FM_REGPF && vnext < k.V) {
       in = load_vertex(d, k, vnext);
-      dw = __ldg(d.dirty + (vnext >> 5));
+      dw = __ldg(dirty + (vnext >> 5));
     }
     if (vnext >= k.V) break;
     v = vnext;
-    if (!AVM_FM_REGPF) { in = load_vertex(d, k, v); if (kSkipDirty) dw = __ldg(d.dirty + (v >> 5)); }
+    if (!AVM_FM_REGPF) { in = load_vertex(d, k, v); if (kSkipDirty) dw = __ldg(dirty + (v >> 5)); }
   }
 }
 
-// Rows a6 + a7 of the previous step inside the fused force_move launch, run by the "flipper"
-// warps (the first F warps of the grid, which take no share of the sweep).  Work is CLAIMED with
-// atomic counters, so a candidate always belongs to a warp that is running: the wait below can
-// never depend on a CTA that has not been scheduled yet (no co-residency assumption).
-//   1. claim candidates one by one; decide and flip each (t1_try_flip);
-//   2. wait until every candidate has been decided (flip_done == prev);
-//   3. claim candidates again: move the flagged vertices of the candidate's four cells with
-//      loads that bypass L1 (whoever clears a vertex's bit moves it) and release the cells'
-//      minimum keys (row a6).
-__device__ __noinline__ void flipper_flips(const Dev& d, const Consts& k, const unsigned prev, const int lane) {
+// Rows a6 + a7 of the previous step inside the fused force_move launch.
+//   flips : candidates are CLAIMED eight at a time with an atomic counter and decided / flipped by
+//           t1_flip_quads (four lanes per candidate).
+//   wait  : until every candidate has been decided (flip_done == prev).
+//   moves : one unit per candidate, claimed likewise: the vertices of its four cells (exactly the
+//           vertices whose inputs a flip can rewrite; the sweep skipped them) are moved now and
+//           the cells' minimum keys are released.
+// A few "flipper" warps do nothing else, so with few candidates all of this runs in the shadow of
+// the sweep; with many candidates every warp also claims what is left once its share of the
+// sweep is done.  Work is claimed, so a candidate always belongs to a warp that is running: the
+// wait can never depend on a CTA that has not been scheduled (no co-residency assumption).
+// The bitmap of flagged vertices is read-only for the whole launch (the cell pass of the previous
+// step wrote it, the cell pass of this step clears it), so the sweep's decision to skip a vertex
+// never changes while flips are in flight.
+// first: a batch already claimed for this warp (by its CTA), or >= prev for none
+__device__ __noinline__ void flipper_flips(const Dev& d, const Consts& k, const unsigned prev, const int lane, const unsigned first) {
   unsigned mine = 0, flips = 0;
+  unsigned i = first;
+#ifdef AVM_TRACE
+  const bool w0 = blockIdx.x == 0 && threadIdx.x == 0;
+  unsigned long long ts[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  ts[0] = gtime();
+#endif
   for (;;) {
-    unsigned i = 0;
-    if (lane == 0) i = atomicAdd(&d.ctr->next_cand, 1u);
-    i = __shfl_sync(kFull, i, 0);
-    if (i >= prev) break;
-    const Cand c = d.cand[i];
-    if (t1_try_flip(d, k, c, lane)) ++flips;
-    ++mine;
+    if (i >= prev) {
+      const unsigned nc = ld_volatile(&d.ctr->next_cand);
+#ifdef AVM_TRACE
+      if (!ts[1]) ts[1] = gtime() + (nc & 0);
+#endif
+      if (nc >= prev) break;        // nothing left: no atomic
+      if (lane == 0) i = atomicAdd(&d.ctr->next_cand, 8u);
+      i = __shfl_sync(kFull, i, 0);
+#ifdef AVM_TRACE
+      if (!ts[2]) ts[2] = gtime() + (i & 0);
+#endif
+      if (i >= prev) break;
+    }
+#ifdef AVM_TRACE
+    const unsigned long long tb = gtime();
+    if (w0) d.ctr->tr2[6] = tb;
+#endif
+#ifdef AVM_TRACE
+    flips += t1_flip_quads(d, k, d.cand, i, prev, lane | 0x100);
+#else
+    flips += t1_flip_quads(d, k, d.cand, i, prev, lane);
+#endif
+#ifdef AVM_TRACE
+    if (w0) d.ctr->tr2[0] = gtime() + (flips & 0);
+    if (!ts[3]) ts[3] = gtime() + (flips & 0);
+    else if (!ts[7]) ts[7] = ts[0] + gtime() + (flips & 0) - tb;      // duration of the second call
+#endif
+    mine += min(8u, prev - i);
+    i = prev;
   }
+#ifdef AVM_TRACE
+  ts[4] = gtime();
+#endif
   if (mine) {
     __threadfence();
+#ifdef AVM_TRACE
+    ts[5] = gtime();
+#endif
     __syncwarp();
     if (lane == 0) {
       if (flips) atomicAdd((unsigned long long*)&d.ctr->t1_flips, (unsigned long long)flips);
@@ -241,45 +288,91 @@ __device__ __noinline__ void flipper_flips(const Dev& d, const Consts& k, const 
       atomicAdd(&d.ctr->flip_done, mine);
     }
   }
+#ifdef AVM_TRACE
+  ts[6] = gtime();
+  if (w0 && mine) for (int j = 1; j < 8; ++j) d.ctr->tr2[8 + j] = ts[j] > ts[0] ? ts[j] - ts[0] : 0;
+#endif
 }
 
-__device__ __noinline__ void flipper_moves(const Dev& d, const Consts& k, const unsigned prev, const int lane) {
-  while (ld_volatile(&d.ctr->flip_done) < prev) __nanosleep(64);
-  __threadfence();
-  // rows of up to 16 entries: two rows per pass (half a warp each), else one row per pass
-  const bool two = k.S <= 16;
-  const int half = two ? lane >> 4 : 0, j = two ? lane & 15 : lane;
-  for (;;) {
-    unsigned i = 0;
-    if (lane == 0) i = atomicAdd(&d.ctr->next_quad, 1u);
-    i = __shfl_sync(kFull, i, 0);
-    if (i >= prev) break;
-    const Cand c = d.cand[i];
-    const int quad[4] = {c.cL, c.cR, c.cE1, c.cE2};
-#pragma unroll 1
-    for (int t0 = 0; t0 < 4; t0 += (two ? 2 : 1)) {
-      const int cell = quad[t0 + half];
-      // the entry is loaded whatever the row length is (padding repeats entry 0): no dependent load
-      const int n = __ldcg(d.cvn + cell);
-      const int u = __ldcg(reinterpret_cast<const int*>(d.cv + (size_t)(j >> 2) * k.N + cell) + (j & 3));
-      if (j < n) {
-        const unsigned bit = 1u << (u & 31);
-        if (atomicAnd(&d.dirty[u >> 5], ~bit) & bit) move_vertex_coherent(d, k, u);
+// One unit of post-flip work = one candidate (few-candidate mode): every vertex of the (post-flip)
+// rows of its four cells is moved, with loads that bypass L1, and the cells' minimum keys go back
+// to idle (row a6).  Units are assigned statically: nothing ever waits for a unit.
+// Lanes = 4 cells x 8 row entries per pass (96 % of the cells need one pass); a vertex that sits
+// in several of the four rows is moved by the lowest lane holding it.  A vertex shared with
+// another candidate's cells is moved twice, with the same inputs and the same result.
+__device__ __noinline__ void mover_unit(const Dev& d, const Consts& k, const unsigned i, const int lane) {
+  const int t = lane >> 3, j8 = lane & 7;
+  const int4 q = __ldcg(reinterpret_cast<const int4*>(d.cand + i) + 1);   // (cL, cR, cE1, cE2)
+  const int cell = t == 0 ? q.x : t == 1 ? q.y : t == 2 ? q.z : q.w;
+  // entry j8 is loaded whatever the row length is (padding repeats entry 0): no dependent load
+  const int n = __ldcg(d.cvn + cell);
+  int u = __ldcg(reinterpret_cast<const int*>(d.cv + (size_t)(j8 >> 2) * k.N + cell) + (j8 & 3));
+  int nmax = max(n, __shfl_xor_sync(kFull, n, 8));
+  nmax = max(nmax, __shfl_xor_sync(kFull, nmax, 16));
+  for (int j0 = 0; j0 < nmax; j0 += 8) {
+    const int j = j0 + j8;
+    if (j0 > 0 && j < n) u = __ldcg(reinterpret_cast<const int*>(d.cv + (size_t)(j >> 2) * k.N + cell) + (j & 3));
+    const int uu = j < n ? u : -1 - lane;                                   // inactive lanes match nobody
+    const unsigned same = __match_any_sync(kFull, uu);
+    if (j < n && __ffs(same) - 1 == lane) move_vertex_coherent(d, k, u);
+  }
+  if (lane < 4) d.minkey[lane == 0 ? q.x : lane == 1 ? q.y : lane == 2 ? q.z : q.w] = ~0ull;
+}
+
+// Moves every flagged vertex of this warp's slice of the bitmap (many-candidate mode).  The set
+// bits of up to 32 words (1024 vertices) are compacted so that all 32 lanes work: an inclusive
+// scan of the population counts, then each lane finds the word and the bit of "its" vertex.
+__device__ __noinline__ void dirty_pass(const Dev& d, const Consts& k, const unsigned int* __restrict__ dirty,
+                                        const unsigned gwarp, const unsigned nwarps, const int lane) {
+  const unsigned per = ((unsigned)k.nw + nwarps - 1u) / nwarps;
+  const unsigned w0 = min(gwarp * per, (unsigned)k.nw), w1 = min(w0 + per, (unsigned)k.nw);
+  for (unsigned base = w0; base < w1; base += 32u) {
+    const unsigned word = base + lane < w1 ? __ldg(dirty + base + lane) : 0u;
+    if (!__any_sync(kFull, word != 0u)) continue;
+    int incl = __popc(word);
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int y = __shfl_up_sync(kFull, incl, o);
+      if (lane >= o) incl += y;
+    }
+    const int total = __shfl_sync(kFull, incl, 31);
+    for (int k0 = 0; k0 < total; k0 += 32) {
+      const int idx = k0 + lane;
+      int j = 0;                                   // number of words whose inclusive count is <= idx
+#pragma unroll
+      for (int st = 16; st > 0; st >>= 1) {
+        const int probe = __shfl_sync(kFull, incl, j + st - 1);
+        if (probe <= idx) j += st;
+      }
+      j = min(j, 31);
+      const unsigned wj = __shfl_sync(kFull, word, j);
+      const int excl = __shfl_sync(kFull, incl, j) - __popc(wj);
+      if (idx < total) {
+        const int bit = (int)__fns(wj, 0u, idx - excl + 1);
+        move_vertex_coherent(d, k, (int)((base + (unsigned)j) * 32u) + bit);
       }
     }
-    if (lane < 4) d.minkey[quad[lane & 3]] = ~0ull;
   }
 }
 
-// Persistent grid-stride kernel: each thread keeps the streaming loads of its NEXT vertex in
-// flight while it gathers and computes the current one.
+// minimum keys of candidates [i0, i1) back to idle (row a6), thread per candidate
+__device__ __forceinline__ void release_minkeys(const Dev& d, const unsigned i0, const unsigned i1, const unsigned step, const unsigned first) {
+  for (unsigned i = i0 + first; i < i1; i += step) {
+    const int4 q = __ldcg(reinterpret_cast<const int4*>(d.cand + i) + 1);   // (cL, cR, cE1, cE2)
+    d.minkey[q.x] = ~0ull; d.minkey[q.y] = ~0ull; d.minkey[q.z] = ~0ull; d.minkey[q.w] = ~0ull;
+  }
+}
+
+// Persistent grid-stride kernel (thread per vertex, rows a2 + a3).
 //
-// kFused also carries rows a6 + a7 of the PREVIOUS step (flipper_flips / flipper_moves above):
-// a few warps decide and flip that step's candidates while all other warps already move
-// vertices.  A vertex whose inputs a flip may rewrite has its bit set in d.dirty (the marking
-// thread flagged every vertex of the candidate's four cells); the sweep skips it and a flipper
-// moves it once every candidate has been decided.  The latency-bound flips thus overlap the
-// gather-bound sweep and the step needs no third launch.
+// kFused also carries rows a6 + a7 of the PREVIOUS step (above): a few warps decide and flip that
+// step's candidates while all other warps already move vertices.  A vertex whose inputs a flip may
+// rewrite has its bit set in the bitmap; the sweep skips it and the dirty pass moves it once every
+// candidate has been decided.  The latency-bound flips thus overlap the gather-bound sweep and
+// the step needs no third launch.
+#ifndef AVM_LIGHT_MAX
+#define AVM_LIGHT_MAX 256       // up to this many candidates: one dedicated flipper warp per candidate
+#endif
 template <bool kFused>
 __global__ void __launch_bounds__(kVertexBlock, AVM_FM_MINB)
 force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, const unsigned parity) {
@@ -290,26 +383,50 @@ force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts 
   const int lane = threadIdx.x & 31;
   const unsigned prev = min(d.ctr->n_cand[parity ^ 1u], (unsigned)k.cap_a);
   const unsigned gwarp = (unsigned)tid >> 5, nwarps = (unsigned)stride >> 5;
-  if (tid == 0) d.ctr->n_cand[parity] = 0;
+  if (tid == 0) { d.ctr->n_cand[parity] = 0; *d.feedback = prev; }
   if (kFused) {
-    if (tid == 0 && prev) atomicAdd((unsigned long long*)&d.ctr->t1_candidates, (unsigned long long)prev);
-    if (2u * prev <= nwarps) {
-      // few candidates: the first `prev` warps only flip (they would start the sweep late and
-      // finish it last), all others only sweep
-      if (gwarp < prev) {
-        flipper_flips(d, k, prev, lane);
-        flipper_moves(d, k, prev, lane);
+    if (prev == 0u) { sweep<false>(d, k, nullptr, tid, stride, lane); return; }
+    if (tid == 0) atomicAdd((unsigned long long*)&d.ctr->t1_candidates, (unsigned long long)prev);
+#ifdef AVM_TRACE
+    if (lane == 0) atomicMin(&d.ctr->tr[0], gtime());
+#endif
+    const unsigned int* __restrict__ dirty = d.dirty + (size_t)(parity ^ 1u) * (size_t)k.nw;
+    if (prev <= AVM_LIGHT_MAX) {
+      // few candidates: one dedicated warp per candidate (warp 0 of the first CTAs, then warp 1, ...:
+      // consecutive CTAs sit on different SMs) flips it, waits for all decisions and moves the
+      // vertices of its cells, all in the shadow of the sweep; every other warp only sweeps
+      const unsigned wib = threadIdx.x >> 5, nb = gridDim.x;
+      const unsigned fid = wib * nb + blockIdx.x;                          // flipper id of this warp, if < prev
+      const unsigned full = prev / nb, rest = prev % nb;                   // warps 0..full-1 of every CTA, warp `full` of `rest` CTAs
+      if (fid < prev) {
+        if (fid * 8u < prev) flipper_flips(d, k, prev, lane, prev);        // the first prev/8 of them claim the flips
+        AVM_TR_MAX(1);
+        while (ld_volatile(&d.ctr->flip_done) < prev) __nanosleep(64);
+        __threadfence();
+        AVM_TR_MAX(3);
+        mover_unit(d, k, fid, lane);
+        AVM_TR_MAX(4);
       } else {
-        const int first = (int)(gwarp - prev) * 32 + lane, step_v = (int)(nwarps - prev) * 32;
-        if (prev) sweep<true>(d, k, first, step_v, lane);
-        else sweep<false>(d, k, first, step_v, lane);
+        const unsigned before = blockIdx.x * full + min(blockIdx.x, rest) + min(wib, full) + (wib > full && blockIdx.x < rest ? 1u : 0u);
+        sweep<true>(d, k, dirty, (int)((gwarp - before) * 32u) + lane, (int)((nwarps - prev) * 32u), lane);
+        AVM_TR_MAX(2);
       }
     } else {
-      // many candidates (the burst after a random start, T1-heavy regimes): every warp flips,
-      // then sweeps its share, then moves flagged vertices
-      flipper_flips(d, k, prev, lane);
-      sweep<true>(d, k, tid, stride, lane);
-      flipper_moves(d, k, prev, lane);
+      // many candidates (the burst after a random start, T1-heavy regimes): the flips come first,
+      // claimed by all warps while the SMs are quiet (under the sweep's load every dependent access
+      // of a flip takes ~3x longer, and a warp that flips would start a static share of the sweep
+      // late and finish last); when every candidate has been decided, a plain sweep moves all vertices
+      __shared__ unsigned s_first;
+      if (threadIdx.x == 0) s_first = atomicAdd(&d.ctr->next_cand, 8u * (kVertexBlock / 32));   // one claim per CTA
+      __syncthreads();
+      flipper_flips(d, k, prev, lane, s_first + 8u * (threadIdx.x >> 5));
+      AVM_TR_MAX(1);
+      while (ld_volatile(&d.ctr->flip_done) < prev) __nanosleep(32);
+      __threadfence();
+      AVM_TR_MAX(3);
+      release_minkeys(d, 0u, prev, (unsigned)stride, (unsigned)tid);       // every decision has been taken (row a6)
+      sweep<false>(d, k, nullptr, tid, stride, lane);
+      AVM_TR_MAX(2);
     }
   } else {
     // the previous step's T1 candidates are done: clear their cells' minimum keys (row a6)
@@ -317,7 +434,7 @@ force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts 
       const Cand c = d.cand[i];
       d.minkey[c.cL] = ~0ull; d.minkey[c.cR] = ~0ull; d.minkey[c.cE1] = ~0ull; d.minkey[c.cE2] = ~0ull;
     }
-    sweep<false>(d, k, tid, stride, lane);
+    sweep<false>(d, k, nullptr, tid, stride, lane);
   }
 }
 
@@ -325,7 +442,13 @@ force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts 
 // rows a5 (eligibility, R10) + a6 (marking half of the conflict rule, R11) for ONE short edge,
 // run by the thread that found it.  (va, vb) are current vertex indices.  Cold path.
 // ---------------------------------------------------------------------------------------------
-__device__ __noinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va, int vb, unsigned parity, bool count_stats) {
+// mode: kMarkFirstPass = the step's detection on the moved positions (counts t1_short /
+// overflow_rejects, flags the dirty bitmap of the fused schedule); kMarkRepeatedPass = a repeated
+// pass of NEXT-1 (no statistics, but the sticky overflow bit is still raised);
+// kMarkSilent = the debug hook (no side effects beyond the list and the minimum keys).
+enum : int { kMarkSilent = 0, kMarkFirstPass = 1, kMarkRepeatedPass = 2 };
+__device__ __noinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va, int vb, unsigned parity, const int mode) {
+  const bool count_stats = mode == kMarkFirstPass;
   // The marking thread delays the end of the cell pass when it sits in the last wave, so its
   // loads are issued in two batches of independent loads instead of a chain of five.
   // ---- batch 1: everything known from (va, vb) ----
@@ -365,10 +488,8 @@ __device__ __noinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va,
   const int x1s1 = d.vn[k.Vs + x1], x1s2 = d.vn[2 * k.Vs + x1], x2s1 = d.vn[k.Vs + x2], x2s2 = d.vn[2 * k.Vs + x2];
   if (!(nq[0] > 3 && nq[1] > 3)) return;                       // no 2-gons (T2 absent)
   if (!(nq[2] < k.S && nq[3] < k.S)) {                         // row would exceed the stride
-    if (count_stats) {
-      atomicAdd((unsigned long long*)&d.ctr->overflow_rejects, 1ull);
-      atomicOr((unsigned long long*)&d.ctr->error, 2ull);
-    }
+    if (count_stats) atomicAdd((unsigned long long*)&d.ctr->overflow_rejects, 1ull);
+    if (mode != kMarkSilent) atomicOr((unsigned long long*)&d.ctr->error, 2ull);
     return;
   }
   Cand cd;
@@ -392,14 +513,15 @@ __device__ __noinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va,
   // force/move pass, belongs to a vertex of these four cells: flag them, so that force_move can
   // run the flips while the untouched vertices already move.
   if (count_stats && k.flag_dirty) {
+    unsigned int* __restrict__ dirty = d.dirty + (size_t)parity * (size_t)k.nw;   // this step's bitmap
 #pragma unroll
     for (int t = 0; t < 4; ++t) {
       const int e[8] = {q[t][0].x, q[t][0].y, q[t][0].z, q[t][0].w, q[t][1].x, q[t][1].y, q[t][1].z, q[t][1].w};
 #pragma unroll
-      for (int j = 0; j < 8; ++j) atomicOr(&d.dirty[e[j] >> 5], 1u << (e[j] & 31));   // padding repeats entry 0
+      for (int j = 0; j < 8; ++j) atomicOr(&dirty[e[j] >> 5], 1u << (e[j] & 31));   // padding repeats entry 0
       for (int j = 8; j < nq[t]; ++j) {
         const int u = row_entry(d.cv, k.N, quad[t], j);
-        atomicOr(&d.dirty[u >> 5], 1u << (u & 31));
+        atomicOr(&dirty[u >> 5], 1u << (u & 31));
       }
     }
   }
@@ -414,7 +536,7 @@ __device__ __noinline__ void t1_report_cell(const Dev& d, const Consts& k, int c
     const int j = __ffs(smask);     // edge (j-1) -> (j mod n)
     smask &= smask - 1u;
     const int va = row_entry(d.cv, k.N, c, j - 1), vb = row_entry(d.cv, k.N, c, j == n ? 0 : j);
-    if (va < vb) t1_mark_edge(d, k, va, vb, parity, true);
+    if (va < vb) t1_mark_edge(d, k, va, vb, parity, kMarkFirstPass);
   }
 }
 
@@ -441,7 +563,17 @@ cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts
   pdl_launch_dependents();
   pdl_wait();
   const int gid = blockIdx.x * kCellBlock + threadIdx.x;
-  if (kStep && gid == 0) { d.ctr->flip_done = 0; d.ctr->next_cand = 0; d.ctr->next_quad = 0; }   // the previous list is long done
+  if (kStep && gid == 0) { d.ctr->flip_done = 0; d.ctr->next_cand = 0; }   // the previous list is long done
+#ifdef AVM_TRACE
+  if (kStep && gid == 0) {
+    const unsigned long long t0 = d.ctr->tr[0];
+    if (t0 != ~0ull) { for (int i = 1; i < 8; ++i) if (d.ctr->tr[i] > t0) d.ctr->tr_acc[i] += d.ctr->tr[i] - t0; d.ctr->tr_acc[0] += 1; }
+    d.ctr->tr[0] = ~0ull;
+    for (int i = 1; i < 8; ++i) d.ctr->tr[i] = 0;
+  }
+#endif
+  // the bitmap the force/move launch of this step swept with is spent: clear it for the next step's cell pass
+  if (kStep && k.clear_dirty && gid < k.nw) d.dirty[(size_t)(parity ^ 1u) * (size_t)k.nw + gid] = 0u;
   const bool valid = gid < k.N;
   const int c = valid ? k.N - 1 - gid : 0;
   const double2* __restrict__ pos = d.pos;
@@ -536,7 +668,7 @@ __global__ void detect_mark_kernel(const __grid_constant__ Dev d, const __grid_c
       // cheap pre-test; t1_mark_edge repeats the canonical one
       const double2 q = d.pos[w];
       const double dx = min_image(q.x - h.x, k.Lx, k.hLx), dy = min_image(q.y - h.y, k.Ly, k.hLy);
-      if (dx * dx + dy * dy < k.lc2) t1_mark_edge(d, k, v, w, parity, count_stats);
+      if (dx * dx + dy * dy < k.lc2) t1_mark_edge(d, k, v, w, parity, count_stats ? kMarkFirstPass : kMarkSilent);
     }
   }
 }
@@ -594,39 +726,75 @@ t1_local_detect_kernel(const __grid_constant__ Dev d, const __grid_constant__ Co
         if (atomicExch(&d.estamp[(size_t)oslot * k.Vs + owner], stamp) == stamp) continue;   // tested in this pass already
         const double2 hw = d.pos[wv];
         const double dx = min_image(hw.x - hu.x, k.Lx, k.hLx), dy = min_image(hw.y - hu.y, k.Ly, k.hLy);
-        if (dx * dx + dy * dy < k.lc2) t1_mark_edge(d, k, owner, other, list_new, false);
+        if (dx * dx + dy * dy < k.lc2) t1_mark_edge(d, k, owner, other, list_new, kMarkRepeatedPass);
       }
     }
   }
 }
 
 // ---------------------------------------------------------------------------------------------
-// rows a6 (deciding half) + a7: flip + rewrite (R9 geometry, R12 lists), one WARP per candidate.
-// A candidate flips iff its key is the minimum recorded on all four of its cells (R11); winners
-// therefore own disjoint cell quadruples and every word written below belongs to a vertex or row
-// inside the winner's own quadruple.  minkey is only read here (cleared by the next force_move).
+// rows a6 (deciding half) + a7: flip + rewrite (R9 geometry, R12 lists).  FOUR LANES per candidate:
+// lane t of a group owns cell t of the candidate's quadruple (L, R, E1, E2), so a warp carries
+// eight candidates at once.  A candidate flips iff its key is the minimum recorded on all four of
+// its cells (R11); winners therefore own disjoint cell quadruples and every word written below
+// belongs to a vertex or row inside the winner's own quadruple.  minkey is only read here.
+// Handles candidates base .. base+7 (< n) of `list`; returns how many of them flipped (warp-uniform).
+// Used by the stand-alone T1 kernel and by the flippers of the fused force_move launch.
 // ---------------------------------------------------------------------------------------------
-// One candidate, one warp: decide (R11) and, if it wins, flip and rewrite (R9, R12).  Returns
-// whether the edge flipped.  Used by the stand-alone T1 kernel and by force_move's fused prologue.
-__device__ __noinline__ bool t1_try_flip(const Dev& d, const Consts& k, const Cand& c, const int lane) {
-  const int cells[4] = {c.cL, c.cR, c.cE1, c.cE2};
-  const int l4 = lane & 3;
-  // ---- everything is read before anything is written; the loads below are independent of
-  // one another (the marking thread decoded the neighbourhood), so the minimum-key test
-  // costs no extra round trip ----
-  const unsigned long long mk = d.minkey[l4 == 0 ? c.cL : l4 == 1 ? c.cR : l4 == 2 ? c.cE1 : c.cE2];
-  const int v1 = c.v1, v2 = c.v2, k1 = c.k1, k2 = c.k2;
-  const int a1 = (k1 + 1) % 3, b1 = (k1 + 2) % 3, a2 = (k2 + 1) % 3, b2 = (k2 + 2) % 3;
-  const double2 h1 = d.pos[v1], h2 = d.pos[v2];
-  const int x1 = c.x1, y1 = c.y1, x2 = c.x2, y2 = c.y2;
-  int row[4], nrow[4];
-#pragma unroll
-  for (int t = 0; t < 4; ++t) {
-    nrow[t] = d.cvn[cells[t]];
-    row[t] = row_entry(d.cv, k.N, cells[t], lane < k.S ? lane : 0);
+// kR = number of row entries held per lane: 16 (rows live in registers, every index is static and
+// all loads of a phase are in flight together) for S <= 16, 32 (a local array) for larger strides.
+template <int kR>
+__device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Consts& k, const Cand* __restrict__ list,
+                                                       const unsigned base, const unsigned n, const int lane_in) {
+  const int lane = lane_in & 31;
+#ifdef AVM_TRACE
+  const bool trq = (lane_in & 0x100) != 0;
+#endif
+  const int t = lane & 3;
+  const unsigned i = base + (unsigned)(lane >> 2);
+  const bool have = i < n;
+  // ---- everything is read before anything is written; the loads of a phase are independent of
+  // one another (the marking thread decoded the neighbourhood), so the decision costs no extra
+  // round trip: phase 1 = the candidate, phase 2 = keys, rows and the two end points
+  int4 ca = make_int4(0, 0, 0, 0), cb = ca, cc = ca, cd = ca;
+#ifdef AVM_TRACE
+  unsigned long long tq0 = 0;
+  const unsigned long long tqe = gtime();
+  if (trq && blockIdx.x == 0 && threadIdx.x < 32) d.ctr->tr2[16 + threadIdx.x] = 0, d.ctr->tr2[48 + threadIdx.x] = 0;
+  if (trq && blockIdx.x == 0 && threadIdx.x == 0) d.ctr->tr2[7] = tqe;
+#endif
+  AVM_TR_W0(0, 0);
+  if (have) {
+    const int4* __restrict__ src = reinterpret_cast<const int4*>(list + i);
+    ca = __ldcg(src); cb = __ldcg(src + 1); cc = __ldcg(src + 2); cd = __ldcg(src + 3);
   }
-  if (!__all_sync(kFull, mk == c.key)) return false;
-  // ---- geometry: rigid counter-clockwise quarter turn about the midpoint, new length 1.5 l_c (R9)
+  AVM_TR_W0(1, ca.x + cb.x + cc.x + cd.x);
+  const int v1 = ca.x, v2 = ca.y, k1 = ca.z, k2 = ca.w;
+  const int cL = cb.x, cR = cb.y, cE1 = cb.z, cE2 = cb.w;
+  const unsigned long long key = ((unsigned long long)(unsigned)cc.y << 32) | (unsigned)cc.x;
+  const int sx1 = cc.z, sx2 = cc.w;
+  const int x1 = cd.x, y1 = cd.y, x2 = cd.z, y2 = cd.w;
+  const int cell = t == 0 ? cL : t == 1 ? cR : t == 2 ? cE1 : cE2;     // 0 for idle groups: a valid index
+  const unsigned long long mk = d.minkey[cell];
+  const int nrow = d.cvn[cell];
+  const double2 h1 = d.pos[v1], h2 = d.pos[v2];
+  int r[kR];
+#pragma unroll
+  for (int q = 0; q < kR / 4; ++q) {
+    int4 e = make_int4(0, 0, 0, 0);
+    if (4 * q < k.S) e = d.cv[(size_t)q * k.N + cell];
+    r[4 * q] = e.x; r[4 * q + 1] = e.y; r[4 * q + 2] = e.z; r[4 * q + 3] = e.w;
+  }
+  const unsigned agree = __ballot_sync(kFull, have && mk == key);
+  const unsigned wins = __ballot_sync(kFull, ((agree >> (lane & ~3)) & 0xfu) == 0xfu);
+  const unsigned nflips = (unsigned)__popc(wins & 0x11111111u);
+  AVM_TR_W0(2, (int)wins + r[0] + r[4] + r[8] + r[12] + nrow + (int)h1.x + (int)h2.x);
+#ifdef AVM_TRACE
+  if (trq && blockIdx.x == 0 && threadIdx.x < 32) d.ctr->tr2[16 + threadIdx.x] = gtime() - tqe + (((int)wins + r[0] + r[4] + r[8] + r[12] + nrow + (int)h1.x + (int)h2.x) & 0);
+#endif
+  if (!((wins >> lane) & 1u)) return nflips;
+  // ---- geometry: rigid counter-clockwise quarter turn about the midpoint, new length 1.5 l_c (R9);
+  // every lane of the group evaluates it (same bits) because each needs both new positions below
   const double dx = min_image(h2.x - h1.x, k.Lx, k.hLx), dy = min_image(h2.y - h1.y, k.Ly, k.hLy);
   const double l = sqrt(dx * dx + dy * dy);
   const double mx = h1.x + 0.5 * dx, my = h1.y + 0.5 * dy;
@@ -635,100 +803,99 @@ __device__ __noinline__ bool t1_try_flip(const Dev& d, const Consts& k, const Ca
   const double half = 0.75 * k.lc;
   const double2 n2 = make_double2(wrap_box(mx + half * px, k.Lx), wrap_box(my + half * py, k.Ly));
   const double2 n1 = make_double2(wrap_box(mx - half * px, k.Lx), wrap_box(my - half * py, k.Ly));
-  if (lane == 0) {
-    d.pos[v2] = n2;
+  // ---- lists: u = ([w, x, y]; [C0, C1, C2]) cyclic from the partner slot
+  //          -> ([w, y, z]; [C1, C2, C']), z = partner's old x, C' = partner's old C1 (R12);
+  // outer vertices: x1 was joined to v1 and is now joined to v2 (same slot), x2 likewise.
+  // Lane 0 rewrites v1, lane 1 v2, lane 2 x1, lane 3 x2.
+  if (t == 0) {
+    const int a1 = (k1 + 1) % 3, b1 = (k1 + 2) % 3;
     d.pos[v1] = n1;
-    // lists: u = ([w, x, y]; [C0, C1, C2]) cyclic from the partner slot
-    //     -> ([w, y, z]; [C1, C2, C']), z = partner's old x, C' = partner's old C1 (R12)
     d.vn[a1 * k.Vs + v1] = y1; d.vn[b1 * k.Vs + v1] = x2;
-    d.vc[k1 * k.Vs + v1] = c.cE1; d.vc[a1 * k.Vs + v1] = c.cR; d.vc[b1 * k.Vs + v1] = c.cE2;
+    d.vc[k1 * k.Vs + v1] = cE1; d.vc[a1 * k.Vs + v1] = cR; d.vc[b1 * k.Vs + v1] = cE2;
+  } else if (t == 1) {
+    const int a2 = (k2 + 1) % 3, b2 = (k2 + 2) % 3;
+    d.pos[v2] = n2;
     d.vn[a2 * k.Vs + v2] = y2; d.vn[b2 * k.Vs + v2] = x1;
-    d.vc[k2 * k.Vs + v2] = c.cE2; d.vc[a2 * k.Vs + v2] = c.cL; d.vc[b2 * k.Vs + v2] = c.cE1;
+    d.vc[k2 * k.Vs + v2] = cE2; d.vc[a2 * k.Vs + v2] = cL; d.vc[b2 * k.Vs + v2] = cE1;
+  } else if (t == 2) {
+    d.vn[sx1 * k.Vs + x1] = v2;
+  } else {
+    d.vn[sx2 * k.Vs + x2] = v1;
   }
-  // outer vertices: x1 was joined to v1 and is now joined to v2 (same slot); x2 likewise
-  if (lane == 1) d.vn[c.sx1 * k.Vs + x1] = v2;
-  if (lane == 2) d.vn[c.sx2 * k.Vs + x2] = v1;
-  // rows (lane = row entry): L deletes v1, R deletes v2 (later entries shift down); E1 inserts
-  // v2 immediately after v1, E2 inserts v1 immediately after v2 (later entries shift up).
-  // The new rows are formed in registers, written back, and reused by the refresh below.
-  int nnew[4];
+  __syncwarp(wins);     // reconverge: the four lanes of a group must issue the loads below together
+  // ---- my row: L deletes v1, R deletes v2 (later entries shift down); E1 inserts v2 immediately
+  // after v1, E2 inserts v1 immediately after v2 (later entries shift up); padding repeats entry 0.
+  // All indices are static so that the row stays in registers.
+  const int mark = (t & 1) ? v2 : v1;             // L, E1 look for v1; R, E2 look for v2
+  const int ins = t == 2 ? v2 : v1;
+  int p = 0;
 #pragma unroll
-  for (int t = 0; t < 4; ++t) {
-    int r = row[t];
-    if (t < 2) {
-      const int victim = t == 0 ? v1 : v2;
-      const int p = __ffs(__ballot_sync(kFull, lane < nrow[t] && r == victim)) - 1;
-      const int nxt = __shfl_down_sync(kFull, r, 1);
-      nnew[t] = nrow[t] - 1;
-      if (lane >= p) r = nxt;
-    } else {
-      const int after = t == 2 ? v1 : v2, ins = t == 2 ? v2 : v1;
-      const int p = __ffs(__ballot_sync(kFull, lane < nrow[t] && r == after)) - 1;
-      const int prv = __shfl_up_sync(kFull, r, 1);
-      nnew[t] = nrow[t] + 1;
-      if (lane > p) r = lane == p + 1 ? ins : prv;
-    }
-    const int r0 = __shfl_sync(kFull, r, 0);
-    if (lane >= nnew[t]) r = r0;                         // padding repeats entry 0
-    if (lane < k.S && r != row[t]) row_entry(d.cv, k.N, cells[t], lane) = r;
-    if (lane == 0) d.cvn[cells[t]] = nnew[t];
-    row[t] = r;
+  for (int j = kR - 1; j >= 0; --j) if (j < nrow && r[j] == mark) p = j;
+  int nnew;
+  if (t < 2) {
+#pragma unroll
+    for (int j = 0; j < kR - 1; ++j) if (j >= p) r[j] = r[j + 1];
+    nnew = nrow - 1;
+  } else {
+#pragma unroll
+    for (int j = kR - 1; j > 0; --j) if (j > p + 1) r[j] = r[j - 1];      // nrow < S (R10): nothing falls off
+#pragma unroll
+    for (int j = 1; j < kR; ++j) if (j == p + 1) r[j] = ins;
+    nnew = nrow + 1;
   }
-  // refresh the cached geometry of the four cells (directors unchanged): every lane fetches
-  // the position of "its" entry of each row (v1 and v2 take their new positions from
-  // registers), then the warp runs the same serial sum as the per-step pass, so that a resumed
-  // run reproduces these records bit for bit.  Lane t keeps cell t's result.
-  double2 hr[4];
+  __syncwarp(wins);
+  const int e0 = r[0];
 #pragma unroll
-  for (int t = 0; t < 4; ++t) {
-    hr[t] = make_double2(0.0, 0.0);
-    const int v = row[t];
-    if (lane < nnew[t]) hr[t] = v == v1 ? n1 : v == v2 ? n2 : d.pos[v];
-  }
-  // lane j holds entry j of each row: unwrapped position (ux, uy) and the length of the edge
-  // that ENDS at entry j (lane 0: the closing edge), computed in parallel with geom_edge's
-  // arithmetic; the order-dependent sums then run as four interleaved serial chains.
-  double ux[4], uy[4], sl[4];
-  int nmax = 0;
+  for (int j = 1; j < kR; ++j) if (j >= nnew) r[j] = e0;
 #pragma unroll
-  for (int t = 0; t < 4; ++t) {
-    const double h0x = __shfl_sync(kFull, hr[t].x, 0), h0y = __shfl_sync(kFull, hr[t].y, 0);
-    ux[t] = min_image(__dsub_rn(hr[t].x, h0x), k.Lx, k.hLx);
-    uy[t] = min_image(__dsub_rn(hr[t].y, h0y), k.Ly, k.hLy);
-    const int prev = lane == 0 ? nnew[t] - 1 : lane - 1;
-    const double pxv = __shfl_sync(kFull, ux[t], prev), pyv = __shfl_sync(kFull, uy[t], prev);
-    const double dx = __dsub_rn(ux[t], pxv), dy = __dsub_rn(uy[t], pyv);
-    sl[t] = sqrt_pos(__fma_rn(dx, dx, __fma_rn(dy, dy, kTiny)));
-    nmax = max(nmax, nnew[t]);
-  }
-  double rxp[4] = {0.0, 0.0, 0.0, 0.0}, ryp[4] = {0.0, 0.0, 0.0, 0.0}, acc[4] = {0.0, 0.0, 0.0, 0.0},
-         per[4] = {0.0, 0.0, 0.0, 0.0};
-  for (int j = 1; j <= nmax; ++j) {
+  for (int q = 0; q < kR / 4; ++q)
+    if (4 * q < k.S) d.cv[(size_t)q * k.N + cell] = make_int4(r[4 * q], r[4 * q + 1], r[4 * q + 2], r[4 * q + 3]);
+  d.cvn[cell] = nnew;
+  AVM_TR_W0(3, nnew);
+  // ---- refresh the cached geometry of my cell (directors unchanged): the same serial sum as the
+  // per-step pass (geom_edge), so that a resumed run reproduces these records bit for bit.  v1 and
+  // v2 take their new positions from registers; positions are fetched eight at a time (entries
+  // beyond the row repeat entry 0, whose position is substituted without a load).
+  const double2 h0 = e0 == v1 ? n1 : e0 == v2 ? n2 : d.pos[e0];
+  double rxp = 0.0, ryp = 0.0, acc = 0.0, per = 0.0;
 #pragma unroll
-    for (int t = 0; t < 4; ++t) {
-      if (j <= nnew[t]) {                          // warp-uniform
-        const int src = j < nnew[t] ? j : 0;       // j == n: the closing edge back to entry 0 (r = 0)
-        const double x = __shfl_sync(kFull, ux[t], src), y = __shfl_sync(kFull, uy[t], src);
-        const double l = __shfl_sync(kFull, sl[t], src);
-        acc[t] = __fma_rn(rxp[t], y, acc[t]);
-        acc[t] = __fma_rn(-ryp[t], x, acc[t]);
-        per[t] = __dadd_rn(per[t], l);
-        rxp[t] = x; ryp[t] = y;
+  for (int j0 = 1; j0 < kR; j0 += 8) {
+    if (j0 < nnew) {
+      double2 hh[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        hh[u] = h0;
+        if (j0 + u < kR) {
+          const int e = r[j0 + u < kR ? j0 + u : 0];
+          if (j0 + u < nnew) hh[u] = e == v1 ? n1 : e == v2 ? n2 : d.pos[e];
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        if (j0 + u < nnew) {
+          const double rx = min_image(__dsub_rn(hh[u].x, h0.x), k.Lx, k.hLx);
+          const double ry = min_image(__dsub_rn(hh[u].y, h0.y), k.Ly, k.hLy);
+          geom_edge(rxp, ryp, rx, ry, acc, per);
+          rxp = rx; ryp = ry;
+        }
       }
     }
   }
-  double myA = 0.0, myP = 0.0;
-#pragma unroll
-  for (int t = 0; t < 4; ++t)
-    if (lane == t) { myA = __dmul_rn(0.5, acc[t]); myP = per[t]; }
-  if (lane < 4) {
-    const int cc = cells[lane == 0 ? 0 : lane == 1 ? 1 : lane == 2 ? 2 : 3];
-    const double2 tg = cell_targets(d, k, cc);
-    d.rec[cc].a = k.KA2 * (myA - tg.x);
-    d.rec[cc].p = k.KP2 * (myP - tg.y);
-  }
-  __syncwarp();
-  return true;
+  geom_edge(rxp, ryp, 0.0, 0.0, acc, per);      // the closing edge back to entry 0
+  AVM_TR_W0(4, (int)acc);
+  const double2 tg = cell_targets(d, k, cell);
+  d.rec[cell].a = k.KA2 * (__dmul_rn(0.5, acc) - tg.x);
+  d.rec[cell].p = k.KP2 * (per - tg.y);
+  AVM_TR_W0(5, 0);
+#ifdef AVM_TRACE
+  if (trq && blockIdx.x == 0 && threadIdx.x < 32) d.ctr->tr2[48 + threadIdx.x] = gtime() - tqe;
+  if (trq && blockIdx.x == 0 && threadIdx.x == 0) d.ctr->tr2[8] = gtime();
+#endif
+  return nflips;
+}
+__device__ __noinline__ unsigned t1_flip_quads(const Dev& d, const Consts& k, const Cand* __restrict__ list, const unsigned base,
+                                               const unsigned n, const int lane) {
+  return k.S <= 16 ? t1_flip_quads_impl<16>(d, k, list, base, n, lane) : t1_flip_quads_impl<32>(d, k, list, base, n, lane);
 }
 
 __global__ void __launch_bounds__(kT1Block)
@@ -740,14 +907,14 @@ t1_flip_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, 
   const int lane = threadIdx.x & 31;
   const unsigned gwarp = (blockIdx.x * kT1Block + threadIdx.x) >> 5, nwarps = (gridDim.x * kT1Block) >> 5;
   if (count_stats && gwarp == 0 && lane == 0 && n_cand) atomicAdd((unsigned long long*)&d.ctr->t1_candidates, (unsigned long long)n_cand);
-  unsigned int flips = 0, blocked = 0;
-  for (unsigned int i = gwarp; i < n_cand; i += nwarps) {
-    const Cand c = list[i];
-    if (t1_try_flip(d, k, c, lane)) ++flips; else ++blocked;
+  unsigned int flips = 0, seen = 0;
+  for (unsigned int i = gwarp * 8u; i < n_cand; i += nwarps * 8u) {
+    flips += t1_flip_quads(d, k, list, i, n_cand, lane);
+    seen += min(8u, n_cand - i);
   }
   if (count_stats && lane == 0) {
     if (flips) atomicAdd((unsigned long long*)&d.ctr->t1_flips, (unsigned long long)flips);
-    if (blocked) atomicAdd((unsigned long long*)&d.ctr->t1_blocked, (unsigned long long)blocked);
+    if (seen - flips) atomicAdd((unsigned long long*)&d.ctr->t1_blocked, (unsigned long long)(seen - flips));
   }
 }
 
@@ -762,7 +929,7 @@ t1_reset_kernel(const Dev d, const unsigned cap) {
     d.minkey[c.cL] = ~0ull; d.minkey[c.cR] = ~0ull; d.minkey[c.cE1] = ~0ull; d.minkey[c.cE2] = ~0ull;
   }
 }
-__global__ void zero_counts_kernel(const Dev d) { d.ctr->n_cand[0] = 0; d.ctr->n_cand[1] = 0; d.ctr->n_cand[2] = 0; d.ctr->n_cand[3] = 0; d.ctr->n_win = 0; d.ctr->flip_done = 0; d.ctr->next_cand = 0; d.ctr->next_quad = 0; }
+__global__ void zero_counts_kernel(const Dev d) { d.ctr->n_cand[0] = 0; d.ctr->n_cand[1] = 0; d.ctr->n_cand[2] = 0; d.ctr->n_cand[3] = 0; d.ctr->n_win = 0; d.ctr->flip_done = 0; d.ctr->next_cand = 0; }
 
 // debug hook: winners without flipping; (tag_min, tag_max) pairs out
 __global__ void t1_debug_kernel(const Dev d, int* cand_pairs, int* win_pairs, long long capacity) {
@@ -879,75 +1046,79 @@ __global__ void philox_words_kernel(unsigned long long seed, unsigned long long 
 // ---------------------------------------------------------------------------------------------
 static inline int cdiv(long long a, int b) { return (int)((a + b - 1) / b); }
 
-static int force_move_grid(const Consts& k) {
-  // persistent: a whole number of CTAs per SM (148 SMs), never more CTAs than there is work
-  static int per_sm = 0;
-  if (!per_sm) {
-    int a = 0, b = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, force_move_kernel<true>, kVertexBlock, 0);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, force_move_kernel<false>, kVertexBlock, 0);
-    per_sm = a < b ? a : b;
-    if (per_sm < 1) per_sm = 1;
-  }
-  const int want = cdiv(k.V, kVertexBlock);
-  const int cap = 148 * per_sm;
+// Grid of the persistent force/move kernel: a whole number of CTAs per SM of the current device,
+// never more CTAs than there is work.  Called once per simulation (avm_create); the result lives
+// in Consts::fm_grid.
+int force_move_grid(int V) {
+  int a = 0, b = 0, dev = 0, sms = 148;
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, force_move_kernel<true>, kVertexBlock, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, force_move_kernel<false>, kVertexBlock, 0);
+  int per_sm = a < b ? a : b;
+  if (per_sm < 1) per_sm = 1;
+  if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  const int want = cdiv(V, kVertexBlock);
+  const int cap = sms * per_sm;
   return want < cap ? want : cap;
 }
 
-// Launch with the programmatic-stream-serialization attribute (see pdl_wait above) and,
-// optionally, as a cooperative grid (every CTA resident: force_move<true> spins on a counter
-// that other CTAs advance).
+// Launch with the programmatic-stream-serialization attribute (see pdl_wait above).
 template <typename... KArgs, typename... Args>
-static cudaError_t launch_chained(void (*kernel)(KArgs...), int grid, int block, cudaStream_t s, bool pdl, bool coop,
-                                  Args... args) {
+static cudaError_t launch_chained(void (*kernel)(KArgs...), int grid, int block, cudaStream_t s, bool pdl, Args... args) {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block); cfg.dynamicSmemBytes = 0; cfg.stream = s;
-  cudaLaunchAttribute attr[2];
+  cudaLaunchAttribute attr[1];
   int na = 0;
   if (pdl) { attr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization; attr[na].val.programmaticStreamSerializationAllowed = 1; ++na; }
-  if (coop) { attr[na].id = cudaLaunchAttributeCooperative; attr[na].val.cooperative = 1; ++na; }
   cfg.attrs = attr; cfg.numAttrs = (unsigned)na;
   return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
 // One timestep.  d.pos = positions at the start of the step, d.pos_next = buffer for the moved
 // positions (the caller swaps them afterwards).
-//   fused = true : two launches; the T1 flips of the PREVIOUS step ride in force_move's
-//                  prologue, those of this step stay pending (launch_t1_flush applies them).
-//   fused = false: three launches, each step complete on return (also the per-kernel timing mode).
+//   consume_pending: the previous step left its T1 flips pending; they ride in this force/move launch.
+//   leave_pending  : this step leaves its own flips pending (two launches) instead of running the
+//                    stand-alone T1 kernel (three launches, the step complete on return).
 // ev (optional, AVM_K_COUNT+1 events): recorded before/after each kernel by avm_step_profile.
-int launch_step(const Dev& d, const Consts& k, unsigned long long step, cudaStream_t s, cudaEvent_t* ev, bool fused) {
+int launch_step(const Dev& d, const Consts& k, unsigned long long step, cudaStream_t s, cudaEvent_t* ev, bool consume_pending,
+                bool leave_pending) {
   const unsigned parity = (unsigned)(step & 1ull);
   if (ev) cudaEventRecord(ev[0], s);
   const bool pdl = AVM_PDL && ev == nullptr;   // events between the kernels would break the chain anyway
-  static int coop_pdl_ok = 1;                  // cooperative + programmatic launch accepted by this driver?
-  if (fused) {
-    cudaError_t e = cudaErrorUnknown;
-    if (pdl && coop_pdl_ok) {
-      e = launch_chained(force_move_kernel<true>, force_move_grid(k), kVertexBlock, s, true, AVM_FM_COOP != 0, d, k, parity);
-      if (e != cudaSuccess) { coop_pdl_ok = 0; cudaGetLastError(); if (getenv("AVM_B200_DEBUG")) fprintf(stderr, "avm: cooperative+programmatic launch rejected\n"); }
-    }
-    if (e != cudaSuccess) e = launch_chained(force_move_kernel<true>, force_move_grid(k), kVertexBlock, s, false, AVM_FM_COOP != 0, d, k, parity);
-    if (e != cudaSuccess) return -1;           // the caller falls back to the unfused schedule
-  } else {
-    launch_chained(force_move_kernel<false>, force_move_grid(k), kVertexBlock, s, pdl, false, d, k, parity);
-  }
+  if (consume_pending) launch_chained(force_move_kernel<true>, k.fm_grid, kVertexBlock, s, pdl, d, k, parity);
+  else launch_chained(force_move_kernel<false>, k.fm_grid, kVertexBlock, s, pdl, d, k, parity);
   if (ev) cudaEventRecord(ev[1], s);
   Dev m = d;                      // from here on the moved positions are "the" positions
   m.pos = d.pos_next; m.pos_next = d.pos;
-  if (k.per_cell) launch_chained(cell_update_kernel<true, true>, cdiv(k.N, kCellBlock), kCellBlock, s, pdl, false, m, k, step, parity);
-  else launch_chained(cell_update_kernel<true, false>, cdiv(k.N, kCellBlock), kCellBlock, s, pdl, false, m, k, step, parity);
+  Consts kc = k;
+  kc.flag_dirty = leave_pending ? 1 : 0;       // the flagged-vertex bitmap is only needed when the flips stay pending
+  kc.clear_dirty = consume_pending ? 1 : 0;    // the bitmap this step's force/move launch swept with is spent
+  if (k.per_cell) launch_chained(cell_update_kernel<true, true>, cdiv(k.N, kCellBlock), kCellBlock, s, pdl, m, kc, step, parity);
+  else launch_chained(cell_update_kernel<true, false>, cdiv(k.N, kCellBlock), kCellBlock, s, pdl, m, kc, step, parity);
   if (ev) cudaEventRecord(ev[2], s);
-  if (!fused) launch_chained(t1_flip_kernel, kT1Grid, kT1Block, s, pdl, false, m, k, parity, true);
+  if (!leave_pending) launch_chained(t1_flip_kernel, kT1Grid, kT1Block, s, pdl, m, k, parity, true);
   if (ev) cudaEventRecord(ev[3], s);
-  return fused ? 2 : 3;
+  return leave_pending ? 2 : 3;
 }
 
-// Applies the flips a fused step left pending (d = the state after that step) and leaves the T1
-// work lists idle, so that any other entry point sees a complete step.
-int launch_t1_flush(const Dev& d, const Consts& k, unsigned long long last_step, cudaStream_t s) {
-  t1_flip_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, k, (unsigned)(last_step & 1ull), true);
-  return 1 + launch_t1_reset(d, k, s);
+// number of edges shorter than l_c in the current state -> ctr->n_win (creation: first guess of the T1 load)
+__global__ void count_short_edges_kernel(const Dev d, const Consts k) {
+  const int v = blockIdx.x * blockDim.x + threadIdx.x;
+  if (v >= k.V) return;
+  const double2 h = d.pos[v];
+  int n = 0;
+  for (int s = 0; s < 3; ++s) {
+    const int w = d.vn[s * k.Vs + v];
+    if (v < w) {
+      const double2 q = d.pos[w];
+      const double dx = min_image(q.x - h.x, k.Lx, k.hLx), dy = min_image(q.y - h.y, k.Ly, k.hLy);
+      n += dx * dx + dy * dy < k.lc2;
+    }
+  }
+  if (n) atomicAdd(&d.ctr->n_win, (unsigned)n);
+}
+int launch_count_short_edges(const Dev& d, const Consts& k, cudaStream_t s) {
+  count_short_edges_kernel<<<cdiv(k.V, 256), 256, 0, s>>>(d, k);
+  return 1;
 }
 
 int launch_refresh_cells(const Dev& d, const Consts& k, cudaStream_t s) {
@@ -960,7 +1131,7 @@ int launch_refresh_cells(const Dev& d, const Consts& k, cudaStream_t s) {
 int launch_t1_reset(const Dev& d, const Consts& k, cudaStream_t s) {
   t1_reset_kernel<<<kT1Grid, kT1Block, 0, s>>>(d, (unsigned)k.cap_a);
   zero_counts_kernel<<<1, 1, 0, s>>>(d);
-  cudaMemsetAsync(d.dirty, 0, sizeof(unsigned int) * (size_t)((k.V + 31) / 32), s);
+  cudaMemsetAsync(d.dirty, 0, sizeof(unsigned int) * 2 * (size_t)k.nw, s);
   return 2;
 }
 
@@ -973,15 +1144,15 @@ int launch_t1_pass_only(const Dev& d, const Consts& k, cudaStream_t s) {
 }
 
 int launch_t1_release(const Dev& d, const Consts& k, unsigned list, cudaStream_t s) {
-  launch_chained(t1_release_kernel, kT1Grid, kT1Block, s, AVM_PDL != 0, false, d, k, list, (int)list);
+  launch_chained(t1_release_kernel, kT1Grid, kT1Block, s, AVM_PDL != 0, d, k, list, (int)list);
   return 1;
 }
 
 int launch_t1_extra_pass(const Dev& d, const Consts& k, unsigned list_prev, unsigned list_new, unsigned stamp, cudaStream_t s) {
   const bool pdl = AVM_PDL != 0;     // part of the step's chain of dependent launches
-  launch_chained(t1_release_kernel, kT1Grid, kT1Block, s, pdl, false, d, k, list_prev, (int)list_new);
-  launch_chained(t1_local_detect_kernel, kT1Grid, kT1Block, s, pdl, false, d, k, list_prev, list_new, stamp);
-  launch_chained(t1_flip_kernel, kT1Grid, kT1Block, s, pdl, false, d, k, list_new, true);
+  launch_chained(t1_release_kernel, kT1Grid, kT1Block, s, pdl, d, k, list_prev, (int)list_new);
+  launch_chained(t1_local_detect_kernel, kT1Grid, kT1Block, s, pdl, d, k, list_prev, list_new, stamp);
+  launch_chained(t1_flip_kernel, kT1Grid, kT1Block, s, pdl, d, k, list_new, true);
   return 3;
 }
 

@@ -343,7 +343,7 @@ def test_full_size_configs_against_oracle(B, k, steps):
     _TILINGS.pop(k, None)
 
 
-def test_two_launch_schedule_equals_three_launch_schedule(B, monkeypatch):
+def test_two_launch_schedule_equals_three_launch_schedule(B):
     """The default schedule applies the T1 flips of a step inside the next force/move launch
     (flagged vertices are moved after the flips); the plain schedule runs a third kernel per
     step.  Both must give the same bits, whatever the chunking of avm_step calls, including the
@@ -351,20 +351,16 @@ def test_two_launch_schedule_equals_three_launch_schedule(B, monkeypatch):
     t = tiling(1)
     p = dict(w.config_params(1), sort_every=7)
     keys = ("pos", "theta", "cell_vertices", "vertex_neighbors", "vertex_cell_neighbors", "cell_vertex_num")
-    monkeypatch.setenv("AVM_B200_FUSED", "1")      # small systems default to the three-launch schedule
-    a = B.from_tiling(t, **p)
+    a = B.from_tiling(t, schedule="fused", **p)     # small systems default to the three-launch schedule
     a.step(40)
     sa = to_np(a.get_state())
-    b = B.from_tiling(t, **p)
+    b = B.from_tiling(t, schedule="fused", **p)
     for n in (1, 1, 3, 5, 13, 17):
         b.step(n)
     sb = to_np(b.get_state())
-    monkeypatch.delenv("AVM_B200_FUSED")
-    monkeypatch.setenv("AVM_B200_UNFUSED", "1")
-    c = B.from_tiling(t, **p)
+    c = B.from_tiling(t, schedule="unfused", **p)
     c.step(40)
     sc = to_np(c.get_state())
-    monkeypatch.delenv("AVM_B200_UNFUSED")
     assert sa["stats"]["kernel_launches"] < sc["stats"]["kernel_launches"]
     for key in keys:
         assert np.array_equal(sa[key], sb[key]), f"chunking changes {key}: max diff {np.abs(sa[key] - sb[key]).max()}"
@@ -453,7 +449,7 @@ def test_long_run_at_the_config_length_keeps_every_invariant(B):
     assert np.array_equal(s1["pos"], s2["pos"]) and np.array_equal(s1["theta"], s2["theta"])
 
 
-def test_two_launch_schedule_at_full_size_equals_three_launch_schedule(B, monkeypatch):
+def test_two_launch_schedule_at_full_size_equals_three_launch_schedule(B):
     """configs[3] (N = 1,048,576, the bench workload) for 300 steps with a re-sort every 100: the
     default two-launch schedule — ~96 000 simultaneous candidates in step 0 (every warp flips),
     then a few dozen per step (a few flipper warps) — against the three-launch schedule, bit for bit."""
@@ -465,12 +461,10 @@ def test_two_launch_schedule_at_full_size_equals_three_launch_schedule(B, monkey
     area = a.compute_forces()[1][:, 0].sum().item()
     a.close()
     del a
-    monkeypatch.setenv("AVM_B200_UNFUSED", "1")
-    b = B.from_tiling(t, **p)
+    b = B.from_tiling(t, schedule="unfused", **p)
     b.step(300)
     sb = to_np(b.get_state())
     b.close()
-    monkeypatch.delenv("AVM_B200_UNFUSED")
     assert sa["stats"]["kernel_launches"] < sb["stats"]["kernel_launches"]
     for key in ("pos", "theta", "cell_vertices", "vertex_neighbors", "vertex_cell_neighbors", "cell_vertex_num"):
         assert np.array_equal(sa[key], sb[key]), key
@@ -537,13 +531,12 @@ def test_per_cell_targets_match_the_oracle(B, k, steps, sort_every):
 
 @pytest.mark.parametrize("S", [20, 32])
 @pytest.mark.parametrize("fused", [False, True])
-def test_other_row_strides_match_the_oracle(B, S, fused, monkeypatch):
+def test_other_row_strides_match_the_oracle(B, S, fused):
     """rows longer than 16 entries use different code (one row per pass in the flippers, planes
     4..7 of the padded rows, bit 31 of the short-edge mask): configs[1] geometry with S = 20 and
     the maximum S = 32, in both schedules, through the step-0 burst."""
-    monkeypatch.setenv("AVM_B200_FUSED" if fused else "AVM_B200_UNFUSED", "1")
     t = w.voronoi_tiling(4096, 64.0, 2, S=S)
-    p = w.config_params(1)
+    p = dict(w.config_params(1), schedule="fused" if fused else "unfused")
     g = B.from_tiling(t, **dict(p, sort_every=6, sort_at_create=True))
     o = oracle.from_tiling(t, **p)
     F, ap = g.compute_forces()
