@@ -6,6 +6,11 @@
 A "step" is one AVM timestep (all rows of the hot path) of one synthetic Voronoi tiling.
 value = vertex-updates/s = V * K / (device time of K steps), whole job over all ranks (multi-GPU =
 independent replicas, weak scaling, no collective on the data path).  Prints ONE JSON line.
+
+Besides the `--steps/--warmup` region (`value`, exactly as asked), the line carries `whole_run` and
+`second_half`: the config's nominal run (1000 steps for cfg3) timed from its
+initial state in two halves, because a Voronoi start opens with a burst of T1 transitions that
+decays over ~100 steps and the steady state is what a long run pays for.
 """
 from __future__ import annotations
 
@@ -23,14 +28,23 @@ import numpy as np
 
 METRIC = "AVM vertex-updates/s (= V x timesteps/s) at N cells"
 UNIT = "vertex-updates/s"
+NOMINAL_PEAK_GBS = 8000.0     # north_star: "B200 peak (about 8 TB/s)"
 
-# Algorithmic (compulsory, useful) bytes of the two dense kernels, DESIGN.md §Byte model:
+# Algorithmic (compulsory, useful) bytes of the two dense kernels, DESIGN.md §5:
 #   force_move : per vertex  pos 16 + vertexNeighbors 12 + vertexCellNeighbors 12 + pos_next 16,
 #                plus the cell records gathered once per cell: 32 B/cell = 16 B/vertex      -> 72 B/vertex
 #   cell_update: per cell    cellVertexNum 4 + tag 4 + theta 8+8 + record write 32 + row entries 4*6
 #                + positions gathered once per vertex 16 B/vertex = 32 B/cell             -> 112 B/cell
+# SURVEY.md §8(d)'s reference model of the same step: 134 B/vertex-step as stored.
 BYTES_FORCE_MOVE_PER_VERTEX = 72.0
 BYTES_CELL_UPDATE_PER_CELL = 112.0
+SURVEY_BYTES_PER_VERTEX_STEP = 134.0
+
+
+def workload_string(cfg, N, V):
+    return (f"{cfg['name']}: AVM N={N} cells, V={V}, L={cfg['L'] * (N / cfg['N']) ** 0.5:g}, periodic Voronoi of uniform points "
+            f"(seed {cfg['points_seed']}), p0={cfg['p0']}, v0={cfg['v0']}, Dr={cfg['Dr']}, dt={cfg['dt']}, "
+            f"l_c={cfg['l_c']}, Hilbert-sorted at create={cfg['sort_at_create']}, sort_every={cfg['sort_every']}")
 
 
 def measured_peaks():
@@ -77,7 +91,7 @@ class ClockSampler:
         except Exception:
             pass
 
-    def start(self, period_s: float = 0.004):
+    def start(self, period_s: float = 0.001):
         """sample from a background thread while the caller enqueues and waits (ctypes releases the GIL)"""
         import threading
         self._stop = threading.Event()
@@ -100,15 +114,17 @@ class ClockSampler:
                 "samples": len(self.sm)}
 
 
-def ncu_traffic(kernel: str, workload: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed ncu
-    capture (profiles/r1_v4_dram_traffic.csv; the command is in profiles/r1_v4_two_launch.md)."""
-    path = os.path.join(ROOT, "profiles", "r1_v4_dram_traffic.csv")
+def ncu_capture(kernel: str, workload: str):
+    """ncu figures of `kernel` from the committed capture (profiles/r2_ncu_kernels.csv; the commands, the
+    commit and the step range of each capture are in profiles/r2_ncu_kernels.md): DRAM bytes per
+    launch (dram__bytes_read.sum + dram__bytes_write.sum) and pipe utilisations.  Static evidence
+    read from a file, not measured in this run; the record says which capture it is."""
+    path = os.path.join(ROOT, "profiles", "r2_ncu_kernels.csv")
     try:
         import csv
         for row in csv.DictReader(open(path)):
             if row["kernel"] == kernel and row["workload"] == workload:
-                return float(row["dram_bytes_read_per_launch"]) + float(row["dram_bytes_write_per_launch"])
+                return row
     except Exception:
         pass
     return None
@@ -131,9 +147,15 @@ def aggregate_value(units_per_rank: float, steps: int, ms: float, world: int) ->
     return world * units_per_rank * steps / (ms * 1e-3)
 
 
+def bandwidth_fractions(bytes_per_step: float, ms_per_step: float, peak: float) -> dict:
+    gbs = bytes_per_step / (ms_per_step * 1e-3) / 1e9
+    return {"GBps": gbs, "frac_of_measured_peak": gbs / peak, "frac_of_nominal_8TBps": gbs / NOMINAL_PEAK_GBS}
+
+
 def run_reference(args):
-    """--impl reference: the CPU oracle as it stands, rank 0 only, on a bounded sample of the
-    workload (a smaller tiling of the same recipe and density) so that K+W steps end in minutes."""
+    """--impl reference: the CPU oracle as it stands, rank 0 only.  The full tiling of the config is
+    used whenever K+W steps of it end within the time budget; otherwise a smaller tiling of the same
+    recipe and density, and config.workload says which N really ran."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
@@ -142,7 +164,7 @@ def run_reference(args):
     cfg = w.CONFIGS[args.config]
     p = w.config_params(args.config)
     total = max(1, args.steps + args.warmup)
-    budget_cells = 100.0 / (total * 1.5e-6)              # ~1.5 us per cell-step on one core
+    budget_cells = 150.0 / (total * 1.5e-6)              # ~1.5 us per cell-step on one core, ~150 s in all
     Ns = cfg["N"]
     while Ns > 1024 and Ns > budget_cells:
         Ns //= 4
@@ -154,14 +176,15 @@ def run_reference(args):
     sim.step(args.steps)
     dt = time.perf_counter() - t0
     value = t.V * args.steps / dt
-    sample = f"{Ns}-cell tiling of the {cfg['name']} recipe (same density, parameters, seed), {args.steps} steps after {args.warmup}"
+    sample = (f"the oracle (oracle/avm_oracle.cpp, one thread) on {'the full' if Ns == cfg['N'] else 'a reduced'} {Ns}-cell tiling "
+              f"of the {cfg['name']} recipe, steps {args.warmup}..{args.warmup + args.steps - 1}")
     out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(1, args.steps),
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-           "config": {"workload": f"{cfg['name']}: AVM N={cfg['N']} cells, L={cfg['L']}, Voronoi seed {cfg['points_seed']}",
-                      "sample": sample},
+           "config": {"workload": workload_string(cfg, Ns, t.V), "cells_run": Ns, "cells_of_config": cfg["N"]},
            "timesteps_per_s": args.steps / dt,
-           "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+           "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                            "host_cpus": os.cpu_count()},
            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
            "gpu_launches": 0}
     print(json.dumps(out))
@@ -176,9 +199,12 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (kernel experiments only)")
-    ap.add_argument("--profile-steps", type=int, default=100)
+    ap.add_argument("--no-nominal-run", action="store_true", help="skip the whole_run / second_half records")
+    ap.add_argument("--profile-steps", type=int, default=0,
+                    help="steps of the per-kernel event pass (default: the timed region itself, at most 200 steps)")
     ap.add_argument("--t1-passes", type=int, default=1,
                     help="T1 passes per step: 1 = north_star's rule (default, the headline), P > 1 = repeat until none (NEXT-1)")
+    ap.add_argument("--schedule", default="auto", choices=["auto", "fused", "unfused"])
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
 
@@ -206,50 +232,105 @@ def main():
         torch.cuda.synchronize()
 
     cfg = w.CONFIGS[args.config]
-    p = dict(w.config_params(args.config), device=local_rank)
+    p = dict(w.config_params(args.config), device=local_rank, schedule=args.schedule)
     if args.t1_passes > 1:
         p["t1_max_passes"] = args.t1_passes
     t = w.config_tiling(args.config)
     N, V = t.N, t.V
+    peak, peak_src = measured_peaks()
+    kbytes = {"force_move": BYTES_FORCE_MOVE_PER_VERTEX * V, "cell_update": BYTES_CELL_UPDATE_PER_CELL * N}
+    step_bytes = sum(kbytes.values())
+    survey_step_bytes = SURVEY_BYTES_PER_VERTEX_STEP * V
+
+    def timed_steps(sim, n):
+        """device time of n steps (CUDA events on the stream the library launches on), clocks sampled meanwhile"""
+        sampler = ClockSampler(local_rank)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        sampler.start()
+        e0.record()
+        sim.step(n)
+        e1.record()
+        e1.synchronize()
+        sampler.stop()
+        barrier()
+        return max_over_ranks(e0.elapsed_time(e1), dist, "cuda"), sampler
+
+    def region_record(ms, n, first_step, st0, st1, sampler):
+        per = ms / n
+        return {"steps": f"{first_step}..{first_step + n - 1}", "ms_per_step": per,
+                "value": aggregate_value(V, n, ms, world), "unit": UNIT, "timesteps_per_s": n / (ms * 1e-3),
+                "t1_flips_per_step": (st1["t1_flips"] - st0["t1_flips"]) / n,
+                "bandwidth": {"bytes_model_this_repo_128B_per_vertex": bandwidth_fractions(step_bytes, per, peak),
+                              "bytes_model_survey_134B_per_vertex": bandwidth_fractions(survey_step_bytes, per, peak)},
+                "clocks": sampler.summary()}
 
     # ---------------- device-resident run: inputs already in HBM when the clock starts -----------
     sim = B.from_tiling(t, **p)
     sim.step(args.warmup)
     st0 = sim.stats()
-    sampler = ClockSampler(local_rank)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    sampler.start()
-    e0.record()
-    sim.step(args.steps)
-    e1.record()
-    e1.synchronize()
-    sampler.stop()
-    barrier()
-    ms = e0.elapsed_time(e1)
+    ms, sampler = timed_steps(sim, args.steps)
     st1 = sim.stats()
-    ms = max_over_ranks(ms, dist, "cuda")
     value = aggregate_value(V, args.steps, ms, world)
-
-    # ---------------- per-kernel device time (CUDA events inside the library) --------------------
-    prof = sim.step_profile(args.profile_steps)
-    peak, peak_src = measured_peaks()
-    per_launch_ms = {k: v / max(1, args.profile_steps) for k, v in prof.items()}
-    kbytes = {"force_move": BYTES_FORCE_MOVE_PER_VERTEX * V, "cell_update": BYTES_CELL_UPDATE_PER_CELL * N}
-    dom = max(kbytes, key=lambda k: per_launch_ms[k])
-    ach = kbytes[dom] / (per_launch_ms[dom] * 1e-3) / 1e9
-    step_bytes = sum(kbytes.values())
-    roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": ncu_traffic(dom, cfg["name"]), "peak_source": peak_src,
-                "timing": "CUDA events on the library's stream around every launch of a separate pass of "
-                          f"{args.profile_steps} steps (same schedule as the timed region, launches serialised by the events)",
-                "bytes_per_launch": kbytes[dom], "ms_per_launch": per_launch_ms[dom],
-                "kernels_ms_per_launch": per_launch_ms,
-                "step": {"algorithmic_bytes": step_bytes, "achieved_GBps": step_bytes / (ms / args.steps * 1e-3) / 1e9,
-                         "frac": step_bytes / (ms / args.steps * 1e-3) / 1e9 / peak}}
-    state_after = sim.stats()
+    state_after = st1
     sim.close()
     del sim
+
+    # ---------------- per-kernel device time over the SAME steps (CUDA events inside the library) -
+    # A fresh simulation repeats the warm-up (the run is deterministic), then avm_step_profile
+    # brackets every kernel of the timed steps with events; clocks are sampled during this pass too.
+    prof_steps = args.profile_steps if args.profile_steps > 0 else min(args.steps, 200)
+    simp = B.from_tiling(t, **p)
+    simp.step(args.warmup)
+    psampler = ClockSampler(local_rank)
+    torch.cuda.synchronize()
+    psampler.start()
+    prof = simp.step_profile(prof_steps)
+    torch.cuda.synchronize()
+    psampler.stop()
+    simp.close()
+    del simp
+    per_launch_ms = {k: v / max(1, prof_steps) for k, v in prof.items()}
+    dom = max(kbytes, key=lambda k: per_launch_ms[k])
+    ach = kbytes[dom] / (per_launch_ms[dom] * 1e-3) / 1e9
+    cap = ncu_capture(dom, cfg["name"])
+    traffic = (float(cap["dram_bytes_read_per_launch"]) + float(cap["dram_bytes_write_per_launch"])) if cap else None
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "frac_of_nominal_8TBps": ach / NOMINAL_PEAK_GBS,
+                "traffic": traffic,
+                "traffic_source": (f"ncu capture {cap['capture']} (commit {cap['commit']}, steps {cap['steps']}; profiles/r2_ncu_kernels.md), "
+                                   "not measured in this run") if cap else None,
+                "ncu": {k: cap[k] for k in cap if k not in ("kernel", "workload")} if cap else None,
+                "peak_source": peak_src,
+                "timing": f"CUDA events on the library's stream around every launch of steps {args.warmup}..{args.warmup + prof_steps - 1} "
+                          "of a second, identical run (same schedule decisions as the timed region; the events serialise the launches)",
+                "bytes_per_launch": kbytes[dom], "ms_per_launch": per_launch_ms[dom],
+                "kernels_ms_per_launch": per_launch_ms,
+                "kernels_frac_of_measured_peak": {k: kbytes[k] / (per_launch_ms[k] * 1e-3) / 1e9 / peak for k in kbytes if per_launch_ms[k] > 0},
+                "clocks_during_profile_pass": psampler.summary(),
+                "step": {"algorithmic_bytes": step_bytes, **bandwidth_fractions(step_bytes, ms / args.steps, peak),
+                         "survey_134B_model": bandwidth_fractions(survey_step_bytes, ms / args.steps, peak)}}
+    roofline["step"]["frac"] = roofline["step"]["frac_of_measured_peak"]
+    roofline["step"]["achieved_GBps"] = roofline["step"]["GBps"]
+
+    # ---------------- the config's nominal run from its initial state, in two halves --------------
+    whole_run = second_half = None
+    if not args.no_nominal_run:
+        nominal = cfg["steps"] if cfg["steps"] <= 2000 else 2000     # cfg1/cfg2 name 10^4 steps: the first 2000 are timed
+        simn = B.from_tiling(t, **p)
+        s0 = simn.stats()
+        h1 = nominal // 2
+        ms1, smp1 = timed_steps(simn, h1)
+        s1 = simn.stats()
+        ms2, smp2 = timed_steps(simn, nominal - h1)
+        s2 = simn.stats()
+        smp_all = ClockSampler(local_rank)
+        smp_all.sm, smp_all.reasons, smp_all.sm_max = smp1.sm + smp2.sm, smp1.reasons | smp2.reasons, smp1.sm_max
+        whole_run = region_record(ms1 + ms2, nominal, 0, s0, s2, smp_all)
+        whole_run["includes_resorts"] = s2["n_sorts"] - s0["n_sorts"]
+        second_half = region_record(ms2, nominal - h1, h1, s1, s2, smp2)
+        simn.close()
+        del simn
 
     # ---------------- end to end through the host-pointer entry points --------------------------
     # One job = avm_create_host (H2D of the whole state from pinned memory) + K steps +
@@ -284,16 +365,22 @@ def main():
                "job": "avm_create_host + avm_step(K) + avm_get_state_host, pinned host buffers", "ms": e2e_t}
 
     # ---------------- CPU baseline: the oracle as it stands, one core, bounded sample ------------
+    # BASELINE.md §3 / SURVEY §8(d): time >= 20 consecutive steps AFTER the initial burst (the oracle's
+    # own first 50 steps) for the large configs.  A million-cell step takes the oracle ~0.7 s, so the
+    # sample is sized to ~25 s of timed work plus the untimed skip.
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle
         o = oracle.from_tiling(t, **p)
-        n_o = max(2, min(200, int(15.0 / (1.5e-6 * N))))      # ~15 s of single-core work
+        est = 0.7e-6 * N                                       # s per step, one core
+        n_o = max(20, min(400, int(15.0 / est)))
+        skip = 50 if est * 50 < 60.0 else max(0, int(60.0 / est))   # cfg4: the skip itself is capped at ~60 s
+        o.step(skip)
         t0 = time.perf_counter()
         o.step(n_o)
         dt = time.perf_counter() - t0
         cpu = {"value": V * n_o / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
-               "sample": f"steps 0..{n_o - 1} of the same {cfg['name']} tiling from its initial state (inside the step-0 T1 burst)",
+               "sample": f"steps {skip}..{skip + n_o - 1} of the same {cfg['name']} tiling ({N} cells), after the oracle's own first {skip} steps",
                "timesteps_per_s": n_o / dt, "host_cpus": os.cpu_count()}
 
     if rank == 0:
@@ -302,11 +389,9 @@ def main():
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"{cfg['name']}: AVM N={N} cells, V={V}, L={cfg['L']}, periodic Voronoi of uniform points "
-                                   f"(seed {cfg['points_seed']}), p0={cfg['p0']}, v0={cfg['v0']}, Dr={cfg['Dr']}, dt={cfg['dt']}, "
-                                   f"l_c={cfg['l_c']}, Hilbert-sorted at create={cfg['sort_at_create']}, sort_every={cfg['sort_every']}",
+            "config": {"workload": workload_string(cfg, N, V),
                        "parallelism": "replicas only" if world > 1 else "1 GPU",
-                       "t1_passes_per_step": args.t1_passes,
+                       "t1_passes_per_step": args.t1_passes, "schedule": args.schedule,
                        "l2": f"inputs larger than L2: resident state {224 * N / 1e6:.0f} MB vs 126 MB L2" if 224 * N > 126e6
                              else "state fits in L2 (latency/launch bound config); no flush",
                        "timed_region": f"steps {st0['step']}..{st1['step'] - 1} after {args.warmup} warm-up steps"},
@@ -318,6 +403,8 @@ def main():
                    "error_word": state_after["error"]},
             "clocks": sampler.summary(),
             "roofline": roofline,
+            "whole_run": whole_run,
+            "second_half": second_half,
             "e2e": e2e,
             "cpu_baseline": cpu,
         }

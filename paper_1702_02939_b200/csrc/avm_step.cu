@@ -27,7 +27,10 @@
 namespace avm {
 
 static constexpr int kVertexBlock = 256;
-static constexpr int kCellBlock = 128;
+#ifndef AVM_CELL_BLOCK
+#define AVM_CELL_BLOCK 128
+#endif
+static constexpr int kCellBlock = AVM_CELL_BLOCK;
 static constexpr int kT1Block = 128;
 static constexpr int kT1Grid = 148 * 2;
 static constexpr unsigned kFull = 0xffffffffu;
@@ -383,7 +386,7 @@ force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts 
   const int lane = threadIdx.x & 31;
   const unsigned prev = min(d.ctr->n_cand[parity ^ 1u], (unsigned)k.cap_a);
   const unsigned gwarp = (unsigned)tid >> 5, nwarps = (unsigned)stride >> 5;
-  if (tid == 0) { d.ctr->n_cand[parity] = 0; *d.feedback = prev; }
+  if (tid == 0) { d.ctr->n_cand[parity] = 0; if (kFused) *d.feedback = prev; }   // whoever applies a list reports its length
   if (kFused) {
     if (prev == 0u) { sweep<false>(d, k, nullptr, tid, stride, lane); return; }
     if (tid == 0) atomicAdd((unsigned long long*)&d.ctr->t1_candidates, (unsigned long long)prev);
@@ -907,6 +910,7 @@ t1_flip_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, 
   const int lane = threadIdx.x & 31;
   const unsigned gwarp = (blockIdx.x * kT1Block + threadIdx.x) >> 5, nwarps = (gridDim.x * kT1Block) >> 5;
   if (count_stats && gwarp == 0 && lane == 0 && n_cand) atomicAdd((unsigned long long*)&d.ctr->t1_candidates, (unsigned long long)n_cand);
+  if (count_stats && parity < 2u && gwarp == 0 && lane == 0) *d.feedback = n_cand;     // the step's list: report the T1 load
   unsigned int flips = 0, seen = 0;
   for (unsigned int i = gwarp * 8u; i < n_cand; i += nwarps * 8u) {
     flips += t1_flip_quads(d, k, list, i, n_cand, lane);
