@@ -461,7 +461,7 @@ int avm_create_host(const avm_params* params, const double* pos_xy, const int32_
 // however far the host runs ahead, which is fine for a slowly varying load), before that from the
 // number of short edges at creation.  Both schedules give the same bits.
 #ifndef AVM_FUSED_MAX_CANDIDATES
-#define AVM_FUSED_MAX_CANDIDATES 96
+#define AVM_FUSED_MAX_CANDIDATES 128
 #endif
 static bool leave_flips_pending(const avm_sim* s, bool last_of_call) {
   if (!s->fused_ok || last_of_call) return false;   // the last step of a call is completed inside the call

@@ -486,8 +486,13 @@ __device__ __noinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va,
   const int quad[4] = {cL, cR, cE1, cE2};
   int nq[4];
   int4 q[4][2];
+  const bool flag = count_stats && k.flag_dirty;     // the rows are only needed to flag their vertices
 #pragma unroll
-  for (int t = 0; t < 4; ++t) { nq[t] = d.cvn[quad[t]]; q[t][0] = d.cv[quad[t]]; q[t][1] = d.cv[(size_t)k.N + quad[t]]; }
+  for (int t = 0; t < 4; ++t) {
+    nq[t] = d.cvn[quad[t]];
+    q[t][0] = q[t][1] = make_int4(0, 0, 0, 0);
+    if (flag) { q[t][0] = d.cv[quad[t]]; q[t][1] = d.cv[(size_t)k.N + quad[t]]; }
+  }
   const int x1s1 = d.vn[k.Vs + x1], x1s2 = d.vn[2 * k.Vs + x1], x2s1 = d.vn[k.Vs + x2], x2s2 = d.vn[2 * k.Vs + x2];
   if (!(nq[0] > 3 && nq[1] > 3)) return;                       // no 2-gons (T2 absent)
   if (!(nq[2] < k.S && nq[3] < k.S)) {                         // row would exceed the stride
@@ -515,7 +520,7 @@ __device__ __noinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va,
   // Everything a flip of this edge would write, and everything that reads it in the next
   // force/move pass, belongs to a vertex of these four cells: flag them, so that force_move can
   // run the flips while the untouched vertices already move.
-  if (count_stats && k.flag_dirty) {
+  if (flag) {
     unsigned int* __restrict__ dirty = d.dirty + (size_t)parity * (size_t)k.nw;   // this step's bitmap
 #pragma unroll
     for (int t = 0; t < 4; ++t) {

@@ -450,26 +450,35 @@ def test_long_run_at_the_config_length_keeps_every_invariant(B):
 
 
 def test_two_launch_schedule_at_full_size_equals_three_launch_schedule(B):
-    """configs[3] (N = 1,048,576, the bench workload) for 300 steps with a re-sort every 100: the
-    default two-launch schedule — ~96 000 simultaneous candidates in step 0 (every warp flips),
-    then a few dozen per step (a few flipper warps) — against the three-launch schedule, bit for bit."""
+    """configs[3] (N = 1,048,576, the bench workload) for 300 steps with a re-sort every 100, three ways:
+    the two-launch schedule forced for every step (~96 000 simultaneous candidates in step 0: the
+    many-candidate path inside force_move; later a few dozen per step: dedicated flipper warps),
+    the schedule avm_step chooses by itself from the T1 load the device reports (stand-alone T1
+    kernel during the burst, two launches afterwards), and the three-launch schedule.  Bit for bit."""
     t = tiling(3)
     p = dict(w.config_params(3), sort_every=100)
-    a = B.from_tiling(t, **p)
-    a.step(300)
-    sa = to_np(a.get_state())
-    area = a.compute_forces()[1][:, 0].sum().item()
-    a.close()
-    del a
-    b = B.from_tiling(t, schedule="unfused", **p)
-    b.step(300)
-    sb = to_np(b.get_state())
-    b.close()
-    assert sa["stats"]["kernel_launches"] < sb["stats"]["kernel_launches"]
-    for key in ("pos", "theta", "cell_vertices", "vertex_neighbors", "vertex_cell_neighbors", "cell_vertex_num"):
-        assert np.array_equal(sa[key], sb[key]), key
-    for key in ("t1_short", "t1_candidates", "t1_flips", "t1_blocked", "overflow_rejects", "error"):
-        assert sa["stats"][key] == sb["stats"][key], key
+    keys = ("pos", "theta", "cell_vertices", "vertex_neighbors", "vertex_cell_neighbors", "cell_vertex_num")
+    states = {}
+    for name in ("fused", "auto", "unfused"):
+        a = B.from_tiling(t, schedule=name, **p)
+        if name == "auto":          # the host sees the reported load only as far as the device has come
+            for n in (250, 50):
+                a.step(n)
+                a.stats()
+        else:
+            a.step(300)
+        states[name] = to_np(a.get_state())
+        if name == "fused":
+            area = a.compute_forces()[1][:, 0].sum().item()
+        a.close()
+        del a
+    sa, sb = states["fused"], states["unfused"]
+    assert sa["stats"]["kernel_launches"] < states["auto"]["stats"]["kernel_launches"] < sb["stats"]["kernel_launches"]
+    for other in ("auto", "unfused"):
+        for key in keys:
+            assert np.array_equal(sa[key], states[other][key]), (other, key)
+        for key in ("t1_short", "t1_candidates", "t1_flips", "t1_blocked", "overflow_rejects", "error"):
+            assert sa["stats"][key] == states[other]["stats"][key], (other, key)
     assert sa["stats"]["error"] == 0 and sa["stats"]["t1_flips"] > 90000
     L2 = t.Lx * t.Ly
     assert abs(area - L2) <= 1e-12 * L2
