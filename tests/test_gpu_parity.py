@@ -569,3 +569,60 @@ def test_smallest_tori(B):
         g.step(200)
         o.step(200)
         assert_states_match(to_np(g.get_state()), o.get_state(), t.Lx, t.Ly, pos_tol=1e-7)
+
+
+@pytest.mark.parametrize("params_of", [3, 4])
+def test_fused_schedule_hammered_at_a_million_cells(B, params_of):
+    """The two-launch schedule against the three-launch schedule over 2000 steps with re-sorts on the
+    N = 1,048,576 tiling, bit for bit: with configs[3]'s parameters (after the burst a few dozen
+    candidates per step: dedicated flipper warps work while every other warp sweeps, the regime
+    in which a skipped vertex must stay skipped for the whole launch) and with configs[4]'s
+    parameters (thousands of candidates in every step: the many-candidate path).  The flagged-vertex
+    bitmap is read-only for the launch that sweeps with it, so both are race-free by construction;
+    this test is the empirical side of that argument (compute-sanitizer is closed on this pool)."""
+    t = tiling(3)
+    p = dict(w.config_params(3), sort_every=250)
+    if params_of == 4:
+        p4 = w.config_params(4)
+        p.update({k: p4[k] for k in ("P0", "v0", "Dr", "dt", "l_c")})
+    keys = ("pos", "theta", "cell_vertices", "vertex_neighbors", "vertex_cell_neighbors", "cell_vertex_num")
+    out = []
+    for sched in ("fused", "unfused", "fused"):
+        a = B.from_tiling(t, schedule=sched, **p)
+        a.step(2000)
+        out.append(to_np(a.get_state()))
+        a.close()
+        del a
+    for other in out[1:]:
+        for key in keys:
+            assert np.array_equal(out[0][key], other[key]), key
+        for key in ("t1_short", "t1_candidates", "t1_flips", "t1_blocked", "overflow_rejects", "error"):
+            assert out[0]["stats"][key] == other["stats"][key], key
+    assert out[0]["stats"]["error"] == 0 and out[0]["stats"]["n_sorts"] == 9      # one at create, eight in the run
+    assert out[0]["stats"]["t1_flips"] > (2_000_000 if params_of == 4 else 100_000)
+    _TILINGS.pop(3, None)
+
+
+def test_fused_schedule_with_resorts_against_the_oracle_at_fused_size(B):
+    """configs[4]'s parameters and density on the smallest tiling that takes the two-launch schedule by
+    default (V = 2^20), re-sorted every 3 steps, followed by the oracle across two re-sort
+    boundaries: pending flips are completed before each re-sort, the candidate lists hold pre-sort
+    indices and are dropped, tags keep priorities and noise unchanged (R11, R16)."""
+    N = 524288
+    cfg = w.CONFIGS[4]
+    L = cfg["L"] * (N / cfg["N"]) ** 0.5
+    t = w.voronoi_tiling(N, L, cfg["points_seed"])
+    p = dict(w.config_params(4), Lx=L, Ly=L, sort_every=3, sort_at_create=True)
+    o = oracle.from_tiling(t, **p)
+    for sched in ("fused", "auto"):
+        g = B.from_tiling(t, schedule=sched, **p)
+        if sched == "fused":
+            g.step(7)
+            o.step(7)
+        else:
+            g.step(4)
+            g.step(3)
+        sg = to_np(g.get_state())
+        assert_states_match(sg, o.get_state(), t.Lx, t.Ly)
+        assert sg["stats"]["n_sorts"] == 3 and sg["stats"]["t1_flips"] > 10000
+        g.close()
