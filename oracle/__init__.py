@@ -65,6 +65,10 @@ def _load() -> ctypes.CDLL:
         lib.oracle_step.argtypes = [p, i64]
         lib.oracle_t1_pass.argtypes = [p]
         lib.oracle_set_cell_targets.argtypes = [p, p, p]
+        lib.oracle_set_cell_moduli.argtypes = [p, p, p]
+        lib.oracle_msd.argtypes = [p]
+        lib.oracle_msd.restype = ctypes.c_double
+        lib.oracle_msd_reset.argtypes = [p]
         lib.oracle_debug_t1.argtypes = [p, p, p, p, p, i64]
         lib.oracle_get_state.argtypes = [p, p, p, p, p, p, p, ctypes.POINTER(OracleStats)]
         lib.oracle_set_positions.argtypes = [p, p]
@@ -143,7 +147,7 @@ class OracleSim:
         ap = self.geometry()
         A, P = ap[:, 0], ap[:, 1]
         pos = A > 0
-        return {"energy": self.energy(), "sum_area": float(A.sum()), "sum_perimeter": float(P.sum()),
+        return {"energy": self.energy(), "msd": self.msd(), "sum_area": float(A.sum()), "sum_perimeter": float(P.sum()),
                 "mean_shape_index": float((P[pos] / np.sqrt(A[pos])).mean()) if pos.any() else 0.0,
                 "area_min": float(A.min()), "area_max": float(A.max()),
                 "area_variance": float((A * A).mean() - A.mean() ** 2),
@@ -164,6 +168,20 @@ class OracleSim:
         b = None if P0 is None else np.ascontiguousarray(P0, dtype=np.float64)
         if _load().oracle_set_cell_targets(self._h, _ptr(a), _ptr(b)) != 0:
             raise ValueError("oracle_set_cell_targets: give both arrays or neither")
+
+    def set_cell_moduli(self, KA=None, KP=None) -> None:
+        """per-cell moduli K_{A,i}, K_{P,i} of Eq. 1 (user order); None, None = uniform again"""
+        a = None if KA is None else np.ascontiguousarray(KA, dtype=np.float64)
+        b = None if KP is None else np.ascontiguousarray(KP, dtype=np.float64)
+        if _load().oracle_set_cell_moduli(self._h, _ptr(a), _ptr(b)) != 0:
+            raise ValueError("oracle_set_cell_moduli: give both arrays or neither")
+
+    def msd(self) -> float:
+        """mean-square displacement of the vertices since creation / the latest msd_reset (unwrapped)"""
+        return float(_load().oracle_msd(self._h))
+
+    def msd_reset(self) -> None:
+        _load().oracle_msd_reset(self._h)
 
     def t1_pass(self) -> None:
         _load().oracle_t1_pass(self._h)

@@ -16,7 +16,9 @@
 // forces vs central finite differences of Eq. A1; sum of areas = Lx*Ly; sum of forces = 0;
 // shift invariance; Euler characteristic / 3-coordination / slot convention after T1 passes;
 // hand-built T1 (Fig. 1 right); brute-force conflict rule; closed-form pure-activity translation;
-// Philox core vs the cuRAND *host* generator (library routine) and moment/KS tests.
+// Philox core vs the cuRAND *host* generator (library routine) and moment/KS tests; per-cell targets and
+// moduli vs finite differences of Eq. 1; mean-square displacement vs the closed-form translation, the
+// closed form of one T1 and an independent numpy unwrapping of the trajectory.
 // "Whole step" parity is unpinned beyond those invariants: the paper prints no trajectory.
 
 #include <cstdint>
@@ -53,9 +55,16 @@ struct Sim {
   std::vector<int32_t> vc;      // [V][3]        vertexCellNeighbors
   std::vector<double> A0c, P0c; // [N] per-cell preferred values A_{0,i}, P_{0,i} of Eq. 1 (
                                 // NEXT-4); empty = the uniform A0, P0 of Eq. A1 (R17)
+  std::vector<double> KAc, KPc; // [N] per-cell moduli K_{A,i}, K_{P,i} (Eq. 1 read with the moduli inside the sum,
+                                // SURVEY 8(f) NEXT-4); empty = the uniform K_A, K_P of Eq. A1
+  std::vector<double> unwrapped;  // [V][2] unwrapped positions: every elementary displacement (the Euler move of
+                                  // Eq. 4, the repositioning of a T1) is added as a minimum-image vector, never wrapped
+  std::vector<double> msd_ref;    // [V][2] unwrapped positions at the reference time of the mean-square displacement
   Stats st;
   double A0(int64_t c) const { return A0c.empty() ? p.A0 : A0c[c]; }
   double P0(int64_t c) const { return P0c.empty() ? p.P0 : P0c[c]; }
+  double KA(int64_t c) const { return KAc.empty() ? p.KA : KAc[c]; }
+  double KP(int64_t c) const { return KPc.empty() ? p.KP : KPc[c]; }
 };
 
 // ------------------------------------------------------------------------------------------
@@ -139,7 +148,7 @@ double energy(const Sim& s, const std::vector<double>& AP) {
   double E = 0.0;
   for (int64_t c = 0; c < s.N; ++c) {
     double dA = AP[2 * c] - s.A0(c), dP = AP[2 * c + 1] - s.P0(c);
-    E += s.p.KA * dA * dA + s.p.KP * dP * dP;
+    E += s.KA(c) * dA * dA + s.KP(c) * dP * dP;
   }
   return E;
 }
@@ -172,7 +181,7 @@ void vertex_force(const Sim& s, const std::vector<double>& AP, int64_t v, double
     if (lp > 0.0) { upx = rpx / lp; upy = rpy / lp; }
     if (ln > 0.0) { unx = rnx / ln; uny = rny / ln; }
     const double dPx = -(upx + unx), dPy = -(upy + uny);
-    const double ca = 2.0 * s.p.KA * (AP[2 * c] - s.A0(c)), cp = 2.0 * s.p.KP * (AP[2 * c + 1] - s.P0(c));
+    const double ca = 2.0 * s.KA(c) * (AP[2 * c] - s.A0(c)), cp = 2.0 * s.KP(c) * (AP[2 * c + 1] - s.P0(c));
     Fx -= ca * dAx + cp * dPx;
     Fy -= ca * dAy + cp * dPy;
   }
@@ -281,8 +290,12 @@ void t1_flip(Sim& s, const Cand& c) {
   double px = 0.0, py = 1.0;
   if (l > 0.0) { px = -dy / l; py = dx / l; }
   const double half = 0.75 * s.p.l_c;
+  const double o1x = s.pos[2 * v1], o1y = s.pos[2 * v1 + 1], o2x = s.pos[2 * v2], o2y = s.pos[2 * v2 + 1];
   s.pos[2 * v2] = wrap(mx + half * px, s.p.Lx); s.pos[2 * v2 + 1] = wrap(my + half * py, s.p.Ly);
   s.pos[2 * v1] = wrap(mx - half * px, s.p.Lx); s.pos[2 * v1 + 1] = wrap(my - half * py, s.p.Ly);
+  // unwrapped positions follow by the minimum-image displacement of the repositioning
+  s.unwrapped[2 * v1] += mi(s.pos[2 * v1] - o1x, s.p.Lx); s.unwrapped[2 * v1 + 1] += mi(s.pos[2 * v1 + 1] - o1y, s.p.Ly);
+  s.unwrapped[2 * v2] += mi(s.pos[2 * v2] - o2x, s.p.Lx); s.unwrapped[2 * v2 + 1] += mi(s.pos[2 * v2 + 1] - o2y, s.p.Ly);
   // --- topology.  Cyclic from the partner's slot: u has (n; c) = ([w, x, y]; [C0, C1, C2]).
   const int k1 = c.k1, k2 = c.k2;
   const int32_t x1 = s.vn[3 * v1 + (k1 + 1) % 3], y1 = s.vn[3 * v1 + (k1 + 2) % 3];
@@ -339,6 +352,8 @@ void step(Sim& s) {
     }
     const double vx = s.p.mu * F[2 * v] + (s.p.v0 / 3.0) * ax;
     const double vy = s.p.mu * F[2 * v + 1] + (s.p.v0 / 3.0) * ay;
+    s.unwrapped[2 * v] += s.p.dt * vx;                  // the displacement itself, before any wrap
+    s.unwrapped[2 * v + 1] += s.p.dt * vy;
     s.pos[2 * v] = wrap(s.pos[2 * v] + s.p.dt * vx, s.p.Lx);
     s.pos[2 * v + 1] = wrap(s.pos[2 * v + 1] + s.p.dt * vy, s.p.Ly);
     if (!std::isfinite(s.pos[2 * v]) || !std::isfinite(s.pos[2 * v + 1])) s.st.error |= 1;
@@ -373,6 +388,8 @@ oracle_sim* oracle_create(const oracle_params* p, const double* pos_xy, const in
   s->p = *p;
   s->N = p->n_cells; s->V = p->n_vertices; s->S = p->max_cell_vertices;
   s->pos.assign(pos_xy, pos_xy + 2 * s->V);
+  s->unwrapped = s->pos;
+  s->msd_ref = s->pos;
   s->theta.assign(theta, theta + s->N);
   s->cvn.assign(cell_vertex_num, cell_vertex_num + s->N);
   s->cv.assign(cell_vertices, cell_vertices + s->N * s->S);
@@ -424,6 +441,26 @@ int oracle_set_cell_targets(oracle_sim* s, const double* A0, const double* P0) {
   return 0;
 }
 
+// NEXT-4: per-cell moduli K_{A,i}, K_{P,i} (Eq. 1 with the moduli inside the sum), user order; NULL, NULL = uniform again
+int oracle_set_cell_moduli(oracle_sim* s, const double* KA, const double* KP) {
+  if (!s || ((KA == nullptr) != (KP == nullptr))) return -1;
+  s->KAc.clear(); s->KPc.clear();
+  if (KA) { s->KAc.assign(KA, KA + s->N); s->KPc.assign(KP, KP + s->N); }
+  return 0;
+}
+
+// NEXT-2: mean-square displacement of the vertices since the reference time (creation, or the latest
+// oracle_msd_reset): <|U_v(t) - U_v(t_ref)|^2> over all vertices, U = unwrapped position
+double oracle_msd(oracle_sim* s) {
+  double acc = 0.0;
+  for (int64_t v = 0; v < s->V; ++v) {
+    const double dx = s->unwrapped[2 * v] - s->msd_ref[2 * v], dy = s->unwrapped[2 * v + 1] - s->msd_ref[2 * v + 1];
+    acc += dx * dx + dy * dy;
+  }
+  return acc / (double)s->V;
+}
+int oracle_msd_reset(oracle_sim* s) { s->msd_ref = s->unwrapped; return 0; }
+
 int oracle_t1_pass(oracle_sim* s) { t1_pass(*s); return 0; }
 
 // detect + resolve on the current state without flipping: sorted (tag_min, tag_max) pairs
@@ -459,8 +496,11 @@ int oracle_get_state(oracle_sim* s, double* pos_xy, int32_t* cell_vertex_num, in
   return 0;
 }
 
+// test hook: overwrite the positions; the unwrapped positions and the MSD reference restart from them
 int oracle_set_positions(oracle_sim* s, const double* pos_xy) {
   std::memcpy(s->pos.data(), pos_xy, sizeof(double) * 2 * s->V);
+  s->unwrapped = s->pos;
+  s->msd_ref = s->pos;
   return 0;
 }
 

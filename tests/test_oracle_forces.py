@@ -248,3 +248,61 @@ def test_per_cell_targets_special_cases():
     assert np.abs(c.compute_forces()[0]).max() == 0.0 and c.energy() == 0.0
     c.set_cell_targets(None, None)
     assert np.array_equal(c.compute_forces()[0], oracle.from_tiling(t, **p).compute_forces()[0])
+
+
+def test_per_cell_moduli_match_finite_differences_of_eq1():
+    """heterogeneous K_{A,i}, K_{P,i} together with heterogeneous targets (Eq. 1, read with the
+    moduli inside the sum): F = -dE/dh against central differences of the energy written out
+    here with numpy from the oracle's geometry; uniform arrays reproduce the scalar path bit for bit;
+    zero moduli on a cell switch that cell's contribution off."""
+    t = w.voronoi_tiling(64, 8.0, 6)
+    rng = np.random.default_rng(1)
+    A0, P0 = rng.uniform(0.6, 1.4, t.N), rng.uniform(3.2, 4.2, t.N)
+    KA, KP = rng.uniform(0.2, 3.0, t.N), rng.uniform(0.1, 2.0, t.N)
+    sim = oracle.from_tiling(t, **PARAMS)
+    sim.set_cell_targets(A0, P0)
+    sim.set_cell_moduli(KA, KP)
+    F, ap0 = sim.compute_forces()
+    assert abs(sim.energy() - np.sum(KA * (ap0[:, 0] - A0) ** 2 + KP * (ap0[:, 1] - P0) ** 2)) < 1e-10
+    rms = np.sqrt((F ** 2).sum(axis=1).mean())
+    worst = 0.0
+    for v in range(0, t.V, 3):
+        cells = t.vertex_cell_neighbors[v]
+        dn = t.pos[t.vertex_neighbors[v]] - t.pos[v]
+        lmin = np.hypot(h.min_image(dn[:, 0], t.Lx), h.min_image(dn[:, 1], t.Ly)).min()
+        delta = min(1e-5, 1e-2 * lmin)
+        g = np.zeros(2)
+        for ax in range(2):
+            e = {}
+            for m in (-2, -1, 1, 2):
+                pos = t.pos.copy()
+                pos[v, ax] += m * delta
+                pos[v, ax] %= (t.Lx, t.Ly)[ax]
+                sim.set_positions(pos)
+                ap = sim.geometry()
+                e[m] = np.sum(KA[cells] * (ap[cells, 0] - A0[cells]) ** 2 + KP[cells] * (ap[cells, 1] - P0[cells]) ** 2)
+            g[ax] = (8 * (e[1] - e[-1]) - (e[2] - e[-2])) / (12 * delta)
+        worst = max(worst, np.linalg.norm(F[v] + g) / max(np.linalg.norm(F[v]), rms))
+    assert worst < 1e-6, worst
+    sim.set_positions(t.pos)
+    assert np.abs(sim.compute_forces()[0].sum(axis=0)).max() < 1e-10
+    # uniform arrays = the scalar path, bit for bit, through T1s
+    t0 = w.config_tiling(0)
+    p = w.config_params(0)
+    a, b = oracle.from_tiling(t0, **p), oracle.from_tiling(t0, **p)
+    b.set_cell_moduli(np.full(t0.N, p["KA"]), np.full(t0.N, p["KP"]))
+    a.step(30)
+    b.step(30)
+    assert np.array_equal(a.get_state()["pos"], b.get_state()["pos"])
+    # a cell with zero moduli exerts no force: the force on a vertex then comes from its other cells only
+    c = oracle.from_tiling(t0, **p)
+    KA0, KP0 = np.full(t0.N, p["KA"]), np.full(t0.N, p["KP"])
+    dead = int(t0.vertex_cell_neighbors[5, 0])
+    KA0[dead] = KP0[dead] = 0.0
+    c.set_cell_moduli(KA0, KP0)
+    F1 = c.compute_forces()[0]
+    far = np.array([v for v in range(t0.V) if dead not in t0.vertex_cell_neighbors[v]])
+    assert np.array_equal(F1[far], a.__class__(t0.pos, t0.cell_vertex_num, t0.cell_vertices, t0.vertex_neighbors,
+                                               t0.vertex_cell_neighbors, t0.theta, **p).compute_forces()[0][far])
+    c.set_cell_moduli(None, None)
+    assert np.array_equal(c.compute_forces()[0], oracle.from_tiling(t0, **p).compute_forces()[0])

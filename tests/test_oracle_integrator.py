@@ -170,3 +170,61 @@ def test_topology_is_tested_on_the_moved_positions():
     r = ref.get_state()["pos"]
     d = r[hi] - r[lo]
     assert abs(np.hypot(h.min_image(d[0], t.Lx), h.min_image(d[1], t.Ly)) - (start_len - closing)) < 1e-13
+
+
+# ---- NEXT-2: mean-square displacement of the vertices (unwrapped positions) ----
+
+def test_msd_of_pure_activity_is_the_closed_form_through_the_box():
+    """K_A = K_P = 0, D_r = 0, uniform theta: every vertex has moved by n*v0*dt along the director, so
+    the mean-square displacement is (n v0 dt)^2 exactly, however often the box wrapped; a reset
+    restarts it from zero."""
+    th0 = 2.1
+    t = w.hex_tiling(6, 4, a=1.0, theta=np.full(24, th0))
+    v0, dt, n = 0.8, 0.01, 1500                      # 12 length units: more than one box length (10.4 x 6)
+    sim = oracle.from_tiling(t, KA=0.0, KP=0.0, v0=v0, Dr=0.0, dt=dt, l_c=0.0)
+    assert sim.msd() == 0.0
+    sim.step(n)
+    assert abs(sim.msd() - (n * v0 * dt) ** 2) < 1e-9 * (n * v0 * dt) ** 2
+    sim.msd_reset()
+    assert sim.msd() == 0.0
+    sim.step(10)
+    assert abs(sim.msd() - (10 * v0 * dt) ** 2) < 1e-12
+
+
+def test_msd_counts_the_repositioning_of_a_t1():
+    """one hand-built flip and nothing else moving: the two end points go from +-len/2 along the edge to
+    +-0.75 l_c across it (R9), so MSD = 2 ((len/2)^2 + (0.75 l_c)^2) / V"""
+    from tests.test_oracle_t1 import shrink_edge
+    l_c = 0.04
+    t = w.hex_tiling(6, 4, a=1.0)
+    v1, v2 = 7, int(t.vertex_neighbors[7, 1])
+    ln = 0.5 * l_c
+    pos, _, _ = shrink_edge(t, min(v1, v2), max(v1, v2), ln)
+    sim = oracle.from_tiling(t, KA=0.0, KP=0.0, v0=0.0, Dr=0.0, dt=0.01, l_c=l_c)
+    sim.set_positions(pos)
+    sim.step(1)
+    assert sim.get_state()["stats"]["t1_flips"] == 1
+    assert abs(sim.msd() - 2 * ((0.5 * ln) ** 2 + (0.75 * l_c) ** 2) / t.V) < 1e-15
+
+
+def test_msd_equals_an_independent_unwrapping_of_the_trajectory():
+    """configs[0] with a large drift so that vertices cross the box: the oracle's MSD against numpy's
+    accumulation of minimum-image differences between consecutive snapshots (valid because one step
+    moves a vertex by far less than L/2)"""
+    t = w.config_tiling(0)
+    p = dict(w.config_params(0), v0=3.0, Dr=0.2)
+    sim = oracle.from_tiling(t, **p)
+    prev = t.pos.copy()
+    U = np.zeros_like(prev)
+    for _ in range(300):
+        sim.step(1)
+        cur = sim.get_state()["pos"]
+        d = cur - prev
+        U[:, 0] += h.min_image(d[:, 0], t.Lx)
+        U[:, 1] += h.min_image(d[:, 1], t.Ly)
+        prev = cur
+    ref = (U ** 2).sum(axis=1).mean()
+    assert np.abs((prev - t.pos) - U).max() > 0.5 * t.Lx        # some vertices really left through the box boundary
+    assert abs(sim.msd() - ref) < 1e-10 * ref
+    assert sim.get_state()["stats"]["t1_flips"] > 0
+    assert abs(sim.observables()["msd"] - sim.msd()) == 0.0
