@@ -149,6 +149,12 @@ int avm_energy(avm_sim* sim, double* energy);
  * Asynchronous.  The values are not part of avm_get_state: a resumed run sets them again. */
 int avm_set_cell_targets(avm_sim* sim, const double* area0, const double* perimeter0);
 
+/* Per-cell moduli K_{A,i}, K_{P,i}: Eq. 1 read with the moduli inside the sum,
+ * E = sum_i K_{A,i} (A_i - A_{0,i})^2 + K_{P,i} (P_i - P_{0,i})^2.
+ * KA, KP: DEVICE pointers, [N] each, user order, copied; both NULL restores the uniform moduli of
+ * avm_params.  Independent of avm_set_cell_targets.  Asynchronous; not part of avm_get_state. */
+int avm_set_cell_moduli(avm_sim* sim, const double* KA, const double* KP);
+
 /* Observables of the current state, reduced on the device in a
  * fixed order (deterministic): the energy of Eq. 1, the area and perimeter totals, the mean shape
  * index <P / sqrt(A)> over the cells with A > 0 (the order parameter of the rigidity transition
@@ -158,8 +164,17 @@ int avm_set_cell_targets(avm_sim* sim, const double* area0, const double* perime
 typedef struct avm_observables {
   double energy, sum_area, sum_perimeter, mean_shape_index, area_min, area_max, area_variance;
   int64_t n_nonpositive_area, step, t1_flips;
+  double msd; /* mean-square displacement of the vertices since the reference time (below) */
 } avm_observables;
 int avm_observe(avm_sim* sim, avm_observables* out);
+
+/* Mean-square displacement (the fluid/solid diagnostic of the regimes of
+ * PAPER.md:114-116): <|U_v(t) - U_v(t_ref)|^2> over all vertices, U = unwrapped position.  The library
+ * counts, per vertex, the box lengths it has left through the boundary (in the move of Eq. 4 and
+ * in the repositioning of a T1), so U = position + count x L costs nothing per step.  The
+ * reference time is avm_create / avm_set_positions, or the latest avm_msd_reset.  Neither the counts
+ * nor the reference are part of avm_get_state: a resumed run measures from its own creation. */
+int avm_msd_reset(avm_sim* sim);
 
 /* Copy the current state out in user order.  stats (HOST pointer, may be NULL) receives the
  * counters; when it is non-NULL, or for the host variant, the call synchronises the stream. */

@@ -21,7 +21,7 @@ LIB_PATH = os.environ.get("AVM_B200_LIB") or os.path.join(_HERE, "libavm_b200.so
 # every symbol include/avm.h declares (tests check that the library exports all of them)
 ABI_SYMBOLS = [
     "avm_workspace_bytes", "avm_create", "avm_create_host", "avm_step", "avm_step_profile", "avm_compute_forces",
-    "avm_compute_forces_host", "avm_energy", "avm_observe", "avm_set_cell_targets", "avm_get_state", "avm_get_state_host", "avm_debug_t1",
+    "avm_compute_forces_host", "avm_energy", "avm_observe", "avm_set_cell_targets", "avm_set_cell_moduli", "avm_msd_reset", "avm_get_state", "avm_get_state_host", "avm_debug_t1",
     "avm_t1_pass", "avm_set_positions", "avm_resort", "avm_philox_words", "avm_hilbert_index",
     "avm_hilbert_index_host", "avm_destroy", "avm_strerror", "avm_last_cuda_error",
 ]
@@ -55,7 +55,7 @@ class AvmStats(ctypes.Structure):
 class AvmObservables(ctypes.Structure):
     _fields_ = [(n, ctypes.c_double) for n in ("energy", "sum_area", "sum_perimeter", "mean_shape_index", "area_min",
                                                "area_max", "area_variance")] + \
-               [(n, ctypes.c_int64) for n in ("n_nonpositive_area", "step", "t1_flips")]
+               [(n, ctypes.c_int64) for n in ("n_nonpositive_area", "step", "t1_flips")] + [("msd", ctypes.c_double)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -91,6 +91,8 @@ def _load() -> ctypes.CDLL:
     lib.avm_t1_pass.argtypes = [p]
     lib.avm_set_positions.argtypes = [p, p]
     lib.avm_set_cell_targets.argtypes = [p, p, p]
+    lib.avm_set_cell_moduli.argtypes = [p, p, p]
+    lib.avm_msd_reset.argtypes = [p]
     lib.avm_resort.argtypes = [p]
     lib.avm_philox_words.argtypes = [p, u64, u64, u64, i64, p]
     lib.avm_hilbert_index.argtypes = [p, i32, i64, p, p, p]
@@ -217,20 +219,30 @@ class AvmSim:
         _check(lib.avm_energy(self._h, ctypes.byref(e)))
         return e.value
 
-    def set_cell_targets(self, area0=None, perimeter0=None) -> None:
-        """per-cell preferred area / perimeter (numpy or CUDA tensors, user order); None, None = uniform"""
+    def _set_cell_pair(self, fn, a0, b0) -> None:
         t = self.torch
-        if area0 is None and perimeter0 is None:
-            _check(lib.avm_set_cell_targets(self._h, None, None))
+        if a0 is None and b0 is None:
+            _check(fn(self._h, None, None))
             return
         dev = []
-        for a in (area0, perimeter0):
+        for a in (a0, b0):
             if isinstance(a, np.ndarray):
                 a = t.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).to(self.device)
             assert a.shape == (self.N,) and a.dtype == t.float64 and a.is_contiguous()
             dev.append(a)
-        _check(lib.avm_set_cell_targets(self._h, _dptr(dev[0]), _dptr(dev[1])))
+        _check(fn(self._h, _dptr(dev[0]), _dptr(dev[1])))
         t.cuda.synchronize(self.device)        # the inputs are copied by then
+
+    def set_cell_targets(self, area0=None, perimeter0=None) -> None:
+        """per-cell preferred area / perimeter (numpy or CUDA tensors, user order); None, None = uniform"""
+        self._set_cell_pair(lib.avm_set_cell_targets, area0, perimeter0)
+
+    def set_cell_moduli(self, KA=None, KP=None) -> None:
+        """per-cell moduli K_A,i / K_P,i (numpy or CUDA tensors, user order); None, None = uniform"""
+        self._set_cell_pair(lib.avm_set_cell_moduli, KA, KP)
+
+    def msd_reset(self) -> None:
+        _check(lib.avm_msd_reset(self._h))
 
     def observe(self) -> dict:
         o = AvmObservables()

@@ -46,11 +46,12 @@ struct BufferSet {
   int4* cv;
   double* theta;
   CellRec* rec;
-  double2* tgt;
+  CellPar* par;
 };
 
 struct Layout {
-  size_t pos[2], vn[2], vc[2], cv[2], cvn[2], theta[2], rec[2], tgt[2], vtag[2], ctag[2];
+  size_t pos[2], vn[2], vc[2], cv[2], cvn[2], theta[2], rec[2], par[2], vtag[2], ctag[2];
+  size_t img, msd_ref;
   size_t minkey, cand, ctr, dirty, estamp, ap, epart, key[2], val[2], hist, newidx_v, newidx_c, order_v, order_c;
   size_t total;
 };
@@ -64,8 +65,9 @@ Layout make_layout(const avm_params& p) {
   for (int i = 0; i < 2; ++i) L.pos[i] = take(16 * V);
   for (int i = 0; i < 2; ++i) {
     L.vn[i] = take(12 * Vs); L.vc[i] = take(12 * Vs); L.cv[i] = take(4 * N * S); L.cvn[i] = take(4 * N);
-    L.theta[i] = take(8 * N); L.rec[i] = take(32 * N); L.tgt[i] = take(16 * N); L.vtag[i] = take(4 * V); L.ctag[i] = take(4 * N);
+    L.theta[i] = take(8 * N); L.rec[i] = take(32 * N); L.par[i] = take(32 * N); L.vtag[i] = take(4 * V); L.ctag[i] = take(4 * N);
   }
+  L.img = take(8 * V); L.msd_ref = take(16 * V);
   L.minkey = take(8 * N);
   L.cand = take(sizeof(Cand) * (t1_passes_of(p) > 1 ? 5 : 3) * N);   // the step's list (3N = every edge) + two lists of N for repeated passes
   L.ctr = take(sizeof(Counters));
@@ -107,6 +109,9 @@ struct avm_sim {
   unsigned int* dirty;
   unsigned int* estamp;
   unsigned int* d_feedback;   // device view of h_feedback (or a word of the counters)
+  int2* img;                  // MSD: image counts, user order
+  double2* msd_ref;           // MSD: unwrapped reference positions, user order
+  bool tgt_custom, mod_custom;   // per-cell targets / moduli in force (Eq. 1); either one switches Consts::per_cell on
   unsigned int stamp;    // id of the latest repeated T1 pass (estamp entries equal to it were tested in that pass)
   int t1_passes;         // T1 passes per step (1 = north_star's rule; > 1 = repeat until none, NEXT-1)
   bool fused_ok;         // the two-launch schedule (T1 flips of a step ride in the next force/move launch) may be used
@@ -125,17 +130,17 @@ struct avm_sim {
     Dev d;
     d.pos = pos[cur_pos]; d.pos_next = pos[1 - cur_pos];
     const BufferSet& b = set[cur_set];
-    d.vn = b.vn; d.vc = b.vc; d.cv = b.cv; d.cvn = b.cvn; d.theta = b.theta; d.rec = b.rec; d.tgt = b.tgt;
+    d.vn = b.vn; d.vc = b.vc; d.cv = b.cv; d.cvn = b.cvn; d.theta = b.theta; d.rec = b.rec; d.par = b.par;
     d.vtag = b.vtag; d.ctag = b.ctag;
     d.minkey = minkey; d.cand = cand; d.ctr = ctr; d.dirty = dirty; d.estamp = estamp;
-    d.feedback = d_feedback;
+    d.feedback = d_feedback; d.img = img; d.msd_ref = msd_ref;
     return d;
   }
   Dev dev_alt() const {   // the other buffer set, target of a re-sort / staging area
     Dev d = dev();
     const BufferSet& b = set[1 - cur_set];
     d.pos = pos[1 - cur_pos]; d.pos_next = pos[cur_pos];
-    d.vn = b.vn; d.vc = b.vc; d.cv = b.cv; d.cvn = b.cvn; d.theta = b.theta; d.rec = b.rec; d.tgt = b.tgt;
+    d.vn = b.vn; d.vc = b.vc; d.cv = b.cv; d.cvn = b.cvn; d.theta = b.theta; d.rec = b.rec; d.par = b.par;
     d.vtag = b.vtag; d.ctag = b.ctag;
     return d;
   }
@@ -151,6 +156,8 @@ __global__ void import_kernel(const Dev d, const Consts k, const int* __restrict
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < k.V) {
     d.vtag[i] = i;
+    d.img[i] = make_int2(0, 0);          // the mean-square displacement is measured from the initial state
+    d.msd_ref[i] = d.pos[i];
 #pragma unroll
     for (int s = 0; s < 3; ++s) { d.vn[s * k.Vs + i] = vn_u[3 * i + s]; d.vc[s * k.Vs + i] = vc_u[3 * i + s]; }
   }
@@ -216,20 +223,41 @@ __global__ void export_cells_kernel(const Dev d, const Consts k, int* cvn, int* 
   if (cv)
     for (int j = 0; j < k.S; ++j) cv[(size_t)t * k.S + j] = j < n ? d.vtag[row_entry(d.cv, k.N, c, j)] : -1;
 }
-__global__ void import_targets_kernel(const Dev d, const Consts k, const double* __restrict__ A0, const double* __restrict__ P0) {
+// which = 0: (A0_i, P0_i) <- (a, b); which = 1: (K_A,i, K_P,i) <- (a, b); user order in, internal order out.
+// a == NULL restores the uniform pair; keep = 0 starts from the uniform values of avm_params.
+__global__ void import_cell_params_kernel(const Dev d, const Consts k, const double* __restrict__ a, const double* __restrict__ b,
+                                          const int which, const int keep) {
   const int c = blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= k.N) return;
   const int t = d.ctag[c];
-  d.tgt[c] = make_double2(A0[t], P0[t]);
+  CellPar q;
+  if (keep) q = d.par[c];
+  else { q.A0 = k.A0; q.P0 = k.P0; q.KA = k.KA; q.KP = k.KP; }
+  if (which == 0) { q.A0 = a ? a[t] : k.A0; q.P0 = a ? b[t] : k.P0; }
+  else { q.KA = a ? a[t] : k.KA; q.KP = a ? b[t] : k.KP; }
+  d.par[c] = q;
 }
+// overwrites the positions; the unwrapped positions and the MSD reference restart from them
 __global__ void import_positions_kernel(const Dev d, const Consts k, const double* pos) {
   const int v = blockIdx.x * blockDim.x + threadIdx.x;
   if (v >= k.V) return;
   const int t = d.vtag[v];
   d.pos[v] = make_double2(pos[2 * t], pos[2 * t + 1]);
+  d.msd_ref[t] = d.pos[v];
+  d.img[t] = make_int2(0, 0);
 }
 
 inline int cdiv(long long a, int b) { return (int)((a + b - 1) / b); }
+
+// the current unwrapped positions become the reference of the mean-square displacement
+__global__ void msd_reset_kernel(const Dev d, const Consts k) {
+  const int v = blockIdx.x * blockDim.x + threadIdx.x;
+  if (v >= k.V) return;
+  const int t = d.vtag[v];
+  const double2 h = d.pos[v];
+  const int2 im = d.img[t];
+  d.msd_ref[t] = make_double2(h.x + (double)im.x * k.Lx, h.y + (double)im.y * k.Ly);
+}
 
 int do_sort(avm_sim* s) {
   const Dev a = s->dev(), b = s->dev_alt();
@@ -300,10 +328,12 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
     s->pos[i] = (double2*)(w + L.pos[i]);
     BufferSet& b = s->set[i];
     b.vn = (int*)(w + L.vn[i]); b.vc = (int*)(w + L.vc[i]); b.cv = (int4*)(w + L.cv[i]);
-    b.cvn = (int*)(w + L.cvn[i]); b.theta = (double*)(w + L.theta[i]); b.rec = (CellRec*)(w + L.rec[i]); b.tgt = (double2*)(w + L.tgt[i]);
+    b.cvn = (int*)(w + L.cvn[i]); b.theta = (double*)(w + L.theta[i]); b.rec = (CellRec*)(w + L.rec[i]); b.par = (CellPar*)(w + L.par[i]);
     b.vtag = (int*)(w + L.vtag[i]); b.ctag = (int*)(w + L.ctag[i]);
     s->sc.key[i] = (unsigned int*)(w + L.key[i]); s->sc.val[i] = (int*)(w + L.val[i]);
   }
+  s->img = (int2*)(w + L.img); s->msd_ref = (double2*)(w + L.msd_ref);
+  s->tgt_custom = s->mod_custom = false;
   s->minkey = (unsigned long long*)(w + L.minkey);
   s->cand = (Cand*)(w + L.cand);
   s->ctr = (Counters*)(w + L.ctr);
@@ -581,6 +611,7 @@ int avm_observe(avm_sim* s, avm_observables* out) {
   out->area_variance = c.obs[5] / N - (c.obs[1] / N) * (c.obs[1] / N);
   out->area_min = c.obs[6];
   out->area_max = c.obs[7];
+  out->msd = c.obs[8] / (double)s->k.V;
   out->step = (int64_t)s->step;
   out->t1_flips = c.t1_flips;
   return AVM_OK;
@@ -636,12 +667,27 @@ int avm_set_positions(avm_sim* s, const double* pos_xy) {
   return AVM_OK;
 }
 
-int avm_set_cell_targets(avm_sim* s, const double* area0, const double* perimeter0) {
-  if (!s || ((area0 == nullptr) != (perimeter0 == nullptr))) return AVM_EINVAL;
-  s->k.per_cell = area0 ? 1 : 0;
+static int set_cell_params(avm_sim* s, const double* a, const double* b, int which) {
+  if (!s || ((a == nullptr) != (b == nullptr))) return AVM_EINVAL;
+  const int keep = s->k.per_cell;
+  (which == 0 ? s->tgt_custom : s->mod_custom) = a != nullptr;
   const Dev d = s->dev();
-  if (area0) { import_targets_kernel<<<cdiv(s->k.N, 256), 256, 0, s->stream>>>(d, s->k, area0, perimeter0); ++s->launches; }
-  s->launches += launch_refresh_cells(d, s->k, s->stream);   // the cached records hold (A - A0_i), (P - P0_i)
+  import_cell_params_kernel<<<cdiv(s->k.N, 256), 256, 0, s->stream>>>(d, s->k, a, b, which, keep);
+  ++s->launches;
+  s->k.per_cell = (s->tgt_custom || s->mod_custom) ? 1 : 0;
+  s->launches += launch_refresh_cells(s->dev(), s->k, s->stream);   // the cached records hold 2 K_A,i (A - A0_i), 2 K_P,i (P - P0_i)
+  AVM_CUDA(cudaPeekAtLastError());
+  return AVM_OK;
+}
+
+int avm_set_cell_targets(avm_sim* s, const double* area0, const double* perimeter0) { return set_cell_params(s, area0, perimeter0, 0); }
+
+int avm_set_cell_moduli(avm_sim* s, const double* KA, const double* KP) { return set_cell_params(s, KA, KP, 1); }
+
+int avm_msd_reset(avm_sim* s) {
+  if (!s) return AVM_EINVAL;
+  msd_reset_kernel<<<cdiv(s->k.V, 256), 256, 0, s->stream>>>(s->dev(), s->k);
+  ++s->launches;
   AVM_CUDA(cudaPeekAtLastError());
   return AVM_OK;
 }

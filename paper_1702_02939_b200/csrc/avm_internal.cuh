@@ -17,6 +17,9 @@ namespace avm {
 //   nx = cos(theta_c), ny = sin(theta_c)   (director)
 struct __align__(32) CellRec { double a, p, nx, ny; };
 
+// Per-cell parameters of Eq. 1 (NEXT-4): preferred area / perimeter and moduli.
+struct __align__(32) CellPar { double A0, P0, KA, KP; };
+
 // One eligible T1 candidate (R10), decoded once by the detecting thread and reused by the flip.
 struct __align__(16) Cand {
   int v1, v2;           // v1 = endpoint with the smaller tag
@@ -41,7 +44,7 @@ struct Counters {
   unsigned int flip_done; // candidates decided so far
   unsigned int pad2[31];
   long long t1_short, t1_candidates, t1_flips, t1_blocked, overflow_rejects, error;
-  double obs[8];   // observables of the latest avm_energy / avm_observe call (slots: avm_step.cu)
+  double obs[16];  // observables of the latest avm_energy / avm_observe call (slots: avm_step.cu)
   // phase trace of the fused force/move launch (variant builds with -DAVM_TRACE only): tr = this launch's
   // min start / max phase-end times (ns, %globaltimer), tr_acc = sums of (phase end - start) over launches
   unsigned long long tr[8], tr_acc[8], tr2[80];
@@ -61,7 +64,7 @@ struct Consts {
   int clear_dirty;           // 1: the cell pass clears the bitmap the force/move launch of this step swept with
   int nw;                    // words per dirty bitmap (V/32 rounded up to a multiple of 32)
   int fm_grid;               // CTAs of the persistent force/move grid (a whole number per SM, set at create)
-  int per_cell;              // 1: preferred values A0_i, P0_i per cell (Dev::tgt, Eq. 1), 0: uniform A0, P0 (Eq. A1)
+  int per_cell;              // 1: A0_i, P0_i, K_A,i, K_P,i per cell (Dev::par, Eq. 1), 0: the uniform values of Eq. A1
   int cap_a;                 // capacity of the step's candidate list (3N: every edge of the tiling)
   unsigned long long seed;
   uint2 rkey[10];            // Philox round keys of `seed` (the key schedule is uniform: done once on the host)
@@ -91,7 +94,9 @@ struct Dev {
   unsigned int* dirty; // [2][nw] bit v of buffer (s & 1): vertex v belongs to a cell of a T1 candidate found in
                        // step s.  Written only by the cell pass of step s, read only by the force/move launch
                        // of step s+1 (read-only for that whole launch), cleared by the cell pass of step s+1.
-  double2* tgt;       // [N] (A0_i, P0_i), internal order; read only when Consts::per_cell (NEXT-4)
+  CellPar* par;       // [N] (A0_i, P0_i, K_A,i, K_P,i), internal order; read only when Consts::per_cell (NEXT-4)
+  int2* img;          // [V] USER order: how many box lengths each vertex has left through the boundary (NEXT-2, MSD)
+  double2* msd_ref;   // [V] USER order: unwrapped positions at the reference time of the mean-square displacement
   unsigned int* estamp; // [3*Vs] per directed half-edge (slot plane, owner vertex): id of the repeated pass that tested it last
   Counters* ctr;
   unsigned int* feedback; // mapped HOST word: every force/move launch reports the candidate count of the previous step
@@ -121,9 +126,22 @@ __device__ __forceinline__ int row_entry(const int4* cv, int N, int c, int j) {
   return reinterpret_cast<const int*>(cv + (size_t)(j >> 2) * N + c)[j & 3];
 }
 
-// preferred (area, perimeter) of cell c: Eq. 1 per cell or the uniform pair of Eq. A1
-__device__ __forceinline__ double2 cell_targets(const Dev& d, const Consts& k, int c) {
-  return k.per_cell ? d.tgt[c] : make_double2(k.A0, k.P0);
+// parameters of cell c: Eq. 1 per cell or the uniform values of Eq. A1
+__device__ __forceinline__ CellPar cell_params(const Dev& d, const Consts& k, int c) {
+  if (k.per_cell) return d.par[c];
+  CellPar q; q.A0 = k.A0; q.P0 = k.P0; q.KA = k.KA; q.KP = k.KP;
+  return q;
+}
+// the cached record of a cell from its area and perimeter: a = 2 K_A (A - A0), p = 2 K_P (P - P0) (Eq. A3)
+__device__ __forceinline__ void rec_from_geometry(const CellPar& q, double A, double P, double& a, double& p) {
+  a = (2.0 * q.KA) * (A - q.A0);
+  p = (2.0 * q.KP) * (P - q.P0);
+}
+// Image counts of a wrapped coordinate (NEXT-2): wrap_box with the number of box lengths added
+__device__ __forceinline__ double wrap_box_count(double x, double L, int& n) {
+  if (x < 0.0) { x += L; --n; }
+  if (x >= L) { x -= L; ++n; }
+  return x;
 }
 
 // Square roots of squared lengths.  Every squared length in this library is formed as

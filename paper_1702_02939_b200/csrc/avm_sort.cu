@@ -227,7 +227,7 @@ __global__ void permute_cells_kernel(const Dev a, const Dev b, const Consts k, c
   b.cvn[i] = n;
   b.theta[i] = a.theta[o];
   b.rec[i] = a.rec[o];
-  if (k.per_cell) b.tgt[i] = a.tgt[o];
+  if (k.per_cell) b.par[i] = a.par[o];
   b.ctag[i] = a.ctag[o];
   for (int q = 0; q < k.S / 4; ++q) {
     const int4 src = a.cv[(size_t)q * k.N + o];

@@ -149,8 +149,13 @@ __device__ __forceinline__ void move_vertex(const Dev& d, const Consts& k, int v
   double x = __fma_rn(k.dt, vx, h.x), y = __fma_rn(k.dt, vy, h.y);
   // negative, >= L (conservatively) and non-finite values all have a large unsigned high word
   if ((hi_word(x) >= hi_word(k.Lx)) | (hi_word(y) >= hi_word(k.Ly))) {
-    x = wrap_box(x, k.Lx); y = wrap_box(y, k.Ly);
+    int ix = 0, iy = 0;
+    x = wrap_box_count(x, k.Lx, ix); y = wrap_box_count(y, k.Ly, iy);
     if (!(isfinite(x) && isfinite(y))) atomicOr((unsigned long long*)&d.ctr->error, 1ull);
+    if (ix | iy) {                      // the vertex left through the boundary: keep its unwrapped position (MSD)
+      int2* im = d.img + d.vtag[v];
+      int2 c = *im; c.x += ix; c.y += iy; *im = c;
+    }
   }
   d.pos_next[v] = make_double2(x, y);
 }
@@ -654,9 +659,8 @@ cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts
   }
   if (!valid) return;
   CellRec r;
-  const double2 tg = kPerCell ? d.tgt[c] : make_double2(k.A0, k.P0);   // Eq. 1 per cell (NEXT-4) / Eq. A1
-  r.a = k.KA2 * (__dmul_rn(0.5, acc) - tg.x);
-  r.p = k.KP2 * (per - tg.y);
+  if (kPerCell) rec_from_geometry(d.par[c], __dmul_rn(0.5, acc), per, r.a, r.p);   // Eq. 1 per cell (NEXT-4)
+  else { r.a = k.KA2 * (__dmul_rn(0.5, acc) - k.A0); r.p = k.KP2 * (per - k.P0); }   // Eq. A1
   r.nx = cs; r.ny = sn;
   st_rec(d.rec + c, r);
   smask &= n >= 32 ? ~0u : (1u << n) - 1u;     // edges beyond the closing one are padding
@@ -815,6 +819,16 @@ __device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Const
   //          -> ([w, y, z]; [C1, C2, C']), z = partner's old x, C' = partner's old C1 (R12);
   // outer vertices: x1 was joined to v1 and is now joined to v2 (same slot), x2 likewise.
   // Lane 0 rewrites v1, lane 1 v2, lane 2 x1, lane 3 x2.
+  if (t < 2) {
+    // unwrapped positions (MSD): the end point moved from h to (m -+ half p) before wrapping; count the box lengths
+    const double ux = t == 0 ? mx - half * px : h2.x - 0.5 * dx + half * px, uy = t == 0 ? my - half * py : h2.y - 0.5 * dy + half * py;
+    const double2 nn = t == 0 ? n1 : n2;
+    const int ix = __double2int_rn((ux - nn.x) / k.Lx), iy = __double2int_rn((uy - nn.y) / k.Ly);
+    if (ix | iy) {
+      int2* im = d.img + d.vtag[t == 0 ? v1 : v2];
+      int2 c = *im; c.x += ix; c.y += iy; *im = c;     // unwrapped = wrapped + count x L
+    }
+  }
   if (t == 0) {
     const int a1 = (k1 + 1) % 3, b1 = (k1 + 2) % 3;
     d.pos[v1] = n1;
@@ -891,9 +905,8 @@ __device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Const
   }
   geom_edge(rxp, ryp, 0.0, 0.0, acc, per);      // the closing edge back to entry 0
   AVM_TR_W0(4, (int)acc);
-  const double2 tg = cell_targets(d, k, cell);
-  d.rec[cell].a = k.KA2 * (__dmul_rn(0.5, acc) - tg.x);
-  d.rec[cell].p = k.KP2 * (per - tg.y);
+  if (k.per_cell) rec_from_geometry(d.par[cell], __dmul_rn(0.5, acc), per, d.rec[cell].a, d.rec[cell].p);
+  else { d.rec[cell].a = k.KA2 * (__dmul_rn(0.5, acc) - k.A0); d.rec[cell].p = k.KP2 * (per - k.P0); }
   AVM_TR_W0(5, 0);
 #ifdef AVM_TRACE
   if (trq && blockIdx.x == 0 && threadIdx.x < 32) d.ctr->tr2[48 + threadIdx.x] = gtime() - tqe;
@@ -988,8 +1001,10 @@ __global__ void forces_kernel(const Dev d, const Consts k, const double2* __rest
   for (int s = 0; s < 3; ++s) {
     q[s] = d.pos[d.vn[s * k.Vs + v]];
     const int cell = d.vc[s * k.Vs + v];
-    const double2 a = ap[cell], tg = cell_targets(d, k, cell);
-    c[s].a = k.KA2 * (a.x - tg.x); c[s].p = k.KP2 * (a.y - tg.y); c[s].nx = 0.0; c[s].ny = 0.0;
+    const double2 a = ap[cell];
+    if (k.per_cell) rec_from_geometry(d.par[cell], a.x, a.y, c[s].a, c[s].p);
+    else { c[s].a = k.KA2 * (a.x - k.A0); c[s].p = k.KP2 * (a.y - k.P0); }
+    c[s].nx = 0.0; c[s].ny = 0.0;
   }
   const double2 f = vertex_force(h, q[0], q[1], q[2], c[0], c[1], c[2], k);
   const int t = d.vtag[v];
@@ -999,11 +1014,12 @@ __global__ void forces_kernel(const Dev d, const Consts k, const double2* __rest
 // Observables of the current state (NEXT-2): energy, Eq. 1 / A1, and the
 // per-cell statistics a user of the model measures (shape index P / sqrt(A), area moments).
 // Slots: 0 energy, 1 sum A, 2 sum P, 3 sum P/sqrt(A) over cells with A > 0, 4 number of cells with
-// A <= 0, 5 sum A^2, 6 min A, 7 max A.  Block partials in a fixed order, finished by one block
-// (deterministic, no floating-point atomics).
-static constexpr int kObs = 8;
+// A <= 0, 5 sum A^2, 6 min A, 7 max A, 8 sum over vertices of the squared unwrapped displacement since the
+// MSD reference.  Block partials in a fixed order, finished by one block (deterministic, no
+// floating-point atomics).
+static constexpr int kObs = 9;
 __device__ __forceinline__ double obs_combine(int slot, double a, double b) {
-  return slot < 6 ? a + b : slot == 6 ? fmin(a, b) : fmax(a, b);
+  return slot == 6 ? fmin(a, b) : slot == 7 ? fmax(a, b) : a + b;
 }
 __device__ __forceinline__ void obs_block_reduce(double (&x)[kObs], double (*sm)[256]) {
 #pragma unroll
@@ -1019,16 +1035,24 @@ __device__ __forceinline__ void obs_block_reduce(double (&x)[kObs], double (*sm)
 __global__ void __launch_bounds__(256)
 observables_partial_kernel(const Dev d, const Consts k, double* __restrict__ partial) {
   __shared__ double sm[kObs][256];
-  double x[kObs] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 1.0e300, -1.0e300};
+  double x[kObs] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 1.0e300, -1.0e300, 0.0};
   for (int c = blockIdx.x * 256 + threadIdx.x; c < k.N; c += gridDim.x * 256) {
     double A, P;
     cell_area_perimeter(d.pos, d.cv, c, d.cvn[c], k, A, P);
-    const double2 tg = cell_targets(d, k, c);
-    x[0] += k.KA * (A - tg.x) * (A - tg.x) + k.KP * (P - tg.y) * (P - tg.y);
+    const CellPar q = cell_params(d, k, c);
+    x[0] += q.KA * (A - q.A0) * (A - q.A0) + q.KP * (P - q.P0) * (P - q.P0);
     x[1] += A; x[2] += P;
     if (A > 0.0) x[3] += P / sqrt(A); else x[4] += 1.0;
     x[5] += A * A;
     x[6] = fmin(x[6], A); x[7] = fmax(x[7], A);
+  }
+  // mean-square displacement: unwrapped position = wrapped position + image count x box length
+  for (int v = blockIdx.x * 256 + threadIdx.x; v < k.V; v += gridDim.x * 256) {
+    const int t = d.vtag[v];
+    const double2 h = d.pos[v], r0 = d.msd_ref[t];
+    const int2 im = d.img[t];
+    const double dx = (h.x + (double)im.x * k.Lx) - r0.x, dy = (h.y + (double)im.y * k.Ly) - r0.y;
+    x[8] += dx * dx + dy * dy;
   }
   obs_block_reduce(x, sm);
   if (threadIdx.x < kObs) partial[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = sm[threadIdx.x][0];
@@ -1036,7 +1060,7 @@ observables_partial_kernel(const Dev d, const Consts k, double* __restrict__ par
 __global__ void __launch_bounds__(256)
 observables_final_kernel(const Dev d, const double* __restrict__ partial, int n) {
   __shared__ double sm[kObs][256];
-  double x[kObs] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 1.0e300, -1.0e300};
+  double x[kObs] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 1.0e300, -1.0e300, 0.0};
   for (int i = threadIdx.x; i < n; i += 256)
 #pragma unroll
     for (int q = 0; q < kObs; ++q) x[q] = obs_combine(q, x[q], partial[(size_t)q * n + i]);

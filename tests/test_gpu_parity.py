@@ -626,3 +626,134 @@ def test_fused_schedule_with_resorts_against_the_oracle_at_fused_size(B):
         assert_states_match(sg, o.get_state(), t.Lx, t.Ly)
         assert sg["stats"]["n_sorts"] == 3 and sg["stats"]["t1_flips"] > 10000
         g.close()
+
+
+def test_sub_step_order_on_gpu(B):
+    """GPU twins of the oracle's R7 / R6 pins: the move uses the directors of the start of the step
+    (closed form with Dr > 0), and an edge brought below l_c by the move flips in that very step."""
+    t = tiling(0)
+    v0, dt, Dr, seed = 0.7, 0.01, 2.0, 11
+    g = B.from_tiling(t, KA=0.0, KP=0.0, v0=v0, Dr=Dr, dt=dt, l_c=0.0, seed=seed)
+    th1 = t.theta + np.sqrt(2 * Dr * dt) * oracle.director_noise(seed, 0, 0, t.N)
+
+    def drift(th):
+        n = np.stack([np.cos(th), np.sin(th)], axis=1)
+        return dt * v0 / 3.0 * n[t.vertex_cell_neighbors].sum(axis=1)
+    g.step(1)
+    s1 = to_np(g.get_state())
+    assert_positions_close(s1["pos"], np.mod(t.pos + drift(t.theta), [t.Lx, t.Ly]), t.Lx, t.Ly, 1e-14)
+    assert np.abs(s1["theta"] - th1).max() < 1e-14
+    g.step(1)
+    s2 = to_np(g.get_state())
+    assert_positions_close(s2["pos"], np.mod(s1["pos"] + drift(s1["theta"]), [t.Lx, t.Ly]), t.Lx, t.Ly, 1e-14)
+    # R6: same construction as tests/test_oracle_integrator.py
+    from tests.test_oracle_t1 import edge_cells_from_rows, shrink_edge
+    l_c, dt, v0 = 0.04, 0.01, 0.9
+    hx = w.hex_tiling(6, 4, a=1.0)
+    v1 = 7
+    v2 = int(hx.vertex_neighbors[v1, 1])
+    lo, hi = min(v1, v2), max(v1, v2)
+    L, R, E1, E2 = edge_cells_from_rows(hx.cell_vertex_num, hx.cell_vertices, hx.vertex_cell_neighbors, lo, hi)
+    closing = dt * 2.0 * v0 / 3.0
+    pos, m, u = shrink_edge(hx, lo, hi, l_c + 0.5 * closing)
+    theta = np.zeros(hx.N)
+    theta[E1], theta[E2] = np.arctan2(u[1], u[0]), np.arctan2(-u[1], -u[0])
+    theta[L] = theta[R] = 0.3
+    tt = w.Tiling(hx.Lx, hx.Ly, hx.S, pos, hx.cell_vertex_num, hx.cell_vertices, hx.vertex_neighbors,
+                  hx.vertex_cell_neighbors, theta)
+    for sched in ("fused", "unfused"):
+        g = B.from_tiling(tt, KA=0.0, KP=0.0, v0=v0, Dr=0.0, dt=dt, l_c=l_c, schedule=sched)
+        cand, _ = g.debug_t1()
+        assert len(cand) == 0
+        g.step(1)
+        s = to_np(g.get_state())
+        assert s["stats"]["t1_short"] == 1 and s["stats"]["t1_flips"] == 1
+        assert h.cells_adjacent(s["cell_vertices"], s["cell_vertex_num"], E1, E2)
+
+
+def test_repeated_passes_overflow_on_a_later_pass(B):
+    """GPU twin of the oracle pin: t1_short / overflow_rejects are first-pass statistics, the sticky
+    error bit 2 is raised by whichever pass first sees the overflow (local re-detection included)."""
+    from tests.test_oracle_t1 import overflow_on_a_later_pass_case
+    tt, kw, E, _ = overflow_on_a_later_pass_case()
+    for passes in (4, 1):
+        g = B.from_tiling(tt, t1_max_passes=passes, **kw)
+        o = oracle.from_tiling(tt, t1_max_passes=passes, **kw)
+        for _ in range(2):
+            g.step(1)
+            o.step(1)
+            assert_states_match(to_np(g.get_state()), o.get_state(), tt.Lx, tt.Ly)
+        assert o.get_state()["stats"]["error"] == 2
+
+
+@pytest.mark.parametrize("k,steps,sort_every", [(0, 60, 0), (1, 24, 7)])
+def test_per_cell_moduli_match_the_oracle(B, k, steps, sort_every):
+    """NEXT-4: per-cell K_A,i, K_P,i together with per-cell targets (Eq. 1): forces within 1e-10,
+    trajectory within 1e-8 with bit-exact topology (re-sorts included), energy; each pair can be
+    switched back to the uniform values independently."""
+    t = tiling(k)
+    p = w.config_params(k)
+    rng = np.random.default_rng(12)
+    soft = rng.random(t.N) < 0.5
+    KA, KP = np.where(soft, 0.4, 1.7), np.where(soft, 0.6, 1.2)
+    A0, P0 = np.where(soft, 1.2, 0.8), np.where(soft, 3.9 * np.sqrt(1.2), 3.7 * np.sqrt(0.8))
+    g = B.from_tiling(t, **dict(p, sort_every=sort_every, sort_at_create=True))
+    o = oracle.from_tiling(t, **p)
+    g.set_cell_moduli(KA, KP)
+    o.set_cell_moduli(KA, KP)
+    F, ap = g.compute_forces()
+    Fo, apo = o.compute_forces()
+    assert_forces_close(F.cpu().numpy(), Fo, ap.cpu().numpy(), apo)
+    g.set_cell_targets(A0, P0)
+    o.set_cell_targets(A0, P0)
+    F, ap = g.compute_forces()
+    Fo, apo = o.compute_forces()
+    assert_forces_close(F.cpu().numpy(), Fo, ap.cpu().numpy(), apo)
+    assert abs(g.energy() - o.energy()) <= 1e-10 * abs(o.energy())
+    g.step(steps)
+    o.step(steps)
+    assert_states_match(to_np(g.get_state()), o.get_state(), t.Lx, t.Ly)
+    assert abs(g.energy() - o.energy()) <= 1e-8 * abs(o.energy())
+    assert o.get_state()["stats"]["t1_flips"] > 0
+    g.set_cell_targets(None, None)           # moduli stay heterogeneous
+    o.set_cell_targets(None, None)
+    F, ap = g.compute_forces()
+    Fo, apo = o.compute_forces()
+    assert_forces_close(F.cpu().numpy(), Fo, ap.cpu().numpy(), apo)
+    g.set_cell_moduli(None, None)
+    o.set_cell_moduli(None, None)
+    F, ap = g.compute_forces()
+    Fo, apo = o.compute_forces()
+    assert_forces_close(F.cpu().numpy(), Fo, ap.cpu().numpy(), apo)
+    g.step(5)
+    o.step(5)
+    assert_states_match(to_np(g.get_state()), o.get_state(), t.Lx, t.Ly)
+
+
+@pytest.mark.parametrize("sched", ["fused", "unfused"])
+def test_mean_square_displacement_matches_the_oracle(B, sched):
+    """NEXT-2: MSD from the image counts the library keeps (vertices leave through the box boundary, T1s
+    reposition their end points, the Hilbert re-sort permutes everything) against the oracle's
+    unwrapped positions; closed-form pure-activity translation; reset."""
+    t = tiling(0)
+    p = dict(w.config_params(0), v0=3.0, Dr=0.2, sort_every=11, sort_at_create=True, schedule=sched)
+    g = B.from_tiling(t, **p)
+    o = oracle.from_tiling(t, **p)
+    assert g.observe()["msd"] == 0.0
+    for n in (1, 9, 90, 200):
+        g.step(n)
+        o.step(n)
+        a, b = g.observe()["msd"], o.msd()
+        assert abs(a - b) <= 1e-9 * max(b, 1e-12), (n, a, b)
+    assert o.get_state()["stats"]["t1_flips"] > 0 and b > 0.5
+    g.msd_reset()
+    o.msd_reset()
+    assert g.observe()["msd"] == 0.0
+    g.step(30)
+    o.step(30)
+    assert abs(g.observe()["msd"] - o.msd()) <= 1e-9 * o.msd()
+    th0 = 2.1
+    hx = w.hex_tiling(6, 4, a=1.0, theta=np.full(24, th0))
+    g = B.from_tiling(hx, KA=0.0, KP=0.0, v0=0.8, Dr=0.0, dt=0.01, l_c=0.0, schedule=sched)
+    g.step(1500)
+    assert abs(g.observe()["msd"] - 144.0) < 1e-9 * 144.0
