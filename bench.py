@@ -39,6 +39,10 @@ NOMINAL_PEAK_GBS = 8000.0     # north_star: "B200 peak (about 8 TB/s)"
 BYTES_FORCE_MOVE_PER_VERTEX = 72.0
 BYTES_CELL_UPDATE_PER_CELL = 112.0
 SURVEY_BYTES_PER_VERTEX_STEP = 134.0
+# --precision mixed (libavm_b200_mixed.so, NEXT-3; never the headline): positions 8 B, records 16 B
+#   force_move : pos 8 + 12 + 12 + pos_next 8 + records 16 B/cell = 8 B/vertex  -> 48 B/vertex
+#   cell_update: 4 + 4 + theta 8+8 + record write 16 + rows 24 + positions 2 x 8 -> 80 B/cell
+BYTES_MIXED = (48.0, 80.0)
 
 
 def workload_string(cfg, N, V):
@@ -205,6 +209,8 @@ def main():
     ap.add_argument("--t1-passes", type=int, default=1,
                     help="T1 passes per step: 1 = north_star's rule (default, the headline), P > 1 = repeat until none (NEXT-1)")
     ap.add_argument("--schedule", default="auto", choices=["auto", "fused", "unfused"])
+    ap.add_argument("--precision", default="f64", choices=["f64", "mixed"],
+                    help="f64 = the default library and the headline; mixed = libavm_b200_mixed.so (reduced-precision storage, NEXT-3)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
 
@@ -232,13 +238,15 @@ def main():
         torch.cuda.synchronize()
 
     cfg = w.CONFIGS[args.config]
-    p = dict(w.config_params(args.config), device=local_rank, schedule=args.schedule)
+    p = dict(w.config_params(args.config), device=local_rank, schedule=args.schedule, precision=args.precision)
     if args.t1_passes > 1:
         p["t1_max_passes"] = args.t1_passes
     t = w.config_tiling(args.config)
     N, V = t.N, t.V
     peak, peak_src = measured_peaks()
     kbytes = {"force_move": BYTES_FORCE_MOVE_PER_VERTEX * V, "cell_update": BYTES_CELL_UPDATE_PER_CELL * N}
+    if args.precision == "mixed":
+        kbytes = {"force_move": BYTES_MIXED[0] * V, "cell_update": BYTES_MIXED[1] * N}
     step_bytes = sum(kbytes.values())
     survey_step_bytes = SURVEY_BYTES_PER_VERTEX_STEP * V
 
@@ -293,7 +301,7 @@ def main():
     per_launch_ms = {k: v / max(1, prof_steps) for k, v in prof.items()}
     dom = max(kbytes, key=lambda k: per_launch_ms[k])
     ach = kbytes[dom] / (per_launch_ms[dom] * 1e-3) / 1e9
-    cap = ncu_capture(dom, cfg["name"])
+    cap = ncu_capture(dom, cfg["name"] + ("_steady" if args.warmup >= 300 else "")) if args.precision == "f64" else None
     traffic = (float(cap["dram_bytes_read_per_launch"]) + float(cap["dram_bytes_write_per_launch"])) if cap else None
     roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                 "frac_of_nominal_8TBps": ach / NOMINAL_PEAK_GBS,
@@ -371,7 +379,7 @@ def main():
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle
-        o = oracle.from_tiling(t, **p)
+        o = oracle.from_tiling(t, **{a: b for a, b in p.items() if a not in ("precision", "schedule", "device")})
         est = 0.7e-6 * N                                       # s per step, one core
         n_o = max(20, min(400, int(15.0 / est)))
         skip = 50 if est * 50 < 60.0 else max(0, int(60.0 / est))   # cfg4: the skip itself is capped at ~60 s
@@ -388,8 +396,9 @@ def main():
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_string(cfg, N, V),
+            "dtype": "f64" if args.precision == "f64" else "f64 arithmetic on fixed-point-32 positions and f32 cell records",
+            "data": "synthetic",
+            "config": {"workload": workload_string(cfg, N, V), "precision": args.precision,
                        "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "t1_passes_per_step": args.t1_passes, "schedule": args.schedule,
                        "l2": f"inputs larger than L2: resident state {224 * N / 1e6:.0f} MB vs 126 MB L2" if 224 * N > 126e6

@@ -216,6 +216,35 @@ void avm_destroy(avm_sim* sim);
 const char* avm_strerror(int code);
 const char* avm_last_cuda_error(void);
 
+/* Storage precision of the library that was loaded: "f64" (libavm_b200.so, the default and the
+ * timed path: positions double2, cell records 4 doubles, everything fp64) or "mixed"
+ * (libavm_b200_mixed.so: the same sources and the same C ABI built with -DAVM_MIXED=1; SURVEY.md
+ * section 8(f) NEXT-3, after the single-precision variant of PAPER.md:120).
+ *
+ * The mixed library changes STORAGE only; every arithmetic operation of the step stays fp64:
+ *   - positions are held on a fixed-point grid of 2^-32 box lengths per axis (8 bytes per vertex
+ *     instead of 16): a position handed to the library, moved by a step or set by a T1 is rounded
+ *     to the nearest grid point, an absolute error of at most L * 2^-33 per coordinate
+ *     (1.2e-7 at L = 1024, 9.3e-10 at L = 8);
+ *   - the cached cell records 2 K_A (A - A0), 2 K_P (P - P0), cos theta, sin theta are floats
+ *     (16 bytes per cell instead of 32): a relative error of at most 2^-24 each.
+ *   theta, the topology lists, tags, Philox and all user-visible arrays are unchanged (doubles in and out).
+ * Accuracy contract against the float64 oracle, from an identical state whose positions lie on
+ * the grid (tests/test_gpu_mixed.py):
+ *   - areas and perimeters (avm_compute_forces): 1e-10 relative, as in the default library;
+ *   - forces of avm_compute_forces: 1e-10 relative (they do not go through the cached records);
+ *     the force applied inside avm_step: 1e-6 relative to max(|F_v|, rms |F|);
+ *   - one step: positions within L * 2^-32 + 1e-6 dt max|F| of the oracle's for every vertex that no T1
+ *     repositioned (the end points of a T1 land on the old edge turned by 90 degrees, and the direction
+ *     of an old edge of length l is only defined to (grid unit / l): they stay within the new edge length),
+ *     theta within the 1e-8 of the default library;
+ *   - T1 candidate and winner sets of the moved state: equal outside the band | l - l_c | < 4 L 2^-32;
+ *   - trajectories are not comparable step for step beyond a few T1 events (the model is chaotic);
+ *     total area = Lx Ly to 1e-9 relative and all topological invariants hold at any length.
+ * The run is deterministic and resumes bit-identically from avm_get_state (exported positions are
+ * grid points and pack to themselves). */
+const char* avm_precision(void);
+
 #ifdef __cplusplus
 }
 #endif

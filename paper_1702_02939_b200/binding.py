@@ -17,13 +17,15 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 # AVM_B200_LIB overrides the location (an alternative build of the same library)
 LIB_PATH = os.environ.get("AVM_B200_LIB") or os.path.join(_HERE, "libavm_b200.so")
+# the same ABI with reduced-precision storage (NEXT-3); loaded on demand, never the default
+LIB_MIXED_PATH = os.path.join(_HERE, "libavm_b200_mixed.so")
 
 # every symbol include/avm.h declares (tests check that the library exports all of them)
 ABI_SYMBOLS = [
     "avm_workspace_bytes", "avm_create", "avm_create_host", "avm_step", "avm_step_profile", "avm_compute_forces",
     "avm_compute_forces_host", "avm_energy", "avm_observe", "avm_set_cell_targets", "avm_set_cell_moduli", "avm_msd_reset", "avm_get_state", "avm_get_state_host", "avm_debug_t1",
     "avm_t1_pass", "avm_set_positions", "avm_resort", "avm_philox_words", "avm_hilbert_index",
-    "avm_hilbert_index_host", "avm_destroy", "avm_strerror", "avm_last_cuda_error",
+    "avm_hilbert_index_host", "avm_destroy", "avm_strerror", "avm_last_cuda_error", "avm_precision",
 ]
 
 AVM_FLAG_SORT_AT_CREATE = 1
@@ -65,12 +67,12 @@ class AvmError(RuntimeError):
     pass
 
 
-def _load() -> ctypes.CDLL:
-    if not os.path.exists(LIB_PATH):
+def _load(path: str = LIB_PATH) -> ctypes.CDLL:
+    if not os.path.exists(path):
         raise AvmError(
-            f"{LIB_PATH} is missing: build the CUDA library first (python -m paper_1702_02939_b200.build). "
+            f"{path} is missing: build the CUDA library first (python -m paper_1702_02939_b200.build). "
             "There is no CPU fallback.")
-    lib = ctypes.CDLL(LIB_PATH)
+    lib = ctypes.CDLL(path)
     p, i64, u64, i32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_uint64, ctypes.c_int32
     PP = ctypes.POINTER(AvmParams)
     lib.avm_workspace_bytes.restype = ctypes.c_size_t
@@ -103,10 +105,22 @@ def _load() -> ctypes.CDLL:
     lib.avm_strerror.argtypes = [ctypes.c_int]
     lib.avm_strerror.restype = ctypes.c_char_p
     lib.avm_last_cuda_error.restype = ctypes.c_char_p
+    lib.avm_precision.restype = ctypes.c_char_p
     return lib
 
 
 lib = _load()
+_LIBS = {"f64": lib}
+
+
+def library(precision: str = "f64") -> ctypes.CDLL:
+    """the C-ABI library for a storage precision: "f64" (default) or "mixed" (libavm_b200_mixed.so, NEXT-3)"""
+    if precision not in _LIBS:
+        if precision != "mixed":
+            raise AvmError(f"unknown precision {precision!r}")
+        _LIBS[precision] = _load(LIB_MIXED_PATH)
+    assert _LIBS[precision].avm_precision().decode() == precision
+    return _LIBS[precision]
 
 
 def _check(rc: int) -> None:
@@ -144,13 +158,15 @@ class AvmSim:
     """One simulation living on a CUDA device.  Tensors in/out are torch CUDA tensors (device
     entry points) or numpy arrays (``*_host`` entry points), always in user order."""
 
-    def __init__(self, tiling, params: AvmParams, host: bool = False):
+    def __init__(self, tiling, params: AvmParams, host: bool = False, precision: str = "f64"):
         import torch
         self.torch = torch
+        self.lib = library(precision)
+        self.precision = precision
         self.params = params
         self.N, self.V, self.S = params.n_cells, params.n_vertices, params.max_cell_vertices
         self.device = torch.device("cuda", params.device)
-        nbytes = lib.avm_workspace_bytes(ctypes.byref(params))
+        nbytes = self.lib.avm_workspace_bytes(ctypes.byref(params))
         if nbytes == 0:
             raise AvmError("avm_workspace_bytes rejected the parameters")
         self.workspace_bytes = int(nbytes)
@@ -168,11 +184,11 @@ class AvmSim:
         if host:
             self._inputs = arrays
             ptrs = [_hptr(a) for a in arrays]
-            fn = lib.avm_create_host
+            fn = self.lib.avm_create_host
         else:
             self._inputs = [torch.from_numpy(a).to(self.device) for a in arrays]
             ptrs = [_dptr(t) for t in self._inputs]
-            fn = lib.avm_create
+            fn = self.lib.avm_create
         _check(fn(ctypes.byref(params), *ptrs, ctypes.c_void_p(self.workspace.data_ptr()),
                   self.workspace_bytes, ctypes.c_void_p(self.stream.cuda_stream), ctypes.byref(self._h)))
         self._inputs = None
@@ -180,7 +196,7 @@ class AvmSim:
     def close(self):
         if getattr(self, "_h", None) and self._h.value:
             self.torch.cuda.synchronize(self.device)
-            lib.avm_destroy(self._h)
+            self.lib.avm_destroy(self._h)
             self._h = ctypes.c_void_p()
 
     def __del__(self):
@@ -191,32 +207,32 @@ class AvmSim:
 
     # ---- hot path ------------------------------------------------------------------------------
     def step(self, n: int = 1) -> None:
-        _check(lib.avm_step(self._h, n))
+        _check(self.lib.avm_step(self._h, n))
 
     KERNEL_NAMES = ("force_move", "cell_update", "t1_flip")
 
     def step_profile(self, n: int) -> dict:
         """n steps with every kernel bracketed by CUDA events; summed device ms per kernel class."""
         ms = (ctypes.c_double * len(self.KERNEL_NAMES))()
-        _check(lib.avm_step_profile(self._h, n, ms))
+        _check(self.lib.avm_step_profile(self._h, n, ms))
         return dict(zip(self.KERNEL_NAMES, list(ms)))
 
     def compute_forces(self):
         t = self.torch
         F = t.empty((self.V, 2), dtype=t.float64, device=self.device)
         ap = t.empty((self.N, 2), dtype=t.float64, device=self.device)
-        _check(lib.avm_compute_forces(self._h, _dptr(F), _dptr(ap)))
+        _check(self.lib.avm_compute_forces(self._h, _dptr(F), _dptr(ap)))
         return F, ap
 
     def compute_forces_host(self):
         F = np.empty((self.V, 2), dtype=np.float64)
         ap = np.empty((self.N, 2), dtype=np.float64)
-        _check(lib.avm_compute_forces_host(self._h, _hptr(F), _hptr(ap)))
+        _check(self.lib.avm_compute_forces_host(self._h, _hptr(F), _hptr(ap)))
         return F, ap
 
     def energy(self) -> float:
         e = ctypes.c_double(0.0)
-        _check(lib.avm_energy(self._h, ctypes.byref(e)))
+        _check(self.lib.avm_energy(self._h, ctypes.byref(e)))
         return e.value
 
     def _set_cell_pair(self, fn, a0, b0) -> None:
@@ -235,18 +251,18 @@ class AvmSim:
 
     def set_cell_targets(self, area0=None, perimeter0=None) -> None:
         """per-cell preferred area / perimeter (numpy or CUDA tensors, user order); None, None = uniform"""
-        self._set_cell_pair(lib.avm_set_cell_targets, area0, perimeter0)
+        self._set_cell_pair(self.lib.avm_set_cell_targets, area0, perimeter0)
 
     def set_cell_moduli(self, KA=None, KP=None) -> None:
         """per-cell moduli K_A,i / K_P,i (numpy or CUDA tensors, user order); None, None = uniform"""
-        self._set_cell_pair(lib.avm_set_cell_moduli, KA, KP)
+        self._set_cell_pair(self.lib.avm_set_cell_moduli, KA, KP)
 
     def msd_reset(self) -> None:
-        _check(lib.avm_msd_reset(self._h))
+        _check(self.lib.avm_msd_reset(self._h))
 
     def observe(self) -> dict:
         o = AvmObservables()
-        _check(lib.avm_observe(self._h, ctypes.byref(o)))
+        _check(self.lib.avm_observe(self._h, ctypes.byref(o)))
         return o.as_dict()
 
     def get_state(self, stats: bool = True) -> dict:
@@ -258,7 +274,7 @@ class AvmSim:
         vc = t.empty((self.V, 3), dtype=t.int32, device=self.device)
         th = t.empty(self.N, dtype=t.float64, device=self.device)
         st = AvmStats()
-        _check(lib.avm_get_state(self._h, _dptr(pos), _dptr(cvn), _dptr(cv), _dptr(vn), _dptr(vc), _dptr(th),
+        _check(self.lib.avm_get_state(self._h, _dptr(pos), _dptr(cvn), _dptr(cv), _dptr(vn), _dptr(vc), _dptr(th),
                                  ctypes.byref(st) if stats else None))
         return dict(pos=pos, cell_vertex_num=cvn, cell_vertices=cv, vertex_neighbors=vn,
                     vertex_cell_neighbors=vc, theta=th, stats=st.as_dict() if stats else None)
@@ -271,7 +287,7 @@ class AvmSim:
                        vertex_cell_neighbors=np.empty((self.V, 3), dtype=np.int32),
                        theta=np.empty(self.N, dtype=np.float64))
         st = AvmStats()
-        _check(lib.avm_get_state_host(self._h, _hptr(out.get("pos")), _hptr(out.get("cell_vertex_num")),
+        _check(self.lib.avm_get_state_host(self._h, _hptr(out.get("pos")), _hptr(out.get("cell_vertex_num")),
                                       _hptr(out.get("cell_vertices")), _hptr(out.get("vertex_neighbors")),
                                       _hptr(out.get("vertex_cell_neighbors")), _hptr(out.get("theta")),
                                       ctypes.byref(st)))
@@ -280,7 +296,7 @@ class AvmSim:
 
     def stats(self) -> dict:
         st = AvmStats()
-        _check(lib.avm_get_state(self._h, None, None, None, None, None, None, ctypes.byref(st)))
+        _check(self.lib.avm_get_state(self._h, None, None, None, None, None, None, ctypes.byref(st)))
         return st.as_dict()
 
     # ---- test hooks ----------------------------------------------------------------------------
@@ -289,27 +305,27 @@ class AvmSim:
         cand = np.empty((cap, 2), dtype=np.int32)
         win = np.empty((cap, 2), dtype=np.int32)
         nc, nw = ctypes.c_int64(0), ctypes.c_int64(0)
-        _check(lib.avm_debug_t1(self._h, _hptr(cand), ctypes.byref(nc), _hptr(win), ctypes.byref(nw), cap))
+        _check(self.lib.avm_debug_t1(self._h, _hptr(cand), ctypes.byref(nc), _hptr(win), ctypes.byref(nw), cap))
         return cand[:nc.value].copy(), win[:nw.value].copy()
 
     def t1_pass(self) -> None:
-        _check(lib.avm_t1_pass(self._h))
+        _check(self.lib.avm_t1_pass(self._h))
 
     def set_positions(self, pos) -> None:
         t = self.torch
         if isinstance(pos, np.ndarray):
             pos = t.from_numpy(np.ascontiguousarray(pos, dtype=np.float64)).to(self.device)
         assert pos.shape == (self.V, 2) and pos.dtype == t.float64 and pos.is_contiguous()
-        _check(lib.avm_set_positions(self._h, _dptr(pos)))
+        _check(self.lib.avm_set_positions(self._h, _dptr(pos)))
         t.cuda.current_stream(self.device).synchronize()   # keep `pos` alive until consumed
 
     def resort(self) -> None:
-        _check(lib.avm_resort(self._h))
+        _check(self.lib.avm_resort(self._h))
 
     def philox_words(self, seed: int, step: int, cell0: int, n: int):
         t = self.torch
         out = t.empty((n, 4), dtype=t.int32, device=self.device)
-        _check(lib.avm_philox_words(self._h, seed, step, cell0, n, _dptr(out)))
+        _check(self.lib.avm_philox_words(self._h, seed, step, cell0, n, _dptr(out)))
         return out.cpu().numpy().view(np.uint32)
 
     def hilbert_index(self, m: int, ix: np.ndarray, iy: np.ndarray) -> np.ndarray:
@@ -317,10 +333,10 @@ class AvmSim:
         dx = t.from_numpy(ix.astype(np.int64)).to(self.device).to(t.int32)
         dy = t.from_numpy(iy.astype(np.int64)).to(self.device).to(t.int32)
         out = t.empty(ix.shape[0], dtype=t.int32, device=self.device)
-        _check(lib.avm_hilbert_index(self._h, m, ix.shape[0], _dptr(dx), _dptr(dy), _dptr(out)))
+        _check(self.lib.avm_hilbert_index(self._h, m, ix.shape[0], _dptr(dx), _dptr(dy), _dptr(out)))
         return out.cpu().numpy().view(np.uint32)
 
 
-def from_tiling(tiling, host: bool = False, **params) -> AvmSim:
+def from_tiling(tiling, host: bool = False, precision: str = "f64", **params) -> AvmSim:
     p = make_params(tiling.N, tiling.S, **dict(params, Lx=tiling.Lx, Ly=tiling.Ly))
-    return AvmSim(tiling, p, host=host)
+    return AvmSim(tiling, p, host=host, precision=precision)

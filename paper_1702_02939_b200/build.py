@@ -15,6 +15,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libavm_b200.so")
+# same sources, reduced-precision storage (positions on a 2^-32 L grid, float records), fp64 arithmetic: NEXT-3
+LIB_MIXED = os.path.join(HERE, "libavm_b200_mixed.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
@@ -24,20 +26,22 @@ def sources():
     return sorted(glob.glob(os.path.join(CSRC, "*.cu")))
 
 
-def _stale() -> bool:
-    if not os.path.exists(LIB):
+def _stale(lib: str = LIB) -> bool:
+    if not os.path.exists(lib):
         return True
-    t = os.path.getmtime(LIB)
+    t = os.path.getmtime(lib)
     deps = sources() + glob.glob(os.path.join(CSRC, "*.cuh")) + [os.path.join(HERE, "..", "include", "avm.h")]
     return any(os.path.getmtime(d) > t for d in deps)
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    if force or _stale():
-        tmp = LIB + f".tmp{os.getpid()}"
-        cmd = [NVCC] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + sources()
-        subprocess.check_call(cmd)
-        os.replace(tmp, LIB)
+    """builds both libraries; returns the path of the default (fp64) one"""
+    for lib, defs in ((LIB, []), (LIB_MIXED, ["-DAVM_MIXED=1"])):
+        if force or _stale(lib):
+            tmp = lib + f".tmp{os.getpid()}"
+            cmd = [NVCC] + NVCC_FLAGS + defs + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + sources()
+            subprocess.check_call(cmd)
+            os.replace(tmp, lib)
     return LIB
 
 

@@ -45,7 +45,7 @@ struct BufferSet {
   int *vn, *vc, *cvn, *vtag, *ctag;
   int4* cv;
   double* theta;
-  CellRec* rec;
+  rec_t* rec;
   CellPar* par;
 };
 
@@ -62,7 +62,7 @@ Layout make_layout(const avm_params& p) {
   const size_t Vs = (size_t)plane_stride(p.n_vertices);
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
-  for (int i = 0; i < 2; ++i) L.pos[i] = take(16 * V);
+  for (int i = 0; i < 2; ++i) L.pos[i] = take(16 * V);      // also staging for user-layout doubles: fp64 size in every build
   for (int i = 0; i < 2; ++i) {
     L.vn[i] = take(12 * Vs); L.vc[i] = take(12 * Vs); L.cv[i] = take(4 * N * S); L.cvn[i] = take(4 * N);
     L.theta[i] = take(8 * N); L.rec[i] = take(32 * N); L.par[i] = take(32 * N); L.vtag[i] = take(4 * V); L.ctag[i] = take(4 * N);
@@ -101,7 +101,7 @@ struct avm_sim {
   cudaStream_t stream;
   char* ws;
   Layout L;
-  double2* pos[2];
+  pos_t* pos[2];
   BufferSet set[2];
   unsigned long long* minkey;
   Cand* cand;
@@ -151,13 +151,17 @@ namespace {
 // ---- creation-time kernels ---------------------------------------------------------------------
 // user layout (staged in the alternate buffer set: vn/vc [V][3], cv [N][S] row-major) -> internal
 // structure-of-arrays layout (vn/vc planes, cv int4 planes), tags, idle minimum keys
-__global__ void import_kernel(const Dev d, const Consts k, const int* __restrict__ vn_u, const int* __restrict__ vc_u,
-                              const int* __restrict__ cv_u) {
+__global__ void import_kernel(const Dev d, const Consts k, const double* __restrict__ pos_u, const int* __restrict__ vn_u,
+                              const int* __restrict__ vc_u, const int* __restrict__ cv_u) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < k.V) {
     d.vtag[i] = i;
+    const double2 h = make_double2(pos_u[2 * i], pos_u[2 * i + 1]);
+    const bool inside = h.x >= 0.0 && h.x < k.Lx && h.y >= 0.0 && h.y < k.Ly;
+    if (!inside) atomicOr((unsigned long long*)&d.ctr->error, 4ull);
+    pos_st(d.pos + i, inside ? h : make_double2(0.0, 0.0), k);
     d.img[i] = make_int2(0, 0);          // the mean-square displacement is measured from the initial state
-    d.msd_ref[i] = d.pos[i];
+    d.msd_ref[i] = pos_ld(d.pos + i, k);
 #pragma unroll
     for (int s = 0; s < 3; ++s) { d.vn[s * k.Vs + i] = vn_u[3 * i + s]; d.vc[s * k.Vs + i] = vc_u[3 * i + s]; }
   }
@@ -186,8 +190,6 @@ __global__ void validate_kernel(const Dev d, const Consts k) {
       }
   }
   if (i < k.V) {
-    const double2 h = d.pos[i];
-    if (!(h.x >= 0.0 && h.x < k.Lx && h.y >= 0.0 && h.y < k.Ly)) bad = true;
     for (int s = 0; s < 3 && !bad; ++s) {
       const int w = d.vn[s * k.Vs + i], c = d.vc[s * k.Vs + i], wn = d.vn[((s + 1) % 3) * k.Vs + i];
       if (w < 0 || w >= k.V || c < 0 || c >= k.N || w == i) { bad = true; break; }
@@ -207,7 +209,7 @@ __global__ void export_vertices_kernel(const Dev d, const Consts k, double* pos,
   const int v = blockIdx.x * blockDim.x + threadIdx.x;
   if (v >= k.V) return;
   const int t = d.vtag[v];
-  if (pos) { const double2 h = d.pos[v]; pos[2 * t] = h.x; pos[2 * t + 1] = h.y; }
+  if (pos) { const double2 h = pos_ld(d.pos + v, k); pos[2 * t] = h.x; pos[2 * t + 1] = h.y; }
   for (int s = 0; s < 3; ++s) {
     if (vn) vn[3 * t + s] = d.vtag[d.vn[s * k.Vs + v]];
     if (vc) vc[3 * t + s] = d.ctag[d.vc[s * k.Vs + v]];
@@ -242,8 +244,8 @@ __global__ void import_positions_kernel(const Dev d, const Consts k, const doubl
   const int v = blockIdx.x * blockDim.x + threadIdx.x;
   if (v >= k.V) return;
   const int t = d.vtag[v];
-  d.pos[v] = make_double2(pos[2 * t], pos[2 * t + 1]);
-  d.msd_ref[t] = d.pos[v];
+  pos_st(d.pos + v, make_double2(pos[2 * t], pos[2 * t + 1]), k);
+  d.msd_ref[t] = pos_ld(d.pos + v, k);
   d.img[t] = make_int2(0, 0);
 }
 
@@ -254,7 +256,7 @@ __global__ void msd_reset_kernel(const Dev d, const Consts k) {
   const int v = blockIdx.x * blockDim.x + threadIdx.x;
   if (v >= k.V) return;
   const int t = d.vtag[v];
-  const double2 h = d.pos[v];
+  const double2 h = pos_ld(d.pos + v, k);
   const int2 im = d.img[t];
   d.msd_ref[t] = make_double2(h.x + (double)im.x * k.Lx, h.y + (double)im.y * k.Ly);
 }
@@ -317,6 +319,7 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   k.v0_3 = params->v0 / 3.0; k.mu = params->mu; k.dt = params->dt;
   k.amp = sqrt(2.0 * params->Dr * params->dt);
   k.lc = params->l_c; k.lc2 = params->l_c * params->l_c;
+  k.ux = params->Lx / 4294967296.0; k.uy = params->Ly / 4294967296.0; k.iux = 4294967296.0 / params->Lx; k.iuy = 4294967296.0 / params->Ly;
   k.seed = params->seed;
   k.per_cell = 0;
   k.cap_a = 3 * N;
@@ -325,10 +328,10 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   for (int r = 0; r < 10; ++r) k.rkey[r] = philox_round_key(params->seed, r);
   char* w = s->ws;
   for (int i = 0; i < 2; ++i) {
-    s->pos[i] = (double2*)(w + L.pos[i]);
+    s->pos[i] = (pos_t*)(w + L.pos[i]);
     BufferSet& b = s->set[i];
     b.vn = (int*)(w + L.vn[i]); b.vc = (int*)(w + L.vc[i]); b.cv = (int4*)(w + L.cv[i]);
-    b.cvn = (int*)(w + L.cvn[i]); b.theta = (double*)(w + L.theta[i]); b.rec = (CellRec*)(w + L.rec[i]); b.par = (CellPar*)(w + L.par[i]);
+    b.cvn = (int*)(w + L.cvn[i]); b.theta = (double*)(w + L.theta[i]); b.rec = (rec_t*)(w + L.rec[i]); b.par = (CellPar*)(w + L.par[i]);
     b.vtag = (int*)(w + L.vtag[i]); b.ctag = (int*)(w + L.ctag[i]);
     s->sc.key[i] = (unsigned int*)(w + L.key[i]); s->sc.val[i] = (int*)(w + L.val[i]);
   }
@@ -385,7 +388,7 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
       return fail(AVM_ECUDA);                                                               \
     }                                                                                       \
   } while (0)
-  AVM_CUDA_F(cudaMemcpyAsync(s->pos[0], pos_xy, 16 * (size_t)V, kind, st));
+  AVM_CUDA_F(cudaMemcpyAsync(s->pos[1], pos_xy, 16 * (size_t)V, kind, st));    // user-layout doubles, packed by the import kernel
   AVM_CUDA_F(cudaMemcpyAsync(stage.vn, vn, 12 * (size_t)V, kind, st));
   AVM_CUDA_F(cudaMemcpyAsync(stage.vc, vc, 12 * (size_t)V, kind, st));
   AVM_CUDA_F(cudaMemcpyAsync(stage.cv, cv, 4 * (size_t)N * S, kind, st));
@@ -395,7 +398,7 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   AVM_CUDA_F(cudaMemsetAsync(s->dirty, 0, 4 * 2 * (size_t)k.nw, st));
   AVM_CUDA_F(cudaMemsetAsync(s->estamp, 0, 12 * (size_t)k.Vs, st));
   const Dev d = s->dev();
-  import_kernel<<<cdiv(V, 256), 256, 0, st>>>(d, k, stage.vn, stage.vc, (const int*)stage.cv);
+  import_kernel<<<cdiv(V, 256), 256, 0, st>>>(d, k, (const double*)s->pos[1], stage.vn, stage.vc, (const int*)stage.cv);
   validate_kernel<<<cdiv(V, 256), 256, 0, st>>>(d, k);
   s->launches += 2;
   s->launches += launch_count_short_edges(d, k, st);      // first guess of the T1 load (into ctr->n_win)
@@ -737,5 +740,7 @@ const char* avm_strerror(int code) {
 }
 
 const char* avm_last_cuda_error(void) { return g_cuda_error.c_str(); }
+
+const char* avm_precision(void) { return AVM_MIXED ? "mixed" : "f64"; }
 
 }  // extern "C"

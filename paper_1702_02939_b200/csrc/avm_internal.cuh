@@ -17,6 +17,25 @@ namespace avm {
 //   nx = cos(theta_c), ny = sin(theta_c)   (director)
 struct __align__(32) CellRec { double a, p, nx, ny; };
 
+// ---------------------------------------------------------------------------------------------
+// Storage formats.  Default build: positions double2, records 4 doubles (everything fp64).
+// -DAVM_MIXED=1 (libavm_b200_mixed.so; PAPER.md:120 shows a single-precision variant):
+// reduced-precision STORAGE, fp64 arithmetic.  Positions live on a fixed-point grid of 2^-32 box lengths
+// per axis (8 bytes instead of 16; the periodic box is the natural range of the integer), records are
+// four floats (16 bytes instead of 32).  Every kernel unpacks to double on load and packs on store,
+// so the arithmetic of the step is the same code in both builds; the accuracy contract is in avm.h.
+// ---------------------------------------------------------------------------------------------
+#ifndef AVM_MIXED
+#define AVM_MIXED 0
+#endif
+#if AVM_MIXED
+typedef uint2 pos_t;
+struct __align__(16) rec_t { float a, p, nx, ny; };
+#else
+typedef double2 pos_t;
+typedef CellRec rec_t;
+#endif
+
 // Per-cell parameters of Eq. 1 (NEXT-4): preferred area / perimeter and moduli.
 struct __align__(32) CellPar { double A0, P0, KA, KP; };
 
@@ -60,6 +79,7 @@ struct Consts {
   double v0_3, mu, dt;       // v0_3 = v0 / 3 (Eq. 4 with n = 3, R5)
   double amp;                // sqrt(2 Dr dt) (R8)
   double lc, lc2;
+  double ux, uy, iux, iuy;   // mixed build: grid unit Lx / 2^32, Ly / 2^32 and their inverses
   int flag_dirty;            // 1: the marking thread flags the vertices of a candidate's cells (two-launch schedule only)
   int clear_dirty;           // 1: the cell pass clears the bitmap the force/move launch of this step swept with
   int nw;                    // words per dirty bitmap (V/32 rounded up to a multiple of 32)
@@ -79,14 +99,14 @@ struct Consts {
 //            fully coalesced 128-bit load per plane, and cells with <= 8 vertices (96 %) never
 //            touch planes 2, 3.
 struct Dev {
-  double2* pos;       // [V] current positions
-  double2* pos_next;  // [V] written by force_move, then swapped
+  pos_t* pos;         // [V] current positions
+  pos_t* pos_next;    // [V] written by force_move, then swapped
   int* vn;            // [3*Vs] vertexNeighbors planes
   int* vc;            // [3*Vs] vertexCellNeighbors planes
   int4* cv;           // [(S/4)*N] cellVertices planes
   int* cvn;           // [N] cellVertexNum
   double* theta;      // [N]
-  CellRec* rec;       // [N]
+  rec_t* rec;         // [N]
   int* vtag;          // [V] user index of each vertex
   int* ctag;          // [N] user index of each cell
   unsigned long long* minkey;  // [N] per-cell minimum candidate key, ~0 when idle
@@ -117,6 +137,41 @@ __device__ __forceinline__ double wrap_box(double x, double L) {
   return x;
 }
 __device__ __forceinline__ unsigned int hi_word(double x) { return (unsigned int)__double2hiint(x); }
+
+// ---- packing / unpacking of the storage formats (identity in the fp64 build) ----
+#if AVM_MIXED
+__device__ __forceinline__ double2 pos_unpack(const pos_t q, const Consts& k) {
+  return make_double2(__dmul_rn((double)q.x, k.ux), __dmul_rn((double)q.y, k.uy));      // ux = Lx / 2^32
+}
+__device__ __forceinline__ pos_t pos_pack(const double2 h, const Consts& k) {
+  // h in [0, L): nearest grid point; a coordinate that rounds up to the box length wraps to 0
+  return make_uint2((unsigned int)__double2ull_rn(__dmul_rn(h.x, k.iux)), (unsigned int)__double2ull_rn(__dmul_rn(h.y, k.iuy)));
+}
+__device__ __forceinline__ CellRec rec_unpack(const float4 f) { CellRec r; r.a = f.x; r.p = f.y; r.nx = f.z; r.ny = f.w; return r; }
+#else
+__device__ __forceinline__ double2 pos_unpack(const pos_t q, const Consts&) { return q; }
+__device__ __forceinline__ pos_t pos_pack(const double2 h, const Consts&) { return h; }
+#endif
+__device__ __forceinline__ double2 pos_ld(const pos_t* p, const Consts& k) { return pos_unpack(*p, k); }
+__device__ __forceinline__ double2 pos_ldg(const pos_t* p, const Consts& k) { return pos_unpack(__ldg(p), k); }
+__device__ __forceinline__ double2 pos_ldcg(const pos_t* p, const Consts& k) { return pos_unpack(__ldcg(p), k); }
+__device__ __forceinline__ void pos_st(pos_t* p, const double2 h, const Consts& k) { *p = pos_pack(h, k); }
+// the value a stored position reads back as (the packing is not the identity in the mixed build)
+__device__ __forceinline__ double2 pos_round(const double2 h, const Consts& k) { return pos_unpack(pos_pack(h, k), k); }
+#if AVM_MIXED
+__device__ __forceinline__ CellRec rec_ld_plain(const rec_t* p) { return rec_unpack(*reinterpret_cast<const float4*>(p)); }
+__device__ __forceinline__ CellRec rec_ldcg(const rec_t* p) { return rec_unpack(__ldcg(reinterpret_cast<const float4*>(p))); }
+__device__ __forceinline__ void rec_st_ap(rec_t* p, double a, double pp) { *reinterpret_cast<float2*>(p) = make_float2((float)a, (float)pp); }
+#else
+__device__ __forceinline__ CellRec rec_ld_plain(const rec_t* p) { return *p; }
+__device__ __forceinline__ CellRec rec_ldcg(const rec_t* p) {
+  const double2* r = reinterpret_cast<const double2*>(p);
+  const double2 ap = __ldcg(r), nn = __ldcg(r + 1);
+  CellRec c; c.a = ap.x; c.p = ap.y; c.nx = nn.x; c.ny = nn.y;
+  return c;
+}
+__device__ __forceinline__ void rec_st_ap(rec_t* p, double a, double pp) { p->a = a; p->p = pp; }
+#endif
 
 // entry j of cell c's row
 __device__ __forceinline__ int& row_entry(int4* cv, int N, int c, int j) {
@@ -225,14 +280,14 @@ __device__ __forceinline__ double geom_edge(double rxp, double ryp, double rx, d
 
 // Area and perimeter of one cell from its row, one thread, plain loads (safe right after this
 // warp rewrote the row).  Used by the cold paths: T1 refresh, avm_compute_forces, energy.
-__device__ __forceinline__ void cell_area_perimeter(const double2* pos, const int4* cv, int c, int n,
+__device__ __forceinline__ void cell_area_perimeter(const pos_t* pos, const int4* cv, int c, int n,
                                                     const Consts& k, double& A, double& P) {
-  const double2 h0 = pos[row_entry(cv, k.N, c, 0)];
+  const double2 h0 = pos_ld(pos + row_entry(cv, k.N, c, 0), k);
   double rxp = 0.0, ryp = 0.0, acc = 0.0, per = 0.0;
   for (int j = 1; j <= n; ++j) {
     double rx = 0.0, ry = 0.0;
     if (j < n) {
-      const double2 hj = pos[row_entry(cv, k.N, c, j)];
+      const double2 hj = pos_ld(pos + row_entry(cv, k.N, c, j), k);
       rx = min_image(__dsub_rn(hj.x, h0.x), k.Lx, k.hLx);
       ry = min_image(__dsub_rn(hj.y, h0.y), k.Ly, k.hLy);
     }

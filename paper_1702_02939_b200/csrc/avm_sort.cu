@@ -46,7 +46,7 @@ __device__ __forceinline__ unsigned int key_of_position(double x, double y, cons
 __global__ void vertex_keys_kernel(const Dev d, const Consts k, int m, unsigned int* __restrict__ key, int* __restrict__ val) {
   const int v = blockIdx.x * blockDim.x + threadIdx.x;
   if (v >= k.V) return;
-  const double2 h = d.pos[v];
+  const double2 h = pos_ld(d.pos + v, k);
   const int t = d.vtag[v];
   key[t] = key_of_position(h.x, h.y, k, m);
   val[t] = v;
@@ -56,10 +56,10 @@ __global__ void cell_keys_kernel(const Dev d, const Consts k, int m, unsigned in
   const int c = blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= k.N) return;
   const int n = d.cvn[c];
-  const double2 h0 = d.pos[row_entry(d.cv, k.N, c, 0)];
+  const double2 h0 = pos_ld(d.pos + row_entry(d.cv, k.N, c, 0), k);
   double sx = 0.0, sy = 0.0;
   for (int j = 1; j < n; ++j) {
-    const double2 hj = d.pos[row_entry(d.cv, k.N, c, j)];
+    const double2 hj = pos_ld(d.pos + row_entry(d.cv, k.N, c, j), k);
     sx += min_image(hj.x - h0.x, k.Lx, k.hLx);
     sy += min_image(hj.y - h0.y, k.Ly, k.hLy);
   }

@@ -76,7 +76,13 @@ __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefe
 __device__ __forceinline__ int ld_stream(const int* p) { return __ldcs(p); }
 __device__ __forceinline__ int4 ld_stream(const int4* p) { return __ldcs(p); }
 __device__ __forceinline__ double ld_stream(const double* p) { return __ldcs(p); }
-// one 32-byte record with a single 256-bit load (LDG.E.256, sm_100)
+// one record with a single load: 256 bits in the fp64 build (LDG.E.256, sm_100), 128 bits (four floats) in the mixed build
+#if AVM_MIXED
+__device__ __forceinline__ CellRec ld_rec(const rec_t* p) { return rec_unpack(__ldg(reinterpret_cast<const float4*>(p))); }
+__device__ __forceinline__ void st_rec(rec_t* p, const CellRec& r) {
+  *reinterpret_cast<float4*>(p) = make_float4((float)r.a, (float)r.p, (float)r.nx, (float)r.ny);
+}
+#else
 __device__ __forceinline__ CellRec ld_rec(const CellRec* p) {
   CellRec r;
   asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(r.a), "=d"(r.p), "=d"(r.nx), "=d"(r.ny) : "l"(p));
@@ -85,6 +91,7 @@ __device__ __forceinline__ CellRec ld_rec(const CellRec* p) {
 __device__ __forceinline__ void st_rec(CellRec* p, const CellRec& r) {
   asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(r.a), "d"(r.p), "d"(r.nx), "d"(r.ny) : "memory");
 }
+#endif
 // |d| >= L/2 decided conservatively on the high word with integer ALU ops (keeps the FP64 pipe
 // for arithmetic); the exact minimum image runs only where this fires.
 __device__ __forceinline__ unsigned may_wrap(double d, unsigned hi_half) { return (hi_word(d) & 0x7fffffffu) >= hi_half; }
@@ -132,7 +139,7 @@ __device__ __forceinline__ double2 vertex_force(const double2 h, const double2 q
 struct VertexIn { double2 h; int n0, n1, n2, c0, c1, c2; };
 __device__ __forceinline__ VertexIn load_vertex(const Dev& d, const Consts& k, int v) {
   VertexIn in;
-  in.h = __ldg(d.pos + v);
+  in.h = pos_ldg(d.pos + v, k);
   in.n0 = ld_stream(d.vn + v); in.n1 = ld_stream(d.vn + k.Vs + v); in.n2 = ld_stream(d.vn + 2 * k.Vs + v);
   in.c0 = ld_stream(d.vc + v); in.c1 = ld_stream(d.vc + k.Vs + v); in.c2 = ld_stream(d.vc + 2 * k.Vs + v);
   return in;
@@ -148,6 +155,21 @@ __device__ __forceinline__ void move_vertex(const Dev& d, const Consts& k, int v
   const double vy = __fma_rn(k.mu, f.y, __dmul_rn(k.v0_3, __dadd_rn(__dadd_rn(c0.ny, c1.ny), c2.ny)));
   double x = __fma_rn(k.dt, vx, h.x), y = __fma_rn(k.dt, vy, h.y);
   // negative, >= L (conservatively) and non-finite values all have a large unsigned high word
+#if AVM_MIXED
+  int ix = 0, iy = 0;
+  if ((hi_word(x) >= hi_word(k.Lx)) | (hi_word(y) >= hi_word(k.Ly))) {
+    x = wrap_box_count(x, k.Lx, ix); y = wrap_box_count(y, k.Ly, iy);
+    if (!(isfinite(x) && isfinite(y))) atomicOr((unsigned long long*)&d.ctr->error, 1ull);
+  }
+  const pos_t pk = pos_pack(make_double2(x, y), k);
+  if (pk.x == 0u && x > k.hLx) ++ix;    // rounded up to the box length: the grid point is the origin of the next image
+  if (pk.y == 0u && y > k.hLy) ++iy;
+  d.pos_next[v] = pk;
+  if (ix | iy) {
+    int2* im = d.img + d.vtag[v];
+    int2 c = *im; c.x += ix; c.y += iy; *im = c;
+  }
+#else
   if ((hi_word(x) >= hi_word(k.Lx)) | (hi_word(y) >= hi_word(k.Ly))) {
     int ix = 0, iy = 0;
     x = wrap_box_count(x, k.Lx, ix); y = wrap_box_count(y, k.Ly, iy);
@@ -158,20 +180,19 @@ __device__ __forceinline__ void move_vertex(const Dev& d, const Consts& k, int v
     }
   }
   d.pos_next[v] = make_double2(x, y);
+#endif
 }
 
 // the same vertex update with every input read from L2 (after another warp of this launch
 // rewrote the neighbourhood: L1 may hold stale lines)
 __device__ __noinline__ void move_vertex_coherent(const Dev& d, const Consts& k, int v) {
-  const double2 h = __ldcg(d.pos + v);
+  const double2 h = pos_ldcg(d.pos + v, k);
   double2 q[3];
   CellRec c[3];
 #pragma unroll
   for (int s = 0; s < 3; ++s) {
-    q[s] = __ldcg(d.pos + __ldcg(d.vn + s * k.Vs + v));
-    const double2* r = reinterpret_cast<const double2*>(d.rec + __ldcg(d.vc + s * k.Vs + v));
-    const double2 ap = __ldcg(r), nn = __ldcg(r + 1);
-    c[s].a = ap.x; c[s].p = ap.y; c[s].nx = nn.x; c[s].ny = nn.y;
+    q[s] = pos_ldcg(d.pos + __ldcg(d.vn + s * k.Vs + v), k);
+    c[s] = rec_ldcg(d.rec + __ldcg(d.vc + s * k.Vs + v));
   }
   move_vertex(d, k, v, h, q[0], q[1], q[2], c[0], c[1], c[2]);
 }
@@ -212,7 +233,7 @@ __device__ __forceinline__ void sweep(const Dev& d, const Consts& k, const unsig
     const bool skip = kSkipDirty && ((dw >> (v & 31)) & 1u);
     const int vnext = v + step_v;
     if (!skip) {
-      const double2 q0 = __ldg(d.pos + in.n0), q1 = __ldg(d.pos + in.n1), q2 = __ldg(d.pos + in.n2);
+      const double2 q0 = pos_ldg(d.pos + in.n0, k), q1 = pos_ldg(d.pos + in.n1, k), q2 = pos_ldg(d.pos + in.n2, k);
       const CellRec c0 = ld_rec(d.rec + in.c0), c1 = ld_rec(d.rec + in.c1), c2 = ld_rec(d.rec + in.c2);
       const double2 h = in.h;
       if (AVM_FM_REGPF && vnext < k.V) { in = load_vertex(d, k, vnext); if (kSkipDirty) dw = __ldg(dirty + (vnext >> 5)); }
@@ -460,7 +481,7 @@ __device__ __noinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va,
   // The marking thread delays the end of the cell pass when it sits in the last wave, so its
   // loads are issued in two batches of independent loads instead of a chain of five.
   // ---- batch 1: everything known from (va, vb) ----
-  const double2 ha = d.pos[va], hb = d.pos[vb];
+  const double2 ha = pos_ld(d.pos + va, k), hb = pos_ld(d.pos + vb, k);
   const unsigned int ta = (unsigned int)d.vtag[va], tb = (unsigned int)d.vtag[vb];
   int na[3], nb[3], ca[3], cb[3];
 #pragma unroll
@@ -589,7 +610,7 @@ cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts
   if (kStep && k.clear_dirty && gid < k.nw) d.dirty[(size_t)(parity ^ 1u) * (size_t)k.nw + gid] = 0u;
   const bool valid = gid < k.N;
   const int c = valid ? k.N - 1 - gid : 0;
-  const double2* __restrict__ pos = d.pos;
+  const pos_t* __restrict__ pos = d.pos;
   const int n = valid ? ld_stream(d.cvn + c) : 0;
   const int4 qa = ld_stream(d.cv + c), qb = ld_stream(d.cv + k.N + c);
   const int e[8] = {qa.x, qa.y, qa.z, qa.w, qb.x, qb.y, qb.z, qb.w};
@@ -597,7 +618,7 @@ cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts
   const unsigned int tag = (unsigned int)ld_stream(d.ctag + c);
   double2 h[8];
 #pragma unroll
-  for (int j = 0; j < 8; ++j) h[j] = __ldg(pos + e[j]);   // padding entries repeat entry 0: r = 0, no predicate
+  for (int j = 0; j < 8; ++j) h[j] = pos_ldg(pos + e[j], k);   // padding entries repeat entry 0: r = 0, no predicate
   // ---- director (independent of the gathers above) ----
   if (kStep) {
     th += k.amp * director_noise(k, step, (unsigned long long)tag);
@@ -639,7 +660,7 @@ cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts
 #pragma unroll
       for (int i = 0; i < 4; ++i) {
         hh[i] = h[0];
-        if (j0 + i < n) hh[i] = __ldg(pos + ee[i]);
+        if (j0 + i < n) hh[i] = pos_ldg(pos + ee[i], k);
       }
 #pragma unroll
       for (int i = 0; i < 4; ++i) {
@@ -673,12 +694,12 @@ __global__ void detect_mark_kernel(const __grid_constant__ Dev d, const __grid_c
                                    const bool count_stats) {
   const int v = blockIdx.x * blockDim.x + threadIdx.x;
   if (v >= k.V) return;
-  const double2 h = d.pos[v];
+  const double2 h = pos_ld(d.pos + v, k);
   for (int s = 0; s < 3; ++s) {
     const int w = d.vn[s * k.Vs + v];
     if (v < w) {
       // cheap pre-test; t1_mark_edge repeats the canonical one
-      const double2 q = d.pos[w];
+      const double2 q = pos_ld(d.pos + w, k);
       const double dx = min_image(q.x - h.x, k.Lx, k.hLx), dy = min_image(q.y - h.y, k.Ly, k.hLy);
       if (dx * dx + dy * dy < k.lc2) t1_mark_edge(d, k, v, w, parity, count_stats ? kMarkFirstPass : kMarkSilent);
     }
@@ -725,7 +746,7 @@ t1_local_detect_kernel(const __grid_constant__ Dev d, const __grid_constant__ Co
       const int nrow = d.cvn[quad[t]];
       if (lane >= nrow) continue;
       const int u = row_entry(d.cv, k.N, quad[t], lane);
-      const double2 hu = d.pos[u];
+      const double2 hu = pos_ld(d.pos + u, k);
 #pragma unroll 1
       for (int sl = 0; sl < 3; ++sl) {
         const int wv = d.vn[sl * k.Vs + u];
@@ -736,7 +757,7 @@ t1_local_detect_kernel(const __grid_constant__ Dev d, const __grid_constant__ Co
           oslot = d.vn[wv] == u ? 0 : d.vn[k.Vs + wv] == u ? 1 : 2;
         }
         if (atomicExch(&d.estamp[(size_t)oslot * k.Vs + owner], stamp) == stamp) continue;   // tested in this pass already
-        const double2 hw = d.pos[wv];
+        const double2 hw = pos_ld(d.pos + wv, k);
         const double dx = min_image(hw.x - hu.x, k.Lx, k.hLx), dy = min_image(hw.y - hu.y, k.Ly, k.hLy);
         if (dx * dx + dy * dy < k.lc2) t1_mark_edge(d, k, owner, other, list_new, kMarkRepeatedPass);
       }
@@ -789,7 +810,7 @@ __device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Const
   const int cell = t == 0 ? cL : t == 1 ? cR : t == 2 ? cE1 : cE2;     // 0 for idle groups: a valid index
   const unsigned long long mk = d.minkey[cell];
   const int nrow = d.cvn[cell];
-  const double2 h1 = d.pos[v1], h2 = d.pos[v2];
+  const double2 h1 = pos_ld(d.pos + v1, k), h2 = pos_ld(d.pos + v2, k);
   int r[kR];
 #pragma unroll
   for (int q = 0; q < kR / 4; ++q) {
@@ -813,8 +834,9 @@ __device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Const
   double px = 0.0, py = 1.0;
   if (l > 0.0) { px = -dy / l; py = dx / l; }
   const double half = 0.75 * k.lc;
-  const double2 n2 = make_double2(wrap_box(mx + half * px, k.Lx), wrap_box(my + half * py, k.Ly));
-  const double2 n1 = make_double2(wrap_box(mx - half * px, k.Lx), wrap_box(my - half * py, k.Ly));
+  // (pos_round: the value the stored position reads back as; the identity in the fp64 build)
+  const double2 n2 = pos_round(make_double2(wrap_box(mx + half * px, k.Lx), wrap_box(my + half * py, k.Ly)), k);
+  const double2 n1 = pos_round(make_double2(wrap_box(mx - half * px, k.Lx), wrap_box(my - half * py, k.Ly)), k);
   // ---- lists: u = ([w, x, y]; [C0, C1, C2]) cyclic from the partner slot
   //          -> ([w, y, z]; [C1, C2, C']), z = partner's old x, C' = partner's old C1 (R12);
   // outer vertices: x1 was joined to v1 and is now joined to v2 (same slot), x2 likewise.
@@ -831,12 +853,12 @@ __device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Const
   }
   if (t == 0) {
     const int a1 = (k1 + 1) % 3, b1 = (k1 + 2) % 3;
-    d.pos[v1] = n1;
+    pos_st(d.pos + v1, n1, k);
     d.vn[a1 * k.Vs + v1] = y1; d.vn[b1 * k.Vs + v1] = x2;
     d.vc[k1 * k.Vs + v1] = cE1; d.vc[a1 * k.Vs + v1] = cR; d.vc[b1 * k.Vs + v1] = cE2;
   } else if (t == 1) {
     const int a2 = (k2 + 1) % 3, b2 = (k2 + 2) % 3;
-    d.pos[v2] = n2;
+    pos_st(d.pos + v2, n2, k);
     d.vn[a2 * k.Vs + v2] = y2; d.vn[b2 * k.Vs + v2] = x1;
     d.vc[k2 * k.Vs + v2] = cE2; d.vc[a2 * k.Vs + v2] = cL; d.vc[b2 * k.Vs + v2] = cE1;
   } else if (t == 2) {
@@ -878,7 +900,7 @@ __device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Const
   // per-step pass (geom_edge), so that a resumed run reproduces these records bit for bit.  v1 and
   // v2 take their new positions from registers; positions are fetched eight at a time (entries
   // beyond the row repeat entry 0, whose position is substituted without a load).
-  const double2 h0 = e0 == v1 ? n1 : e0 == v2 ? n2 : d.pos[e0];
+  const double2 h0 = e0 == v1 ? n1 : e0 == v2 ? n2 : pos_ld(d.pos + e0, k);
   double rxp = 0.0, ryp = 0.0, acc = 0.0, per = 0.0;
 #pragma unroll
   for (int j0 = 1; j0 < kR; j0 += 8) {
@@ -889,7 +911,7 @@ __device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Const
         hh[u] = h0;
         if (j0 + u < kR) {
           const int e = r[j0 + u < kR ? j0 + u : 0];
-          if (j0 + u < nnew) hh[u] = e == v1 ? n1 : e == v2 ? n2 : d.pos[e];
+          if (j0 + u < nnew) hh[u] = e == v1 ? n1 : e == v2 ? n2 : pos_ld(d.pos + e, k);
         }
       }
 #pragma unroll
@@ -905,8 +927,10 @@ __device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Const
   }
   geom_edge(rxp, ryp, 0.0, 0.0, acc, per);      // the closing edge back to entry 0
   AVM_TR_W0(4, (int)acc);
-  if (k.per_cell) rec_from_geometry(d.par[cell], __dmul_rn(0.5, acc), per, d.rec[cell].a, d.rec[cell].p);
-  else { d.rec[cell].a = k.KA2 * (__dmul_rn(0.5, acc) - k.A0); d.rec[cell].p = k.KP2 * (per - k.P0); }
+  double ra, rp;
+  if (k.per_cell) rec_from_geometry(d.par[cell], __dmul_rn(0.5, acc), per, ra, rp);
+  else { ra = k.KA2 * (__dmul_rn(0.5, acc) - k.A0); rp = k.KP2 * (per - k.P0); }
+  rec_st_ap(d.rec + cell, ra, rp);
   AVM_TR_W0(5, 0);
 #ifdef AVM_TRACE
   if (trq && blockIdx.x == 0 && threadIdx.x < 32) d.ctr->tr2[48 + threadIdx.x] = gtime() - tqe;
@@ -994,12 +1018,12 @@ __global__ void geometry_kernel(const Dev d, const Consts k, double2* __restrict
 __global__ void forces_kernel(const Dev d, const Consts k, const double2* __restrict__ ap, double* __restrict__ force_user) {
   const int v = blockIdx.x * blockDim.x + threadIdx.x;
   if (v >= k.V) return;
-  const double2 h = d.pos[v];
+  const double2 h = pos_ld(d.pos + v, k);
   CellRec c[3];
   double2 q[3];
 #pragma unroll
   for (int s = 0; s < 3; ++s) {
-    q[s] = d.pos[d.vn[s * k.Vs + v]];
+    q[s] = pos_ld(d.pos + d.vn[s * k.Vs + v], k);
     const int cell = d.vc[s * k.Vs + v];
     const double2 a = ap[cell];
     if (k.per_cell) rec_from_geometry(d.par[cell], a.x, a.y, c[s].a, c[s].p);
@@ -1049,7 +1073,7 @@ observables_partial_kernel(const Dev d, const Consts k, double* __restrict__ par
   // mean-square displacement: unwrapped position = wrapped position + image count x box length
   for (int v = blockIdx.x * 256 + threadIdx.x; v < k.V; v += gridDim.x * 256) {
     const int t = d.vtag[v];
-    const double2 h = d.pos[v], r0 = d.msd_ref[t];
+    const double2 h = pos_ld(d.pos + v, k), r0 = d.msd_ref[t];
     const int2 im = d.img[t];
     const double dx = (h.x + (double)im.x * k.Lx) - r0.x, dy = (h.y + (double)im.y * k.Ly) - r0.y;
     x[8] += dx * dx + dy * dy;
@@ -1137,12 +1161,12 @@ int launch_step(const Dev& d, const Consts& k, unsigned long long step, cudaStre
 __global__ void count_short_edges_kernel(const Dev d, const Consts k) {
   const int v = blockIdx.x * blockDim.x + threadIdx.x;
   if (v >= k.V) return;
-  const double2 h = d.pos[v];
+  const double2 h = pos_ld(d.pos + v, k);
   int n = 0;
   for (int s = 0; s < 3; ++s) {
     const int w = d.vn[s * k.Vs + v];
     if (v < w) {
-      const double2 q = d.pos[w];
+      const double2 q = pos_ld(d.pos + w, k);
       const double dx = min_image(q.x - h.x, k.Lx, k.hLx), dy = min_image(q.y - h.y, k.Ly, k.hLy);
       n += dx * dx + dy * dy < k.lc2;
     }

@@ -83,6 +83,15 @@ def test_hilbert_index_is_a_hilbert_curve(binding, m):
 
 def test_missing_library_fails_loudly(binding, tmp_path, monkeypatch):
     import importlib
-    monkeypatch.setattr(binding, "LIB_PATH", str(tmp_path / "nope.so"))
     with pytest.raises(binding.AvmError):
-        binding._load()
+        binding._load(str(tmp_path / "nope.so"))
+
+
+def test_mixed_precision_library_has_the_same_abi(binding):
+    """libavm_b200_mixed.so (NEXT-3): same sources, same exported symbols, says what it is"""
+    mixed = binding.library("mixed")
+    for name in binding.ABI_SYMBOLS:
+        assert hasattr(mixed, name), f"{name} not exported by the mixed library"
+    assert mixed.avm_precision() == b"mixed" and binding.lib.avm_precision() == b"f64"
+    good = binding.make_params(64, 16, Lx=8.0, Ly=8.0)
+    assert mixed.avm_workspace_bytes(ctypes.byref(good)) == binding.lib.avm_workspace_bytes(ctypes.byref(good))
