@@ -208,7 +208,7 @@ def main():
                     help="steps of the per-kernel event pass (default: the timed region itself, at most 200 steps)")
     ap.add_argument("--t1-passes", type=int, default=1,
                     help="T1 passes per step: 1 = north_star's rule (default, the headline), P > 1 = repeat until none (NEXT-1)")
-    ap.add_argument("--schedule", default="auto", choices=["auto", "fused", "unfused"])
+    ap.add_argument("--schedule", default="auto", choices=["auto", "fused", "unfused", "persistent"])
     ap.add_argument("--precision", default="f64", choices=["f64", "mixed"],
                     help="f64 = the default library and the headline; mixed = libavm_b200_mixed.so (reduced-precision storage, NEXT-3)")
     args = ap.parse_args()

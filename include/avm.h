@@ -63,11 +63,15 @@ typedef struct avm_params {
 
 enum {
   AVM_FLAG_SORT_AT_CREATE = 1, /* Hilbert-order cells and vertices once inside avm_create       */
-  /* Kernel schedule of a step.  Default: chosen from the system size.  FUSED: two launches per
-   * step, the T1 flips of a step run inside the next force/move launch.  UNFUSED: three launches,
-   * a stand-alone T1 kernel.  Both give the same bits (tests); giving both flags is an error. */
+  /* Kernel schedule.  Default: chosen from the system size and, per step, from the T1 load.
+   * FUSED: two launches per step, the T1 flips of a step run inside the next force/move launch.
+   * UNFUSED: three launches per step, a stand-alone T1 kernel.  PERSISTENT: one cooperative launch
+   * per avm_step call (per stretch between re-sorts) advances all its steps, with grid-wide barriers
+   * between the stages (launch-free stepping; the default for systems of at most 512 vertices, which
+   * run as one CTA).  All schedules give the same bits (tests); at most one flag may be given. */
   AVM_FLAG_SCHEDULE_FUSED = 4,
   AVM_FLAG_SCHEDULE_UNFUSED = 8,
+  AVM_FLAG_SCHEDULE_PERSISTENT = 16,
   /* bits 8..15: maximum number of T1 passes per step.  0 or 1 = one pass per step (the rule of
    * BASELINE.json's north_star, the default and the timed path).  P > 1 = the paper's own rule
    * (the T1 kernel is "called repeatedly until no changes"): after the first pass

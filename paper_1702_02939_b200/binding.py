@@ -31,6 +31,7 @@ ABI_SYMBOLS = [
 AVM_FLAG_SORT_AT_CREATE = 1
 AVM_FLAG_SCHEDULE_FUSED = 4
 AVM_FLAG_SCHEDULE_UNFUSED = 8
+AVM_FLAG_SCHEDULE_PERSISTENT = 16
 AVM_FLAG_T1_PASSES_SHIFT = 8
 
 
@@ -140,7 +141,8 @@ def make_params(N: int, S: int, *, Lx, Ly, KA=1.0, KP=1.0, A0=1.0, P0=3.8, v0=0.
                 schedule="auto", **_ignored) -> AvmParams:
     if sort_at_create:
         flags |= AVM_FLAG_SORT_AT_CREATE
-    flags |= {"auto": 0, "fused": AVM_FLAG_SCHEDULE_FUSED, "unfused": AVM_FLAG_SCHEDULE_UNFUSED}[schedule]
+    flags |= {"auto": 0, "fused": AVM_FLAG_SCHEDULE_FUSED, "unfused": AVM_FLAG_SCHEDULE_UNFUSED,
+              "persistent": AVM_FLAG_SCHEDULE_PERSISTENT}[schedule]
     if t1_max_passes > 1:
         flags |= (min(int(t1_max_passes), 255) << AVM_FLAG_T1_PASSES_SHIFT)
     return AvmParams(N, 2 * N, S, sort_every, Lx, Ly, KA, KP, A0, P0, v0, Dr, mu, dt, l_c, seed, step0, device, flags)

@@ -62,6 +62,8 @@ struct Counters {
   unsigned int pad1[31];
   unsigned int flip_done; // candidates decided so far
   unsigned int pad2[31];
+  unsigned int bar;       // arrival counter of the persistent kernel's grid barrier (zeroed by the host before each launch)
+  unsigned int pad3[31];
   long long t1_short, t1_candidates, t1_flips, t1_blocked, overflow_rejects, error;
   double obs[16];  // observables of the latest avm_energy / avm_observe call (slots: avm_step.cu)
   // phase trace of the fused force/move launch (variant builds with -DAVM_TRACE only): tr = this launch's
@@ -315,6 +317,8 @@ int force_move_grid(int V);
 int launch_step(const Dev& d, const Consts& k, unsigned long long step, cudaStream_t s, cudaEvent_t* ev, bool consume_pending,
                 bool leave_pending);
 int launch_count_short_edges(const Dev& d, const Consts& k, cudaStream_t s);
+int persistent_grid(int V, bool per_cell);
+int launch_persistent_steps(const Dev& d, const Consts& k, unsigned long long step0, int n_steps, int grid, cudaStream_t s);
 int launch_refresh_cells(const Dev& d, const Consts& k, cudaStream_t s);
 int launch_t1_reset(const Dev& d, const Consts& k, cudaStream_t s);
 int launch_t1_pass_only(const Dev& d, const Consts& k, cudaStream_t s);

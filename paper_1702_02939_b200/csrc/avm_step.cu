@@ -22,9 +22,11 @@
 // computed from the geometry of the current topology exactly as in the paper's cycle.
 #include <cstdio>
 #include <cstdlib>
+#include <cooperative_groups.h>
 #include "avm_internal.cuh"
 
 namespace avm {
+namespace cg = cooperative_groups;
 
 static constexpr int kVertexBlock = 256;
 #ifndef AVM_CELL_BLOCK
@@ -590,13 +592,14 @@ __device__ __noinline__ void t1_report_cell(const Dev& d, const Consts& k, int c
 // Cells are walked in DESCENDING index order while force_move walks vertices in ascending order,
 // so each pass starts on the lines the previous pass touched last (L2 recency).
 // ---------------------------------------------------------------------------------------------
-template <bool kStep, bool kPerCell>
-__global__ void __launch_bounds__(kCellBlock, AVM_CU_MINB)
-cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, const unsigned long long step,
-                   const unsigned parity) {
-  pdl_launch_dependents();
-  pdl_wait();
-  const int gid = blockIdx.x * kCellBlock + threadIdx.x;
+// kCoh: every load of data another CTA may have written earlier in the same launch goes through
+// the coherent path (the persistent multi-step kernel); false = the per-step kernel, where the
+// streams are read with cache hints and the gathers through the non-coherent path.
+template <bool kCoh, typename T> __device__ __forceinline__ T cu_stream(const T* p) { return kCoh ? __ldcg(p) : ld_stream(p); }
+template <bool kCoh> __device__ __forceinline__ double2 cu_pos(const pos_t* p, const Consts& k) { return kCoh ? pos_ldcg(p, k) : pos_ldg(p, k); }
+template <bool kStep, bool kPerCell, bool kCoh>
+__device__ __forceinline__ void cell_update_body(const Dev& d, const Consts& k, const unsigned long long step, const unsigned parity,
+                                                 const int gid) {
   if (kStep && gid == 0) { d.ctr->flip_done = 0; d.ctr->next_cand = 0; }   // the previous list is long done
 #ifdef AVM_TRACE
   if (kStep && gid == 0) {
@@ -611,14 +614,14 @@ cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts
   const bool valid = gid < k.N;
   const int c = valid ? k.N - 1 - gid : 0;
   const pos_t* __restrict__ pos = d.pos;
-  const int n = valid ? ld_stream(d.cvn + c) : 0;
-  const int4 qa = ld_stream(d.cv + c), qb = ld_stream(d.cv + k.N + c);
+  const int n = valid ? cu_stream<kCoh>(d.cvn + c) : 0;
+  const int4 qa = cu_stream<kCoh>(d.cv + c), qb = cu_stream<kCoh>(d.cv + k.N + c);
   const int e[8] = {qa.x, qa.y, qa.z, qa.w, qb.x, qb.y, qb.z, qb.w};
-  double th = ld_stream(d.theta + c);
-  const unsigned int tag = (unsigned int)ld_stream(d.ctag + c);
+  double th = cu_stream<kCoh>(d.theta + c);
+  const unsigned int tag = (unsigned int)cu_stream<kCoh>(d.ctag + c);
   double2 h[8];
 #pragma unroll
-  for (int j = 0; j < 8; ++j) h[j] = pos_ldg(pos + e[j], k);   // padding entries repeat entry 0: r = 0, no predicate
+  for (int j = 0; j < 8; ++j) h[j] = cu_pos<kCoh>(pos + e[j], k);   // padding entries repeat entry 0: r = 0, no predicate
   // ---- director (independent of the gathers above) ----
   if (kStep) {
     th += k.amp * director_noise(k, step, (unsigned long long)tag);
@@ -654,13 +657,13 @@ cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts
   if (n > 8) {
     for (int q = 2; 4 * q < n; ++q) {
       const int j0 = 4 * q;
-      const int4 qq = d.cv[(size_t)q * k.N + c];
+      const int4 qq = kCoh ? __ldcg(d.cv + (size_t)q * k.N + c) : d.cv[(size_t)q * k.N + c];
       const int ee[4] = {qq.x, qq.y, qq.z, qq.w};
       double2 hh[4];
 #pragma unroll
       for (int i = 0; i < 4; ++i) {
         hh[i] = h[0];
-        if (j0 + i < n) hh[i] = pos_ldg(pos + ee[i], k);
+        if (j0 + i < n) hh[i] = cu_pos<kCoh>(pos + ee[i], k);
       }
 #pragma unroll
       for (int i = 0; i < 4; ++i) {
@@ -680,12 +683,20 @@ cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts
   }
   if (!valid) return;
   CellRec r;
-  if (kPerCell) rec_from_geometry(d.par[c], __dmul_rn(0.5, acc), per, r.a, r.p);   // Eq. 1 per cell (NEXT-4)
+  if (kPerCell) rec_from_geometry(d.par[c], __dmul_rn(0.5, acc), per, r.a, r.p);   // Eq. 1 per cell (NEXT-4); written by no kernel
   else { r.a = k.KA2 * (__dmul_rn(0.5, acc) - k.A0); r.p = k.KP2 * (per - k.P0); }   // Eq. A1
   r.nx = cs; r.ny = sn;
   st_rec(d.rec + c, r);
   smask &= n >= 32 ? ~0u : (1u << n) - 1u;     // edges beyond the closing one are padding
   if (kStep && smask) t1_report_cell(d, k, c, n, smask, parity);
+}
+template <bool kStep, bool kPerCell>
+__global__ void __launch_bounds__(kCellBlock, AVM_CU_MINB)
+cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, const unsigned long long step,
+                   const unsigned parity) {
+  pdl_launch_dependents();
+  pdl_wait();
+  cell_update_body<kStep, kPerCell, false>(d, k, step, parity, blockIdx.x * kCellBlock + threadIdx.x);
 }
 
 // Detection alone (test hooks avm_t1_pass / avm_debug_t1): thread per vertex, edge owned by the
@@ -964,6 +975,77 @@ t1_flip_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, 
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Launch-free stepping ("entirely on the GPU"): ONE cooperative
+// launch advances n_steps timesteps.  The three stages of a step (rows a2+a3; a4+a1+a5+a6; a6+a7) are
+// the same device functions as in the per-step kernels, separated by grid-wide barriers instead of
+// kernel boundaries; loads of data written earlier in the launch take the coherent path.  Used
+// for systems that fit in L2 and are bound by launch latency, not bandwidth (configs 0-2); the
+// results are bit-identical to the per-step schedules.  A grid of one CTA needs no barrier but
+// __syncthreads (grid.sync() of a one-CTA cooperative grid is just that).
+// ---------------------------------------------------------------------------------------------
+// Grid-wide barrier of the cooperative launch (every CTA is resident).  Monotonic arrival counter, zeroed by
+// the host before the launch; `epoch` counts the barriers passed.  Release: fence, then arrive; acquire: observe
+// the full count, then fence.  One CTA: __syncthreads is all it takes.
+struct GridBarrier {
+  unsigned int* bar;
+  unsigned int epoch;
+  __device__ __forceinline__ void sync() {
+    ++epoch;
+    if (gridDim.x == 1) { __syncthreads(); return; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      __threadfence();
+      atomicAdd(bar, 1u);
+      const unsigned target = epoch * gridDim.x;
+      while (ld_volatile(bar) < target) { }
+      __threadfence();
+    }
+    __syncthreads();
+  }
+};
+template <bool kPerCell>
+__global__ void __launch_bounds__(kVertexBlock)
+persistent_steps_kernel(Dev d, const __grid_constant__ Consts k, const unsigned long long step0, const int n_steps) {
+  GridBarrier grid = {&d.ctr->bar, 0u};
+  const int tid = blockIdx.x * kVertexBlock + threadIdx.x, stride = gridDim.x * kVertexBlock;
+  const int lane = threadIdx.x & 31;
+  const unsigned gwarp = (unsigned)tid >> 5, nwarps = (unsigned)stride >> 5;
+  const int n_round = (k.N + 31) & ~31;                 // the cell body wants whole warps (it uses no warp collectives, but stays uniform)
+  for (int it = 0; it < n_steps; ++it) {
+    const unsigned long long step = step0 + (unsigned long long)it;
+    const unsigned parity = (unsigned)(step & 1ull);
+    // ---- rows a2 + a3 (and the release of the previous step's minimum keys, row a6)
+    const unsigned prev = min(__ldcg(&d.ctr->n_cand[parity ^ 1u]), (unsigned)k.cap_a);
+    if (tid == 0) d.ctr->n_cand[parity] = 0;           // this step's list; its previous contents were last read two stages ago
+    for (unsigned i = tid; i < prev; i += stride) {
+      const int4 q = __ldcg(reinterpret_cast<const int4*>(d.cand + i) + 1);
+      d.minkey[q.x] = ~0ull; d.minkey[q.y] = ~0ull; d.minkey[q.z] = ~0ull; d.minkey[q.w] = ~0ull;
+    }
+    for (int v = tid; v < k.V; v += stride) move_vertex_coherent(d, k, v);
+    grid.sync();
+    { pos_t* t = d.pos; d.pos = d.pos_next; d.pos_next = t; }
+    // ---- rows a4 + a1 + a5 + a6 (marking half)
+    for (int gid = tid; gid < n_round; gid += stride) cell_update_body<true, kPerCell, true>(d, k, step, parity, gid);
+    grid.sync();
+    // ---- rows a6 (deciding half) + a7
+    const unsigned n_cand = min(__ldcg(&d.ctr->n_cand[parity]), (unsigned)k.cap_a);
+    if (n_cand) {                                        // uniform over the grid: read after the barrier
+      if (tid == 0) atomicAdd((unsigned long long*)&d.ctr->t1_candidates, (unsigned long long)n_cand);
+      unsigned flips = 0, seen = 0;
+      for (unsigned i = gwarp * 8u; i < n_cand; i += nwarps * 8u) {
+        flips += t1_flip_quads(d, k, d.cand, i, n_cand, lane);
+        seen += min(8u, n_cand - i);
+      }
+      if (lane == 0) {
+        if (flips) atomicAdd((unsigned long long*)&d.ctr->t1_flips, (unsigned long long)flips);
+        if (seen - flips) atomicAdd((unsigned long long*)&d.ctr->t1_blocked, (unsigned long long)(seen - flips));
+      }
+      grid.sync();
+    }
+  }
+}
+
 // Clears the minimum keys of both candidate lists and empties them (before a re-sort, around the
 // test hooks).  Inside avm_step this work rides in force_move's prologue instead.
 __global__ void __launch_bounds__(kT1Block)
@@ -1175,6 +1257,36 @@ __global__ void count_short_edges_kernel(const Dev d, const Consts k) {
 }
 int launch_count_short_edges(const Dev& d, const Consts& k, cudaStream_t s) {
   count_short_edges_kernel<<<cdiv(k.V, 256), 256, 0, s>>>(d, k);
+  return 1;
+}
+
+// Largest cooperative grid of the persistent kernel on the current device, capped by the work (0 = unavailable).
+int persistent_grid(int V, bool per_cell) {
+  int dev = 0, sms = 0, coop = 0, per_sm = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return 0;
+  cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (!coop || sms <= 0) return 0;
+  if (per_cell) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, persistent_steps_kernel<true>, kVertexBlock, 0);
+  else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, persistent_steps_kernel<false>, kVertexBlock, 0);
+  if (per_sm < 1) return 0;
+  const int want = V <= 512 ? 1 : cdiv(V, kVertexBlock), cap = sms * per_sm;     // tiny systems: one CTA, barriers are __syncthreads
+  return want < cap ? want : cap;
+}
+
+// n_steps timesteps in one cooperative launch; returns the number of launches (1), or -1 if the launch was refused.
+int launch_persistent_steps(const Dev& d, const Consts& k, unsigned long long step0, int n_steps, int grid, cudaStream_t s) {
+  Dev dd = d;
+  Consts kk = k;
+  kk.flag_dirty = 0; kk.clear_dirty = 0;
+  int ns = n_steps;
+  void* args[] = {(void*)&dd, (void*)&kk, (void*)&step0, (void*)&ns};
+  const void* fn = k.per_cell ? (const void*)persistent_steps_kernel<true> : (const void*)persistent_steps_kernel<false>;
+  cudaMemsetAsync(&d.ctr->bar, 0, sizeof(unsigned int), s);
+  if (cudaLaunchCooperativeKernel(fn, dim3((unsigned)grid), dim3(kVertexBlock), args, 0, s) != cudaSuccess) {
+    cudaGetLastError();
+    return -1;
+  }
   return 1;
 }
 

@@ -757,3 +757,31 @@ def test_mean_square_displacement_matches_the_oracle(B, sched):
     g = B.from_tiling(hx, KA=0.0, KP=0.0, v0=0.8, Dr=0.0, dt=0.01, l_c=0.0, schedule=sched)
     g.step(1500)
     assert abs(g.observe()["msd"] - 144.0) < 1e-9 * 144.0
+
+
+@pytest.mark.parametrize("k,steps,sort_every", [(0, 150, 0), (1, 60, 7), (2, 20, 6)])
+def test_persistent_schedule_equals_the_launched_schedules(B, k, steps, sort_every):
+    """Launch-free stepping (one cooperative launch per call / per stretch between re-sorts, grid-wide
+    barriers between the stages) against one launch per kernel, bit for bit and for any chunking;
+    configs[0] runs as a single CTA, configs[2] with more work than resident threads."""
+    t = tiling(k)
+    p = dict(w.config_params(k), sort_every=sort_every)
+    keys = ("pos", "theta", "cell_vertices", "vertex_neighbors", "vertex_cell_neighbors", "cell_vertex_num")
+    a = B.from_tiling(t, schedule="persistent", **p)
+    a.step(steps)
+    sa = to_np(a.get_state())
+    b = B.from_tiling(t, schedule="persistent", **p)
+    for n in (1, 2, steps - 3):
+        b.step(n)
+    sb = to_np(b.get_state())
+    c = B.from_tiling(t, schedule="unfused", **p)
+    c.step(steps)
+    sc = to_np(c.get_state())
+    assert sa["stats"]["kernel_launches"] < sc["stats"]["kernel_launches"] - 2 * steps     # re-sorts are launched in both
+    for other in (sb, sc):
+        for key in keys:
+            assert np.array_equal(sa[key], other[key]), key
+        for key in ("t1_short", "t1_candidates", "t1_flips", "t1_blocked", "overflow_rejects", "error", "n_sorts"):
+            assert sa["stats"][key] == other["stats"][key], key
+    assert sa["stats"]["t1_flips"] > 0
+    assert abs(a.observe()["msd"] - c.observe()["msd"]) == 0.0
