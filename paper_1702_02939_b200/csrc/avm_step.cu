@@ -23,6 +23,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cooperative_groups.h>
+#include <utility>
 #include "avm_internal.cuh"
 
 namespace avm {
@@ -787,6 +788,29 @@ t1_local_detect_kernel(const __grid_constant__ Dev d, const __grid_constant__ Co
 // ---------------------------------------------------------------------------------------------
 // kR = number of row entries held per lane: 16 (rows live in registers, every index is static and
 // all loads of a phase are in flight together) for S <= 16, 32 (a local array) for larger strides.
+template <int kR> using RowIdx = std::make_integer_sequence<int, kR>;
+// position of `mark` among the first n entries (rows hold distinct vertices; 0 if absent)
+template <int kR, int... J>
+__device__ __forceinline__ int row_find(const int (&r)[kR], const int n, const int mark, std::integer_sequence<int, J...>) {
+  int p = 0;
+  ((p = (J < n && r[J] == mark) ? J : p), ...);
+  return p;
+}
+// w = r without entry p (later entries shift down)
+template <int kR, int... J>
+__device__ __forceinline__ void row_delete(const int (&r)[kR], int (&w)[kR], const int p, std::integer_sequence<int, J...>) {
+  ((w[J] = J < p ? r[J] : r[J + 1 < kR ? J + 1 : kR - 1]), ...);
+}
+// w = r with `ins` inserted immediately after entry p (later entries shift up)
+template <int kR, int... J>
+__device__ __forceinline__ void row_insert(const int (&r)[kR], int (&w)[kR], const int p, const int ins, std::integer_sequence<int, J...>) {
+  ((w[J] = J <= p ? r[J] : J == p + 1 ? ins : r[J > 0 ? J - 1 : 0]), ...);
+}
+// r = w with the entries from n on replaced by entry 0
+template <int kR, int... J>
+__device__ __forceinline__ void row_pad(const int (&w)[kR], int (&r)[kR], const int n, std::integer_sequence<int, J...>) {
+  ((r[J] = J < n ? w[J] : w[0]), ...);
+}
 template <int kR>
 __device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Consts& k, const Cand* __restrict__ list,
                                                        const unsigned base, const unsigned n, const int lane_in) {
@@ -883,53 +907,45 @@ __device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Const
   // All indices are static so that the row stays in registers.
   const int mark = (t & 1) ? v2 : v1;             // L, E1 look for v1; R, E2 look for v2
   const int ins = t == 2 ? v2 : v1;
-  int p = 0;
-#pragma unroll
-  for (int j = kR - 1; j >= 0; --j) if (j < nrow && r[j] == mark) p = j;
+  // (fold expressions over the entry index instead of loops: every index is a literal, so the row
+  // is scalarised into registers whatever the optimiser makes of the conditions)
+  const int p = row_find(r, nrow, mark, RowIdx<kR>{});
+  int w[kR];
   int nnew;
-  if (t < 2) {
-#pragma unroll
-    for (int j = 0; j < kR - 1; ++j) if (j >= p) r[j] = r[j + 1];
-    nnew = nrow - 1;
-  } else {
-#pragma unroll
-    for (int j = kR - 1; j > 0; --j) if (j > p + 1) r[j] = r[j - 1];      // nrow < S (R10): nothing falls off
-#pragma unroll
-    for (int j = 1; j < kR; ++j) if (j == p + 1) r[j] = ins;
-    nnew = nrow + 1;
-  }
+  if (t < 2) { row_delete(r, w, p, RowIdx<kR>{}); nnew = nrow - 1; }
+  else { row_insert(r, w, p, ins, RowIdx<kR>{}); nnew = nrow + 1; }      // nrow < S (R10): nothing falls off
   __syncwarp(wins);
+  row_pad(w, r, nnew, RowIdx<kR>{});                                      // r = the new row, padding repeats entry 0
   const int e0 = r[0];
-#pragma unroll
-  for (int j = 1; j < kR; ++j) if (j >= nnew) r[j] = e0;
 #pragma unroll
   for (int q = 0; q < kR / 4; ++q)
     if (4 * q < k.S) d.cv[(size_t)q * k.N + cell] = make_int4(r[4 * q], r[4 * q + 1], r[4 * q + 2], r[4 * q + 3]);
   d.cvn[cell] = nnew;
   AVM_TR_W0(3, nnew);
   // ---- refresh the cached geometry of my cell (directors unchanged): the same serial sum as the
-  // per-step pass (geom_edge), so that a resumed run reproduces these records bit for bit.  v1 and
-  // v2 take their new positions from registers; positions are fetched eight at a time (entries
-  // beyond the row repeat entry 0, whose position is substituted without a load).
-  const double2 h0 = e0 == v1 ? n1 : e0 == v2 ? n2 : pos_ld(d.pos + e0, k);
+  // per-step pass (geom_edge), so that a resumed run reproduces these records bit for bit.  Positions
+  // are fetched eight at a time with unconditional, mutually independent loads (entries beyond the
+  // row repeat entry 0: a valid index, the same sector); v1 and v2 take their new positions from
+  // registers whatever the loads return.
+  const double2 g0 = pos_ld(d.pos + e0, k);
+  const double2 h0 = e0 == v1 ? n1 : e0 == v2 ? n2 : g0;
   double rxp = 0.0, ryp = 0.0, acc = 0.0, per = 0.0;
 #pragma unroll
-  for (int j0 = 1; j0 < kR; j0 += 8) {
-    if (j0 < nnew) {
-      double2 hh[8];
+  for (int b = 0; 1 + 8 * b < kR; ++b) {
+    if (1 + 8 * b < nnew) {
+      double2 g[8];
 #pragma unroll
       for (int u = 0; u < 8; ++u) {
-        hh[u] = h0;
-        if (j0 + u < kR) {
-          const int e = r[j0 + u < kR ? j0 + u : 0];
-          if (j0 + u < nnew) hh[u] = e == v1 ? n1 : e == v2 ? n2 : pos_ld(d.pos + e, k);
-        }
+        g[u] = g0;
+        if (1 + 8 * b + u < kR) g[u] = pos_ld(d.pos + r[1 + 8 * b + u < kR ? 1 + 8 * b + u : 0], k);
       }
 #pragma unroll
       for (int u = 0; u < 8; ++u) {
-        if (j0 + u < nnew) {
-          const double rx = min_image(__dsub_rn(hh[u].x, h0.x), k.Lx, k.hLx);
-          const double ry = min_image(__dsub_rn(hh[u].y, h0.y), k.Ly, k.hLy);
+        if (1 + 8 * b + u < kR && 1 + 8 * b + u < nnew) {
+          const int e = r[1 + 8 * b + u < kR ? 1 + 8 * b + u : 0];
+          const double2 hu = e == v1 ? n1 : e == v2 ? n2 : g[u];
+          const double rx = min_image(__dsub_rn(hu.x, h0.x), k.Lx, k.hLx);
+          const double ry = min_image(__dsub_rn(hu.y, h0.y), k.Ly, k.hLy);
           geom_edge(rxp, ryp, rx, ry, acc, per);
           rxp = rx; ryp = ry;
         }
@@ -965,8 +981,11 @@ t1_flip_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, 
   if (count_stats && gwarp == 0 && lane == 0 && n_cand) atomicAdd((unsigned long long*)&d.ctr->t1_candidates, (unsigned long long)n_cand);
   if (count_stats && parity < 2u && gwarp == 0 && lane == 0) *d.feedback = n_cand;     // the step's list: report the T1 load
   unsigned int flips = 0, seen = 0;
+  // the implementation is inlined here (pointers and constants come straight from the kernel's
+  // constant bank; the row stays in registers): the kernel is a chain of dependent round trips and
+  // every reload or local-memory access in it would queue behind the outstanding gathers
   for (unsigned int i = gwarp * 8u; i < n_cand; i += nwarps * 8u) {
-    flips += t1_flip_quads(d, k, list, i, n_cand, lane);
+    flips += k.S <= 16 ? t1_flip_quads_impl<16>(d, k, list, i, n_cand, lane) : t1_flip_quads(d, k, list, i, n_cand, lane);
     seen += min(8u, n_cand - i);
   }
   if (count_stats && lane == 0) {
