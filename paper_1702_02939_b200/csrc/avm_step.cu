@@ -534,8 +534,10 @@ __device__ __noinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va,
   cd.cL = cL; cd.cR = cR; cd.cE1 = cE1; cd.cE2 = cE2;
   cd.key = ((unsigned long long)t1 << 32) | t2;
   cd.x1 = x1; cd.y1 = y1; cd.x2 = x2; cd.y2 = y2;
-  cd.sx1 = x1s1 == v1 ? 1 : x1s2 == v1 ? 2 : 0;
-  cd.sx2 = x2s1 == v2 ? 1 : x2s2 == v2 ? 2 : 0;
+  // slots of v1 in x1 and of v2 in x2 (2 bits each) and the vertex counts of the four cells (one byte each): a
+  // winner owns its four cells (R11), so the counts still hold when it flips and the flip need not load them
+  cd.sx1 = (x1s1 == v1 ? 1 : x1s2 == v1 ? 2 : 0) | ((x2s1 == v2 ? 1 : x2s2 == v2 ? 2 : 0) << 2);
+  cd.sx2 = nq[0] | (nq[1] << 8) | (nq[2] << 16) | (nq[3] << 24);
   const unsigned int slot = atomicAdd(&d.ctr->n_cand[parity], 1u);
   if (slot >= list_cap(k, parity)) {          // cannot happen for a tiling (<= 3N edges; N per repeated pass)
     atomicOr((unsigned long long*)&d.ctr->error, 8ull);
@@ -840,17 +842,20 @@ __device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Const
   const int v1 = ca.x, v2 = ca.y, k1 = ca.z, k2 = ca.w;
   const int cL = cb.x, cR = cb.y, cE1 = cb.z, cE2 = cb.w;
   const unsigned long long key = ((unsigned long long)(unsigned)cc.y << 32) | (unsigned)cc.x;
-  const int sx1 = cc.z, sx2 = cc.w;
+  const int sx1 = cc.z & 3, sx2 = (cc.z >> 2) & 3;
   const int x1 = cd.x, y1 = cd.y, x2 = cd.z, y2 = cd.w;
   const int cell = t == 0 ? cL : t == 1 ? cR : t == 2 ? cE1 : cE2;     // 0 for idle groups: a valid index
   const unsigned long long mk = d.minkey[cell];
-  const int nrow = d.cvn[cell];
+  const int nrow = (cc.w >> (8 * t)) & 0xff;            // as counted by the marking thread (a winner's cells are its own)
+  const int need = t < 2 ? nrow : nrow + 1;             // entries of the longer of the old and the new row
   const double2 h1 = pos_ld(d.pos + v1, k), h2 = pos_ld(d.pos + v2, k);
+  // planes 0 and 1 always (their padding is part of the cell pass's fixed-trip head), later planes only when the
+  // row reaches them: nobody reads the padding of a plane the row does not reach
   int r[kR];
 #pragma unroll
   for (int q = 0; q < kR / 4; ++q) {
     int4 e = make_int4(0, 0, 0, 0);
-    if (4 * q < k.S) e = d.cv[(size_t)q * k.N + cell];
+    if (4 * q < k.S && (q < 2 || 4 * q < need)) e = d.cv[(size_t)q * k.N + cell];
     r[4 * q] = e.x; r[4 * q + 1] = e.y; r[4 * q + 2] = e.z; r[4 * q + 3] = e.w;
   }
   const unsigned agree = __ballot_sync(kFull, have && mk == key);
@@ -919,7 +924,7 @@ __device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Const
   const int e0 = r[0];
 #pragma unroll
   for (int q = 0; q < kR / 4; ++q)
-    if (4 * q < k.S) d.cv[(size_t)q * k.N + cell] = make_int4(r[4 * q], r[4 * q + 1], r[4 * q + 2], r[4 * q + 3]);
+    if (4 * q < k.S && (q < 2 || 4 * q < need)) d.cv[(size_t)q * k.N + cell] = make_int4(r[4 * q], r[4 * q + 1], r[4 * q + 2], r[4 * q + 3]);
   d.cvn[cell] = nnew;
   AVM_TR_W0(3, nnew);
   // ---- refresh the cached geometry of my cell (directors unchanged): the same serial sum as the
