@@ -421,6 +421,8 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   if (c.error & 4) return fail(AVM_EINCONSISTENT);
   s->t1_guess = c.n_win;
   if (s->h_feedback) *s->h_feedback = s->t1_guess;
+  // the device rewrites the host word only when the load crosses the schedule threshold: both sides start from the guess
+  AVM_CUDA_F(cudaMemcpyAsync(&s->ctr->fb_last, &s->t1_guess, sizeof(unsigned int), cudaMemcpyHostToDevice, st));
   s->launches += launch_refresh_cells(d, k, st);
   if (params->flags & AVM_FLAG_SORT_AT_CREATE) do_sort(s);
   AVM_CUDA_F(cudaGetLastError());
@@ -505,9 +507,6 @@ int avm_create_host(const avm_params* params, const double* pos_xy, const int32_
 // launch reports through a mapped host word (read here without synchronising; it lags the device by
 // however far the host runs ahead, which is fine for a slowly varying load), before that from the
 // number of short edges at creation.  Both schedules give the same bits.
-#ifndef AVM_FUSED_MAX_CANDIDATES
-#define AVM_FUSED_MAX_CANDIDATES 128
-#endif
 static bool leave_flips_pending(const avm_sim* s, bool last_of_call) {
   if (!s->fused_ok || last_of_call) return false;   // the last step of a call is completed inside the call
   if (s->p.sort_every > 0 && (s->step + 1 - s->p.step0) % (unsigned long long)s->p.sort_every == 0) return false;   // so is the step before a re-sort

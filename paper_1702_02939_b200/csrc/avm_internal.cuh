@@ -55,7 +55,8 @@ struct Counters {
   unsigned int n_cand[4];   // [0], [1]: the step's list by step parity; [2], [3]: lists of repeated passes (NEXT-1)
   unsigned int n_win;     // winners (debug hook); short edges at creation
   unsigned int feedback_sink;   // target of Dev::feedback when no mapped host word is available
-  unsigned int pad0[26];
+  unsigned int fb_last;         // T1 load last written to Dev::feedback (it is rewritten only when the load crosses the schedule threshold)
+  unsigned int pad0[25];
   // fused schedule, zeroed by the cell pass of every step.  Each on a 128-byte line of its own: the
   // first is hammered by claiming atomics while waiting warps poll the second.
   unsigned int next_cand; // next candidate index to be claimed
@@ -70,6 +71,12 @@ struct Counters {
   // min start / max phase-end times (ns, %globaltimer), tr_acc = sums of (phase end - start) over launches
   unsigned long long tr[8], tr_acc[8], tr2[80];
 };
+
+// Up to this many T1 candidates a step leaves its flips to the next force/move launch (two launches per
+// step); beyond, the stand-alone T1 kernel is faster.
+#ifndef AVM_FUSED_MAX_CANDIDATES
+#define AVM_FUSED_MAX_CANDIDATES 128
+#endif
 
 // Model constants, passed by value to every kernel.
 struct Consts {

@@ -200,6 +200,18 @@ __device__ __noinline__ void move_vertex_coherent(const Dev& d, const Consts& k,
   move_vertex(d, k, v, h, q[0], q[1], q[2], c[0], c[1], c[2]);
 }
 
+// The host chooses the schedule of later steps from the T1 load (avm_api.cu: leave_flips_pending), which it
+// reads from a mapped host word.  A store to host memory must be flushed over PCIe before the kernel
+// can complete (measured: up to 0.7 us per step), so the word is only written when the load crosses the
+// threshold the host compares it with.
+__device__ __forceinline__ void report_t1_load(const Dev& d, const unsigned n) {
+  const unsigned last = d.ctr->fb_last;
+  if ((n > (unsigned)AVM_FUSED_MAX_CANDIDATES) != (last > (unsigned)AVM_FUSED_MAX_CANDIDATES)) {
+    d.ctr->fb_last = n;
+    *d.feedback = n;
+  }
+}
+
 __device__ __forceinline__ unsigned int ld_volatile(const unsigned int* p) {
   unsigned int x;
   asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(x) : "l"(p) : "memory");
@@ -415,7 +427,7 @@ force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts 
   const int lane = threadIdx.x & 31;
   const unsigned prev = min(d.ctr->n_cand[parity ^ 1u], (unsigned)k.cap_a);
   const unsigned gwarp = (unsigned)tid >> 5, nwarps = (unsigned)stride >> 5;
-  if (tid == 0) { d.ctr->n_cand[parity] = 0; if (kFused) *d.feedback = prev; }   // whoever applies a list reports its length
+  if (tid == 0) { d.ctr->n_cand[parity] = 0; if (kFused) report_t1_load(d, prev); }   // whoever applies a list reports its length
   if (kFused) {
     if (prev == 0u) { sweep<false>(d, k, nullptr, tid, stride, lane); return; }
     if (tid == 0) atomicAdd((unsigned long long*)&d.ctr->t1_candidates, (unsigned long long)prev);
@@ -984,7 +996,7 @@ t1_flip_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, 
   const int lane = threadIdx.x & 31;
   const unsigned gwarp = (blockIdx.x * kT1Block + threadIdx.x) >> 5, nwarps = (gridDim.x * kT1Block) >> 5;
   if (count_stats && gwarp == 0 && lane == 0 && n_cand) atomicAdd((unsigned long long*)&d.ctr->t1_candidates, (unsigned long long)n_cand);
-  if (count_stats && parity < 2u && gwarp == 0 && lane == 0) *d.feedback = n_cand;     // the step's list: report the T1 load
+  if (count_stats && parity < 2u && gwarp == 0 && lane == 0) report_t1_load(d, n_cand);     // the step's list: report the T1 load
   unsigned int flips = 0, seen = 0;
   // the implementation is inlined here (pointers and constants come straight from the kernel's
   // constant bank; the row stays in registers): the kernel is a chain of dependent round trips and
