@@ -75,7 +75,7 @@ struct Counters {
 // Up to this many T1 candidates a step leaves its flips to the next force/move launch (two launches per
 // step); beyond, the stand-alone T1 kernel is faster.
 #ifndef AVM_FUSED_MAX_CANDIDATES
-#define AVM_FUSED_MAX_CANDIDATES 128
+#define AVM_FUSED_MAX_CANDIDATES 1024
 #endif
 
 // Model constants, passed by value to every kernel.

@@ -29,7 +29,10 @@
 namespace avm {
 namespace cg = cooperative_groups;
 
-static constexpr int kVertexBlock = 256;
+#ifndef AVM_VERTEX_BLOCK
+#define AVM_VERTEX_BLOCK 256
+#endif
+static constexpr int kVertexBlock = AVM_VERTEX_BLOCK;
 #ifndef AVM_CELL_BLOCK
 #define AVM_CELL_BLOCK 128
 #endif
@@ -415,7 +418,7 @@ __device__ __forceinline__ void release_minkeys(const Dev& d, const unsigned i0,
 // candidate has been decided.  The latency-bound flips thus overlap the gather-bound sweep and
 // the step needs no third launch.
 #ifndef AVM_LIGHT_MAX
-#define AVM_LIGHT_MAX 256       // up to this many candidates: one dedicated flipper warp per candidate
+#define AVM_LIGHT_MAX 1024      // up to this many candidates: one dedicated flipper warp per candidate (measured at N = 1M: 256, 512, 1024, 2048)
 #endif
 template <bool kFused>
 __global__ void __launch_bounds__(kVertexBlock, AVM_FM_MINB)
@@ -435,7 +438,7 @@ force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts 
     if (lane == 0) atomicMin(&d.ctr->tr[0], gtime());
 #endif
     const unsigned int* __restrict__ dirty = d.dirty + (size_t)(parity ^ 1u) * (size_t)k.nw;
-    if (prev <= AVM_LIGHT_MAX) {
+    if (prev <= AVM_LIGHT_MAX && 3u * prev <= nwarps) {      // (a small grid must keep most of its warps for the sweep)
       // few candidates: one dedicated warp per candidate (warp 0 of the first CTAs, then warp 1, ...:
       // consecutive CTAs sit on different SMs) flips it, waits for all decisions and moves the
       // vertices of its cells, all in the shadow of the sweep; every other warp only sweeps
