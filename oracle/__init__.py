@@ -63,6 +63,8 @@ def _load() -> ctypes.CDLL:
         lib.oracle_energy.restype = ctypes.c_double
         lib.oracle_compute_forces.argtypes = [p, p, p]
         lib.oracle_step.argtypes = [p, i64]
+        lib.oracle_step_move_and_rotate.argtypes = [p]
+        lib.oracle_step_topology_and_advance.argtypes = [p]
         lib.oracle_t1_pass.argtypes = [p]
         lib.oracle_set_cell_targets.argtypes = [p, p, p]
         lib.oracle_set_cell_moduli.argtypes = [p, p, p]
@@ -161,6 +163,14 @@ class OracleSim:
 
     def step(self, n: int = 1) -> None:
         _load().oracle_step(self._h, n)
+
+    def step_move_and_rotate(self) -> None:
+        """first half of one step: geometry, forces, move, director update"""
+        _load().oracle_step_move_and_rotate(self._h)
+
+    def step_topology_and_advance(self) -> None:
+        """second half: the T1 pass(es) on the moved positions and the step counter"""
+        _load().oracle_step_topology_and_advance(self._h)
 
     def set_cell_targets(self, A0=None, P0=None) -> None:
         """per-cell preferred area / perimeter of Eq. 1 (user order); None, None = uniform again"""

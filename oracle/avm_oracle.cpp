@@ -339,7 +339,10 @@ size_t t1_pass(Sim& s, bool count_detect = true) {
 // vertices with the current directors (Eq. 4, :56; R5, R7) -> rotate the directors (:50, :104;
 // R8) -> test/update the topology on the moved positions (:64, :106-108) -> s <- s+1.
 // ------------------------------------------------------------------------------------------
-void step(Sim& s) {
+// The first four stages: everything up to, and excluding, the topology update.  Split off so that a test can
+// look at the moved tiling of a step before its T1 pass (what the CUDA path's observing geometry
+// pass reduces); step() below is the two halves back to back.
+void step_move_and_rotate(Sim& s) {
   std::vector<double> AP;
   geometry(s, AP);                                                   // 1
   std::vector<double> F(2 * s.V);
@@ -361,12 +364,18 @@ void step(Sim& s) {
   const double amp = std::sqrt(2.0 * s.p.Dr * s.p.dt);               // 4: Euler-Maruyama (R8)
   for (int64_t c = 0; c < s.N; ++c)
     s.theta[c] += amp * director_noise(s.p.seed, (uint64_t)s.st.step, (uint64_t)c);
+}
+void step_topology_and_advance(Sim& s) {
   // 5: one pass (north_star), or the paper's rule ("called repeatedly until no
   // changes"): repeat until a pass finds no candidate, at most t1_max_passes passes
   const int passes = s.p.t1_max_passes > 1 ? s.p.t1_max_passes : 1;
   for (int pass = 0; pass < passes; ++pass)
     if (t1_pass(s, pass == 0) == 0) break;
   ++s.st.step;                                                       // 6
+}
+void step(Sim& s) {
+  step_move_and_rotate(s);
+  step_topology_and_advance(s);
 }
 
 }  // namespace
@@ -431,6 +440,9 @@ int oracle_step(oracle_sim* s, int64_t n_steps) {
   for (int64_t i = 0; i < n_steps; ++i) step(*s);
   return 0;
 }
+// the two halves of one step (test hooks): stages 1-4, then the topology update and the step counter
+int oracle_step_move_and_rotate(oracle_sim* s) { step_move_and_rotate(*s); return 0; }
+int oracle_step_topology_and_advance(oracle_sim* s) { step_topology_and_advance(*s); return 0; }
 
 // one T1 pass on the current state without moving anything else (test hook)
 // NEXT-4: per-cell preferred values of Eq. 1, user order; NULL, NULL = uniform again

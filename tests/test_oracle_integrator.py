@@ -228,3 +228,28 @@ def test_msd_equals_an_independent_unwrapping_of_the_trajectory():
     assert abs(sim.msd() - ref) < 1e-10 * ref
     assert sim.get_state()["stats"]["t1_flips"] > 0
     assert abs(sim.observables()["msd"] - sim.msd()) == 0.0
+
+
+def test_the_two_halves_of_a_step_are_the_step():
+    """oracle.step is step_move_and_rotate followed by step_topology_and_advance (the split only exposes
+    the moved tiling before the topology update, PAPER.md:62-64 order): identical bits, and between the
+    halves the step counter has not advanced, positions have moved and no flip has been counted."""
+    t = w.config_tiling(0)
+    p = w.config_params(0)
+    a = oracle.from_tiling(t, **p)
+    b = oracle.from_tiling(t, **p)
+    for _ in range(30):
+        a.step(1)
+        before = b.get_state()
+        b.step_move_and_rotate()
+        mid = b.get_state()
+        assert mid["stats"]["step"] == before["stats"]["step"]
+        assert mid["stats"]["t1_flips"] == before["stats"]["t1_flips"]
+        assert np.array_equal(mid["cell_vertices"], before["cell_vertices"])
+        assert not np.array_equal(mid["pos"], before["pos"])
+        b.step_topology_and_advance()
+        sa, sb = a.get_state(), b.get_state()
+        for key in ("pos", "theta", "cell_vertices", "cell_vertex_num", "vertex_neighbors", "vertex_cell_neighbors"):
+            assert np.array_equal(sa[key], sb[key]), key
+        assert sa["stats"] == sb["stats"]
+    assert a.get_state()["stats"]["t1_flips"] > 0
