@@ -172,6 +172,16 @@ typedef struct avm_observables {
 } avm_observables;
 int avm_observe(avm_sim* sim, avm_observables* out);
 
+/* Advance n_steps >= 1 timesteps like avm_step and observe WITHOUT an extra pass over the state
+ * ("reductions fused into the geometry pass"): the geometry pass of the
+ * last step, which computes every cell's area and perimeter anyway, also reduces the
+ * observables, in a fixed order (deterministic).  They therefore describe the MOVED tiling of that
+ * step - after its vertex move and director update, before its T1 pass (PAPER.md:62-64 order) -
+ * whereas avm_observe describes the state between steps; the two agree whenever the step flips
+ * nothing.  out->step and out->t1_flips are read after the step.  out is a HOST pointer;
+ * synchronises the stream. */
+int avm_step_observe(avm_sim* sim, int64_t n_steps, avm_observables* out);
+
 /* Mean-square displacement (the fluid/solid diagnostic of the regimes of
  * PAPER.md:114-116): <|U_v(t) - U_v(t_ref)|^2> over all vertices, U = unwrapped position.  The library
  * counts, per vertex, the box lengths it has left through the boundary (in the move of Eq. 4 and

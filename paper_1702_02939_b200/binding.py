@@ -23,7 +23,7 @@ LIB_MIXED_PATH = os.path.join(_HERE, "libavm_b200_mixed.so")
 # every symbol include/avm.h declares (tests check that the library exports all of them)
 ABI_SYMBOLS = [
     "avm_workspace_bytes", "avm_create", "avm_create_host", "avm_step", "avm_step_profile", "avm_compute_forces",
-    "avm_compute_forces_host", "avm_energy", "avm_observe", "avm_set_cell_targets", "avm_set_cell_moduli", "avm_msd_reset", "avm_get_state", "avm_get_state_host", "avm_debug_t1",
+    "avm_compute_forces_host", "avm_energy", "avm_observe", "avm_step_observe", "avm_set_cell_targets", "avm_set_cell_moduli", "avm_msd_reset", "avm_get_state", "avm_get_state_host", "avm_debug_t1",
     "avm_t1_pass", "avm_set_positions", "avm_resort", "avm_philox_words", "avm_hilbert_index",
     "avm_hilbert_index_host", "avm_destroy", "avm_strerror", "avm_last_cuda_error", "avm_precision",
 ]
@@ -88,6 +88,7 @@ def _load(path: str = LIB_PATH) -> ctypes.CDLL:
     lib.avm_compute_forces_host.argtypes = [p, p, p]
     lib.avm_energy.argtypes = [p, ctypes.POINTER(ctypes.c_double)]
     lib.avm_observe.argtypes = [p, ctypes.POINTER(AvmObservables)]
+    lib.avm_step_observe.argtypes = [p, i64, ctypes.POINTER(AvmObservables)]
     for name in ("avm_get_state", "avm_get_state_host"):
         getattr(lib, name).argtypes = [p, p, p, p, p, p, p, ctypes.POINTER(AvmStats)]
     lib.avm_debug_t1.argtypes = [p, p, ctypes.POINTER(i64), p, ctypes.POINTER(i64), i64]
@@ -265,6 +266,12 @@ class AvmSim:
     def observe(self) -> dict:
         o = AvmObservables()
         _check(self.lib.avm_observe(self._h, ctypes.byref(o)))
+        return o.as_dict()
+
+    def step_observe(self, n: int = 1) -> dict:
+        """n steps; the geometry pass of the last one also reduces the observables of its moved tiling"""
+        o = AvmObservables()
+        _check(self.lib.avm_step_observe(self._h, n, ctypes.byref(o)))
         return o.as_dict()
 
     def get_state(self, stats: bool = True) -> dict:

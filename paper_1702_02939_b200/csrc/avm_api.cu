@@ -74,7 +74,7 @@ Layout make_layout(const avm_params& p) {
   L.dirty = take(4 * 2 * dirty_words(V));
   L.estamp = take(12 * Vs);
   L.ap = take(16 * N);
-  L.epart = take(8 * 8 * 512);   // block partials of the observables (8 slots x up to 512 blocks)
+  L.epart = take(8 * 16 * (size_t)(cell_pass_grid(p.n_cells) > 512 ? cell_pass_grid(p.n_cells) : 512));   // block partials of the observables (up to 16 slots x the CTAs of the cell pass)
   for (int i = 0; i < 2; ++i) { L.key[i] = take(4 * V); L.val[i] = take(4 * V); }
   L.hist = take(4 * sort_hist_entries((int)V));
   L.newidx_v = take(4 * V); L.newidx_c = take(4 * N); L.order_v = take(4 * V); L.order_c = take(4 * N);
@@ -629,9 +629,27 @@ int avm_energy(avm_sim* s, double* energy) {
   return AVM_OK;
 }
 
+static int fill_observables(avm_sim* s, avm_observables* out);
+
 int avm_observe(avm_sim* s, avm_observables* out) {
   if (!s || !out) return AVM_EINVAL;
   s->launches += launch_energy(s->dev(), s->k, s->epart, s->stream);
+  return fill_observables(s, out);
+}
+
+int avm_step_observe(avm_sim* s, int64_t n_steps, avm_observables* out) {
+  if (!s || !out || n_steps < 1) return AVM_EINVAL;
+  int rc = avm_step(s, n_steps - 1);            // whole steps: the last one of that call is completed inside it
+  if (rc) return rc;
+  s->launches += launch_step(s->dev(), s->k, s->step, s->stream, nullptr, false, false, s->epart);
+  s->cur_pos = 1 - s->cur_pos;
+  s->launches += extra_t1_passes(s);
+  ++s->step;
+  if (s->p.sort_every > 0 && (s->step - s->p.step0) % (unsigned long long)s->p.sort_every == 0) do_sort(s);
+  return fill_observables(s, out);
+}
+
+static int fill_observables(avm_sim* s, avm_observables* out) {
   Counters c;
   int rc = read_counters(s, &c);
   if (rc) return rc;

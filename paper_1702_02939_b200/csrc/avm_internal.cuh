@@ -321,8 +321,11 @@ __device__ __forceinline__ unsigned list_cap(const Consts& k, unsigned list) { r
 int force_move_grid(int V);
 // One timestep.  consume_pending: the previous step left its T1 flips pending (they ride in this force/move
 // launch); leave_pending: this step leaves its own flips pending (two launches) instead of running t1_flip_kernel.
+// obs_partial (optional, one double per observable slot and CTA of the cell pass): the cell pass also reduces the
+// observables of the moved tiling (avm_step_observe).
 int launch_step(const Dev& d, const Consts& k, unsigned long long step, cudaStream_t s, cudaEvent_t* ev, bool consume_pending,
-                bool leave_pending);
+                bool leave_pending, double* obs_partial = nullptr);
+int cell_pass_grid(int N);
 int launch_count_short_edges(const Dev& d, const Consts& k, cudaStream_t s);
 int persistent_grid(int V, bool per_cell);
 int launch_persistent_steps(const Dev& d, const Consts& k, unsigned long long step0, int n_steps, int grid, cudaStream_t s);

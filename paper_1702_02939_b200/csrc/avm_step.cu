@@ -615,9 +615,16 @@ __device__ __noinline__ void t1_report_cell(const Dev& d, const Consts& k, int c
 // streams are read with cache hints and the gathers through the non-coherent path.
 template <bool kCoh, typename T> __device__ __forceinline__ T cu_stream(const T* p) { return kCoh ? __ldcg(p) : ld_stream(p); }
 template <bool kCoh> __device__ __forceinline__ double2 cu_pos(const pos_t* p, const Consts& k) { return kCoh ? pos_ldcg(p, k) : pos_ldg(p, k); }
-template <bool kStep, bool kPerCell, bool kCoh>
+// Observables (NEXT-2; slots documented at observables_partial_kernel below).  kObs: the pass also reduces
+// them over the moved tiling it is computing anyway (avm_step_observe): per-thread values, a fixed
+// tree over the CTA in shared memory, one partial per CTA and slot; observables_final_kernel finishes.
+static constexpr int kObs = 9;
+__device__ __forceinline__ double obs_combine(int slot, double a, double b) {
+  return slot == 6 ? fmin(a, b) : slot == 7 ? fmax(a, b) : a + b;
+}
+template <bool kStep, bool kPerCell, bool kCoh, bool kObserve = false>
 __device__ __forceinline__ void cell_update_body(const Dev& d, const Consts& k, const unsigned long long step, const unsigned parity,
-                                                 const int gid) {
+                                                 const int gid, double* __restrict__ obs_partial = nullptr) {
   if (kStep && gid == 0) { d.ctr->flip_done = 0; d.ctr->next_cand = 0; }   // the previous list is long done
 #ifdef AVM_TRACE
   if (kStep && gid == 0) {
@@ -662,6 +669,21 @@ __device__ __forceinline__ void cell_update_body(const Dev& d, const Consts& k, 
 #pragma unroll
     for (int j = 1; j < 8; ++j) { rx[j] = min_image(rx[j], k.Lx, k.hLx); ry[j] = min_image(ry[j], k.Ly, k.hLy); }
   }
+  // ---- observing pass: squared unwrapped displacement of the row's vertices since the MSD reference; every
+  // vertex belongs to exactly three rows, so the sum over cells is three times the sum over vertices ----
+  double msd3 = 0.0;
+  if (kObserve) {
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      if (j < n) {
+        const int t = d.vtag[e[j]];
+        const int2 im = d.img[t];
+        const double2 r0 = d.msd_ref[t];
+        const double ux = (h[j].x + (double)im.x * k.Lx) - r0.x, uy = (h[j].y + (double)im.y * k.Ly) - r0.y;
+        msd3 += ux * ux + uy * uy;
+      }
+    }
+  }
   // ---- shoelace + perimeter; bit j-1 of smask = the edge ending at row entry j looks short ----
   double acc = 0.0, per = 0.0, rxp = 0.0, ryp = 0.0;
   unsigned smask = 0;
@@ -691,6 +713,13 @@ __device__ __forceinline__ void cell_update_body(const Dev& d, const Consts& k, 
           const double l2 = geom_edge(rxp, ryp, x, y, acc, per);
           if (kStep && hi_word(l2) <= hlc) smask |= 1u << (j0 + i - 1);
           rxp = x; ryp = y;
+          if (kObserve) {
+            const int t = d.vtag[ee[i]];
+            const int2 im = d.img[t];
+            const double2 r0 = d.msd_ref[t];
+            const double ux = (hh[i].x + (double)im.x * k.Lx) - r0.x, uy = (hh[i].y + (double)im.y * k.Ly) - r0.y;
+            msd3 += ux * ux + uy * uy;
+          }
         }
       }
     }
@@ -698,6 +727,29 @@ __device__ __forceinline__ void cell_update_body(const Dev& d, const Consts& k, 
   {  // closing edge of an n >= 8 cell (an exact no-op for smaller ones, which closed above)
     const double l2 = geom_edge(rxp, ryp, 0.0, 0.0, acc, per);
     if (kStep && hi_word(l2) <= hlc) smask |= 1u << ((n > 8 ? n : 8) - 1);
+  }
+  if (kObserve) {
+    // slots as in observables_partial_kernel; threads beyond the last cell contribute the identities
+    __shared__ double sm[kObs][kCellBlock];
+    const double A = __dmul_rn(0.5, acc), P = per;
+    double x[kObs] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 1.0e300, -1.0e300, 0.0};
+    if (valid) {
+      const CellPar q = cell_params(d, k, c);
+      x[0] = q.KA * (A - q.A0) * (A - q.A0) + q.KP * (P - q.P0) * (P - q.P0);
+      x[1] = A; x[2] = P;
+      if (A > 0.0) x[3] = P / sqrt(A); else x[4] = 1.0;
+      x[5] = A * A; x[6] = A; x[7] = A; x[8] = msd3;
+    }
+#pragma unroll
+    for (int q = 0; q < kObs; ++q) sm[q][threadIdx.x] = x[q];
+    __syncthreads();
+    for (int st = kCellBlock / 2; st > 0; st >>= 1) {
+      if ((int)threadIdx.x < st)
+#pragma unroll
+        for (int q = 0; q < kObs; ++q) sm[q][threadIdx.x] = obs_combine(q, sm[q][threadIdx.x], sm[q][threadIdx.x + st]);
+      __syncthreads();
+    }
+    if (threadIdx.x < kObs) obs_partial[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = sm[threadIdx.x][0];
   }
   if (!valid) return;
   CellRec r;
@@ -707,6 +759,15 @@ __device__ __forceinline__ void cell_update_body(const Dev& d, const Consts& k, 
   st_rec(d.rec + c, r);
   smask &= n >= 32 ? ~0u : (1u << n) - 1u;     // edges beyond the closing one are padding
   if (kStep && smask) t1_report_cell(d, k, c, n, smask, parity);
+}
+// the observing instantiation of the per-step pass (the last step of avm_step_observe)
+template <bool kPerCell>
+__global__ void __launch_bounds__(kCellBlock)
+cell_update_observe_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, const unsigned long long step,
+                           const unsigned parity, double* __restrict__ obs_partial) {
+  pdl_launch_dependents();
+  pdl_wait();
+  cell_update_body<true, kPerCell, false, true>(d, k, step, parity, blockIdx.x * kCellBlock + threadIdx.x, obs_partial);
 }
 template <bool kStep, bool kPerCell>
 __global__ void __launch_bounds__(kCellBlock, AVM_CU_MINB)
@@ -1162,10 +1223,6 @@ __global__ void forces_kernel(const Dev d, const Consts k, const double2* __rest
 // A <= 0, 5 sum A^2, 6 min A, 7 max A, 8 sum over vertices of the squared unwrapped displacement since the
 // MSD reference.  Block partials in a fixed order, finished by one block (deterministic, no
 // floating-point atomics).
-static constexpr int kObs = 9;
-__device__ __forceinline__ double obs_combine(int slot, double a, double b) {
-  return slot == 6 ? fmin(a, b) : slot == 7 ? fmax(a, b) : a + b;
-}
 __device__ __forceinline__ void obs_block_reduce(double (&x)[kObs], double (*sm)[256]) {
 #pragma unroll
   for (int q = 0; q < kObs; ++q) sm[q][threadIdx.x] = x[q];
@@ -1203,14 +1260,15 @@ observables_partial_kernel(const Dev d, const Consts k, double* __restrict__ par
   if (threadIdx.x < kObs) partial[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = sm[threadIdx.x][0];
 }
 __global__ void __launch_bounds__(256)
-observables_final_kernel(const Dev d, const double* __restrict__ partial, int n) {
+observables_final_kernel(const Dev d, const double* __restrict__ partial, int n, const double msd_scale) {
   __shared__ double sm[kObs][256];
   double x[kObs] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 1.0e300, -1.0e300, 0.0};
   for (int i = threadIdx.x; i < n; i += 256)
 #pragma unroll
     for (int q = 0; q < kObs; ++q) x[q] = obs_combine(q, x[q], partial[(size_t)q * n + i]);
   obs_block_reduce(x, sm);
-  if (threadIdx.x < kObs) d.ctr->obs[threadIdx.x] = sm[threadIdx.x][0];
+  // msd_scale: 1 for a sum over vertices, 1/3 for the sum over the rows of all cells (the observing cell pass)
+  if (threadIdx.x < kObs) d.ctr->obs[threadIdx.x] = threadIdx.x == 8 ? sm[8][0] * msd_scale : sm[threadIdx.x][0];
 }
 
 __global__ void philox_words_kernel(unsigned long long seed, unsigned long long step, unsigned long long cell0,
@@ -1223,6 +1281,7 @@ __global__ void philox_words_kernel(unsigned long long seed, unsigned long long 
 // launchers
 // ---------------------------------------------------------------------------------------------
 static inline int cdiv(long long a, int b) { return (int)((a + b - 1) / b); }
+int cell_pass_grid(int N) { return cdiv(N, kCellBlock); }
 
 // Grid of the persistent force/move kernel: a whole number of CTAs per SM of the current device,
 // never more CTAs than there is work.  Called once per simulation (avm_create); the result lives
@@ -1258,7 +1317,7 @@ static cudaError_t launch_chained(void (*kernel)(KArgs...), int grid, int block,
 //                    stand-alone T1 kernel (three launches, the step complete on return).
 // ev (optional, AVM_K_COUNT+1 events): recorded before/after each kernel by avm_step_profile.
 int launch_step(const Dev& d, const Consts& k, unsigned long long step, cudaStream_t s, cudaEvent_t* ev, bool consume_pending,
-                bool leave_pending) {
+                bool leave_pending, double* obs_partial) {
   const unsigned parity = (unsigned)(step & 1ull);
   if (ev) cudaEventRecord(ev[0], s);
   const bool pdl = AVM_PDL && ev == nullptr;   // events between the kernels would break the chain anyway
@@ -1270,12 +1329,20 @@ int launch_step(const Dev& d, const Consts& k, unsigned long long step, cudaStre
   Consts kc = k;
   kc.flag_dirty = leave_pending ? 1 : 0;       // the flagged-vertex bitmap is only needed when the flips stay pending
   kc.clear_dirty = consume_pending ? 1 : 0;    // the bitmap this step's force/move launch swept with is spent
-  if (k.per_cell) launch_chained(cell_update_kernel<true, true>, cdiv(k.N, kCellBlock), kCellBlock, s, pdl, m, kc, step, parity);
-  else launch_chained(cell_update_kernel<true, false>, cdiv(k.N, kCellBlock), kCellBlock, s, pdl, m, kc, step, parity);
+  const int cgrid = cdiv(k.N, kCellBlock);
+  int n_launched = leave_pending ? 2 : 3;
+  if (obs_partial) {
+    // the observing pass: same arithmetic, plus the reduction of the observables of the moved tiling (NEXT-2)
+    if (k.per_cell) launch_chained(cell_update_observe_kernel<true>, cgrid, kCellBlock, s, pdl, m, kc, step, parity, obs_partial);
+    else launch_chained(cell_update_observe_kernel<false>, cgrid, kCellBlock, s, pdl, m, kc, step, parity, obs_partial);
+    observables_final_kernel<<<1, 256, 0, s>>>(m, obs_partial, cgrid, 1.0 / 3.0);
+    ++n_launched;
+  } else if (k.per_cell) launch_chained(cell_update_kernel<true, true>, cgrid, kCellBlock, s, pdl, m, kc, step, parity);
+  else launch_chained(cell_update_kernel<true, false>, cgrid, kCellBlock, s, pdl, m, kc, step, parity);
   if (ev) cudaEventRecord(ev[2], s);
-  if (!leave_pending) launch_chained(t1_flip_kernel, kT1Grid, kT1Block, s, pdl, m, k, parity, true);
+  if (!leave_pending) launch_chained(t1_flip_kernel, kT1Grid, kT1Block, s, pdl && !obs_partial, m, k, parity, true);
   if (ev) cudaEventRecord(ev[3], s);
-  return leave_pending ? 2 : 3;
+  return n_launched;
 }
 
 // number of edges shorter than l_c in the current state -> ctr->n_win (creation: first guess of the T1 load)
@@ -1381,7 +1448,7 @@ int launch_compute_forces(const Dev& d, const Consts& k, double2* ap_scratch, do
 int launch_energy(const Dev& d, const Consts& k, double* partial, cudaStream_t s) {
   const int nb = 148 * 2;      // partial holds kObs * nb doubles
   observables_partial_kernel<<<nb, 256, 0, s>>>(d, k, partial);
-  observables_final_kernel<<<1, 256, 0, s>>>(d, partial, nb);
+  observables_final_kernel<<<1, 256, 0, s>>>(d, partial, nb, 1.0);
   return 2;
 }
 

@@ -785,3 +785,31 @@ def test_persistent_schedule_equals_the_launched_schedules(B, k, steps, sort_eve
             assert sa["stats"][key] == other["stats"][key], key
     assert sa["stats"]["t1_flips"] > 0
     assert abs(a.observe()["msd"] - c.observe()["msd"]) == 0.0
+
+
+@pytest.mark.parametrize("k,steps,sort_every", [(0, 7, 0), (1, 5, 3), (2, 4, 0)])
+def test_observing_geometry_pass_matches_the_oracle(B, k, steps, sort_every):
+    """NEXT-2, reductions fused into the geometry pass: avm_step_observe reduces the observables of the
+    moved tiling of its last step (after the move and the director update, before the T1 pass) inside
+    the cell pass.  Oracle side: the same step taken in its two halves, the numpy definitions evaluated
+    in between.  The step itself is unchanged: states match afterwards, and a further plain step too."""
+    t = w.config_tiling(k)
+    p = w.config_params(k)
+    g = B.from_tiling(t, **dict(p, sort_every=sort_every, sort_at_create=sort_every > 0))
+    o = oracle.from_tiling(t, **p)
+    for rep in range(3):
+        og = g.step_observe(steps)
+        o.step(steps - 1)
+        o.step_move_and_rotate()
+        oo = o.observables()
+        o.step_topology_and_advance()
+        for key in ("energy", "sum_area", "sum_perimeter", "mean_shape_index", "area_min", "area_max", "area_variance", "msd"):
+            assert abs(og[key] - oo[key]) <= 1e-9 * max(1.0, abs(oo[key])), (rep, key, og[key], oo[key])
+        assert og["n_nonpositive_area"] == oo["n_nonpositive_area"]
+        so = o.get_state()
+        assert og["step"] == so["stats"]["step"] and og["t1_flips"] == so["stats"]["t1_flips"]
+        assert_states_match(to_np(g.get_state()), so, t.Lx, t.Ly)
+    assert so["stats"]["t1_flips"] > 0 or k == 0
+    # observing costs nothing afterwards: the between-steps observables agree too
+    a, b = g.observe(), o.observables()
+    assert abs(a["energy"] - b["energy"]) <= 1e-9 * abs(b["energy"]) and abs(a["msd"] - b["msd"]) <= 1e-9 * max(1.0, b["msd"])
