@@ -137,7 +137,7 @@ def test_local_circumcircle_verdict_equals_the_brute_force_one():
     assert margin.min() > 0
     rng = np.random.default_rng(1)
     seen_bad = 0
-    for amp in (0.01, 0.03, 0.06, 0.1, 0.15, 0.2, 0.3):
+    for amp in (1e-6, 1e-5, 1e-4, 1e-3, 3e-3, 0.01, 0.03, 0.1, 0.3):
         for rep in range(3):
             r = np.mod(t.points + amp * rng.standard_normal(t.points.shape), 10.0)
             failed, margin, opp = o.test_triangulation(r)
@@ -145,4 +145,4 @@ def test_local_circumcircle_verdict_equals_the_brute_force_one():
             assert failed.any() == bad.any()
             assert not (failed.any(axis=1) & ~bad).any()
             seen_bad += int(bad.any())
-    assert 3 < seen_bad < 21
+    assert 3 < seen_bad < 24          # both verdicts occur (27 perturbations)
