@@ -199,6 +199,36 @@ int avm_get_state_host(avm_sim* sim, double* pos_xy, int32_t* cell_vertex_num, i
                        int32_t* vertex_neighbors, int32_t* vertex_cell_neighbors, double* theta,
                        avm_stats* stats);
 
+/* The GPU-only parts of one self-propelled-Voronoi (SPV) step on a FIXED triangulation (SURVEY.md section
+ * 8(f) NEXT-4; section II.C, App. A.2 :171-200).  The triangulation is the dual reading of the
+ * lists the simulation holds: vertex v <-> Delaunay triangle with corners
+ * vertex_cell_neighbors[v], row c of cell_vertices = the Voronoi vertices around cell c.  cell_xy: DEVICE
+ * pointer, [N][2] doubles in USER order, in [0,Lx)x[0,Ly), owned by the caller; a Voronoi start is the tiling
+ * whose vertices are the circumcentres of cell_xy.  The repair of an invalid triangulation (CPU/CGAL in the
+ * paper, :96-100) is out of scope: these calls never change the lists.  All pointers DEVICE unless stated.
+ *
+ * avm_spv_geometry: Voronoi vertex of every triangle = circumcentre of its three cells,
+ *   stored as the simulation's vertex positions (as avm_set_positions would) and, if non-NULL, in
+ *   voronoi_xy [V][2]; area_perim [N][2] (may be NULL) = (A_c, P_c) of the resulting cells.  Asynchronous.
+ * avm_spv_forces (Eq. A6-A7): force_xy [N][2] = -dE/dr_i with E of Eq. 1; force_sets
+ *   [N][S][2] (may be NULL) = the contribution of each Voronoi vertex of the row of cell i ("force
+ *   sets"; unused slots 0); the force is their sum in row order.  Asynchronous.
+ * avm_spv_step (Eq. 3): n_steps times geometry -> forces -> r_i += dt (mu F_i + v0 n_i)
+ *   with the director of the start of the step, wrap -> director noise (as in avm_step; the step counter
+ *   advances) -> empty-circumcircle test.  n_failed: HOST pointer to two int64: [0] = circumcircle tests
+ *   that failed after the last step, [1] = index (0-based, within this call) of the first step after
+ *   which any test failed, -1 if none.  cell_flags [N] int32 (may be NULL): 1 for the corners of every
+ *   failing triangle and the intruding cell after the last step ("cells that need an update").
+ *   Afterwards the simulation's vertex positions are the Voronoi vertices of the final cells.
+ *   Synchronises the stream.
+ * avm_spv_test_triangulation: the test alone on cell_xy; n_failed: HOST pointer to one int64.
+ *   A triangle's circumcircle is tested, strictly, against the cell opposite each of its three edges
+ *   (local Delaunay criterion: no test fails <=> the triangulation is the Delaunay triangulation). */
+int avm_spv_geometry(avm_sim* sim, const double* cell_xy, double* voronoi_xy, double* area_perim);
+int avm_spv_forces(avm_sim* sim, const double* cell_xy, double* force_xy, double* force_sets);
+int avm_spv_step(avm_sim* sim, double* cell_xy, int64_t n_steps, int64_t* n_failed, int32_t* cell_flags);
+int avm_spv_test_triangulation(avm_sim* sim, const double* cell_xy, int64_t* n_failed, int32_t* cell_flags);
+
 /* Test hooks, not on the timed path.
  * avm_debug_t1: T1 detection + conflict resolution (R9-R11) on the current state WITHOUT
  *   flipping.  Writes up to `capacity` (tag_min, tag_max) pairs of candidates and of winners to

@@ -23,7 +23,7 @@ LIB_MIXED_PATH = os.path.join(_HERE, "libavm_b200_mixed.so")
 # every symbol include/avm.h declares (tests check that the library exports all of them)
 ABI_SYMBOLS = [
     "avm_workspace_bytes", "avm_create", "avm_create_host", "avm_step", "avm_step_profile", "avm_compute_forces",
-    "avm_compute_forces_host", "avm_energy", "avm_observe", "avm_step_observe", "avm_set_cell_targets", "avm_set_cell_moduli", "avm_msd_reset", "avm_get_state", "avm_get_state_host", "avm_debug_t1",
+    "avm_compute_forces_host", "avm_energy", "avm_observe", "avm_step_observe", "avm_spv_geometry", "avm_spv_forces", "avm_spv_step", "avm_spv_test_triangulation", "avm_set_cell_targets", "avm_set_cell_moduli", "avm_msd_reset", "avm_get_state", "avm_get_state_host", "avm_debug_t1",
     "avm_t1_pass", "avm_set_positions", "avm_resort", "avm_philox_words", "avm_hilbert_index",
     "avm_hilbert_index_host", "avm_destroy", "avm_strerror", "avm_last_cuda_error", "avm_precision",
 ]
@@ -89,6 +89,10 @@ def _load(path: str = LIB_PATH) -> ctypes.CDLL:
     lib.avm_energy.argtypes = [p, ctypes.POINTER(ctypes.c_double)]
     lib.avm_observe.argtypes = [p, ctypes.POINTER(AvmObservables)]
     lib.avm_step_observe.argtypes = [p, i64, ctypes.POINTER(AvmObservables)]
+    lib.avm_spv_geometry.argtypes = [p, p, p, p]
+    lib.avm_spv_forces.argtypes = [p, p, p, p]
+    lib.avm_spv_step.argtypes = [p, p, i64, p, p]
+    lib.avm_spv_test_triangulation.argtypes = [p, p, p, p]
     for name in ("avm_get_state", "avm_get_state_host"):
         getattr(lib, name).argtypes = [p, p, p, p, p, p, p, ctypes.POINTER(AvmStats)]
     lib.avm_debug_t1.argtypes = [p, p, ctypes.POINTER(i64), p, ctypes.POINTER(i64), i64]
@@ -267,6 +271,36 @@ class AvmSim:
         o = AvmObservables()
         _check(self.lib.avm_observe(self._h, ctypes.byref(o)))
         return o.as_dict()
+
+    # ---- SPV on a fixed triangulation (cell_xy: torch float64 [N,2] on the device, user order) ----
+    def spv_geometry(self, cell_xy):
+        t = self.torch
+        vor = t.empty((self.V, 2), dtype=t.float64, device=self.device)
+        ap = t.empty((self.N, 2), dtype=t.float64, device=self.device)
+        _check(self.lib.avm_spv_geometry(self._h, cell_xy.data_ptr(), vor.data_ptr(), ap.data_ptr()))
+        return vor, ap
+
+    def spv_forces(self, cell_xy, sets: bool = True):
+        t = self.torch
+        F = t.empty((self.N, 2), dtype=t.float64, device=self.device)
+        fs = t.empty((self.N, self.S, 2), dtype=t.float64, device=self.device) if sets else None
+        _check(self.lib.avm_spv_forces(self._h, cell_xy.data_ptr(), F.data_ptr(), fs.data_ptr() if sets else None))
+        return F, fs
+
+    def spv_step(self, cell_xy, n: int = 1):
+        """advances cell_xy in place; returns (failed tests after the last step, first failing step or -1, flags [N])"""
+        t = self.torch
+        out = (ctypes.c_int64 * 2)()
+        flags = t.empty(self.N, dtype=t.int32, device=self.device)
+        _check(self.lib.avm_spv_step(self._h, cell_xy.data_ptr(), n, out, flags.data_ptr()))
+        return int(out[0]), int(out[1]), flags
+
+    def spv_test_triangulation(self, cell_xy):
+        t = self.torch
+        out = (ctypes.c_int64 * 1)()
+        flags = t.empty(self.N, dtype=t.int32, device=self.device)
+        _check(self.lib.avm_spv_test_triangulation(self._h, cell_xy.data_ptr(), out, flags.data_ptr()))
+        return int(out[0]), flags
 
     def step_observe(self, n: int = 1) -> dict:
         """n steps; the geometry pass of the last one also reduces the observables of its moved tiling"""

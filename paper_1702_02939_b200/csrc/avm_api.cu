@@ -744,6 +744,66 @@ int avm_msd_reset(avm_sim* s) {
   return AVM_OK;
 }
 
+// ---- SPV on a fixed triangulation (avm_spv.cu) ----
+static int spv_refresh(avm_sim* s, const double* cell_xy, double* voronoi_xy) {
+  s->launches += launch_spv_voronoi(s->dev(), s->k, cell_xy, voronoi_xy, s->stream);
+  s->launches += launch_refresh_cells(s->dev(), s->k, s->stream);
+  return AVM_OK;
+}
+
+int avm_spv_geometry(avm_sim* s, const double* cell_xy, double* voronoi_xy, double* area_perim) {
+  if (!s || !cell_xy) return AVM_EINVAL;
+  spv_refresh(s, cell_xy, voronoi_xy);
+  if (area_perim) s->launches += launch_compute_forces(s->dev(), s->k, s->ap, nullptr, area_perim, s->stream);
+  AVM_CUDA(cudaPeekAtLastError());
+  return AVM_OK;
+}
+
+int avm_spv_forces(avm_sim* s, const double* cell_xy, double* force_xy, double* force_sets) {
+  if (!s || !cell_xy) return AVM_EINVAL;
+  spv_refresh(s, cell_xy, nullptr);
+  const Dev d = s->dev();
+  s->launches += launch_spv_forces(d, s->k, cell_xy, (double2*)d.pos_next, s->ap, force_xy, force_sets, s->stream);
+  AVM_CUDA(cudaPeekAtLastError());
+  return AVM_OK;
+}
+
+static int spv_read_counts(avm_sim* s, int64_t* n_failed, bool with_first) {
+  unsigned long long c[2];
+  AVM_CUDA(cudaMemcpyAsync(c, s->ctr->spv, sizeof(c), cudaMemcpyDeviceToHost, s->stream));
+  AVM_CUDA(cudaStreamSynchronize(s->stream));
+  n_failed[0] = (int64_t)c[0];
+  if (with_first) n_failed[1] = c[1] == ~0ull ? -1 : (int64_t)c[1];
+  return AVM_OK;
+}
+
+int avm_spv_test_triangulation(avm_sim* s, const double* cell_xy, int64_t* n_failed, int32_t* cell_flags) {
+  if (!s || !cell_xy || !n_failed) return AVM_EINVAL;
+  AVM_CUDA(cudaMemsetAsync(s->ctr->spv, 0, sizeof(unsigned long long), s->stream));
+  AVM_CUDA(cudaMemsetAsync(s->ctr->spv + 1, 0xff, sizeof(unsigned long long), s->stream));
+  if (cell_flags) AVM_CUDA(cudaMemsetAsync(cell_flags, 0, sizeof(int32_t) * (size_t)s->k.N, s->stream));
+  s->launches += launch_spv_test(s->dev(), s->k, cell_xy, s->ctr->spv, cell_flags, 0ull, s->stream);
+  return spv_read_counts(s, n_failed, false);
+}
+
+int avm_spv_step(avm_sim* s, double* cell_xy, int64_t n_steps, int64_t* n_failed, int32_t* cell_flags) {
+  if (!s || !cell_xy || !n_failed || n_steps < 0) return AVM_EINVAL;
+  AVM_CUDA(cudaMemsetAsync(s->ctr->spv, 0, sizeof(unsigned long long), s->stream));
+  AVM_CUDA(cudaMemsetAsync(s->ctr->spv + 1, 0xff, sizeof(unsigned long long), s->stream));
+  for (int64_t i = 0; i < n_steps; ++i) {
+    spv_refresh(s, cell_xy, nullptr);
+    const Dev d = s->dev();
+    s->launches += launch_spv_forces(d, s->k, cell_xy, (double2*)d.pos_next, s->ap, nullptr, nullptr, s->stream);   // :86-88
+    s->launches += launch_spv_move(d, s->k, cell_xy, s->ap, s->p.v0, s->step, s->stream);                            // Eq. 3, :92
+    ++s->step;
+    AVM_CUDA(cudaMemsetAsync(s->ctr->spv, 0, sizeof(unsigned long long), s->stream));
+    if (cell_flags) AVM_CUDA(cudaMemsetAsync(cell_flags, 0, sizeof(int32_t) * (size_t)s->k.N, s->stream));
+    s->launches += launch_spv_test(d, s->k, cell_xy, s->ctr->spv, cell_flags, (unsigned long long)i, s->stream);      // :94
+  }
+  spv_refresh(s, cell_xy, nullptr);      // the simulation's vertex positions and records describe the final cells
+  return spv_read_counts(s, n_failed, true);
+}
+
 int avm_resort(avm_sim* s) {
   if (!s) return AVM_EINVAL;
   do_sort(s);

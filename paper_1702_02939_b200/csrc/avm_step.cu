@@ -98,50 +98,6 @@ __device__ __forceinline__ void st_rec(CellRec* p, const CellRec& r) {
   asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(r.a), "d"(r.p), "d"(r.nx), "d"(r.ny) : "memory");
 }
 #endif
-// |d| >= L/2 decided conservatively on the high word with integer ALU ops (keeps the FP64 pipe
-// for arithmetic); the exact minimum image runs only where this fires.
-__device__ __forceinline__ unsigned may_wrap(double d, unsigned hi_half) { return (hi_word(d) & 0x7fffffffu) >= hi_half; }
-
-// ---------------------------------------------------------------------------------------------
-// rows a2 + a3: vertex forces (Eq. A2-A5) and displacement (Eq. 4, :56).
-// Slot convention (R12): in cell c_k = vc[v][k] the CCW neighbours of v are next = vn[v][k],
-// prev = vn[v][k+1], so no row search is needed.  With r_k = mi(h_{n_k} - h_v):
-//   dA_{c_k}/dh_v = 1/2 (r_k.y - r_{k+1}.y, r_{k+1}.x - r_k.x)        (A4, R3)
-//   dP_{c_k}/dh_v = -(rhat_k + rhat_{k+1})                             (A5, R2)
-//   F_v = -sum_k [ a_k dA + p_k dP ],  a = 2K_A(A-A0), p = 2K_P(P-P0)  (A2, A3)
-// ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ double2 vertex_force(const double2 h, const double2 q0, const double2 q1,
-                                                const double2 q2, const CellRec& c0, const CellRec& c1,
-                                                const CellRec& c2, const Consts& k) {
-  // Explicit rounding intrinsics throughout: the function is instantiated in several kernels
-  // (sweep, post-flip move, avm_compute_forces) and must give the same bits in each, so no
-  // contraction is left to the compiler.
-  double r0x = __dsub_rn(q0.x, h.x), r0y = __dsub_rn(q0.y, h.y), r1x = __dsub_rn(q1.x, h.x), r1y = __dsub_rn(q1.y, h.y),
-         r2x = __dsub_rn(q2.x, h.x), r2y = __dsub_rn(q2.y, h.y);
-  const unsigned hx = hi_word(k.hLx), hy = hi_word(k.hLy);
-  if (may_wrap(r0x, hx) | may_wrap(r1x, hx) | may_wrap(r2x, hx) | may_wrap(r0y, hy) | may_wrap(r1y, hy) | may_wrap(r2y, hy)) {
-    r0x = min_image(r0x, k.Lx, k.hLx); r1x = min_image(r1x, k.Lx, k.hLx); r2x = min_image(r2x, k.Lx, k.hLx);
-    r0y = min_image(r0y, k.Ly, k.hLy); r1y = min_image(r1y, k.Ly, k.hLy); r2y = min_image(r2y, k.Ly, k.hLy);
-  }
-  // + kTiny: a zero-length edge gives r * rsqrt = 0, i.e. contributes nothing (R15)
-  const double i0 = rsqrt_pos(__fma_rn(r0x, r0x, __fma_rn(r0y, r0y, kTiny)));
-  const double i1 = rsqrt_pos(__fma_rn(r1x, r1x, __fma_rn(r1y, r1y, kTiny)));
-  const double i2 = rsqrt_pos(__fma_rn(r2x, r2x, __fma_rn(r2y, r2y, kTiny)));
-  const double u0x = __dmul_rn(r0x, i0), u0y = __dmul_rn(r0y, i0), u1x = __dmul_rn(r1x, i1), u1y = __dmul_rn(r1y, i1),
-               u2x = __dmul_rn(r2x, i2), u2y = __dmul_rn(r2y, i2);
-  // cell k uses (next, prev) = (r_k, r_{k+1})
-  double sx = __dmul_rn(c0.a, __dsub_rn(r0y, r1y));
-  sx = __fma_rn(c1.a, __dsub_rn(r1y, r2y), sx);
-  sx = __fma_rn(c2.a, __dsub_rn(r2y, r0y), sx);
-  double sy = __dmul_rn(c0.a, __dsub_rn(r1x, r0x));
-  sy = __fma_rn(c1.a, __dsub_rn(r2x, r1x), sy);
-  sy = __fma_rn(c2.a, __dsub_rn(r0x, r2x), sy);
-  double fx = __dmul_rn(-0.5, sx), fy = __dmul_rn(-0.5, sy);
-  fx = __fma_rn(c0.p, __dadd_rn(u0x, u1x), fx); fx = __fma_rn(c1.p, __dadd_rn(u1x, u2x), fx); fx = __fma_rn(c2.p, __dadd_rn(u2x, u0x), fx);
-  fy = __fma_rn(c0.p, __dadd_rn(u0y, u1y), fy); fy = __fma_rn(c1.p, __dadd_rn(u1y, u2y), fy); fy = __fma_rn(c2.p, __dadd_rn(u2y, u0y), fy);
-  return make_double2(fx, fy);
-}
-
 struct VertexIn { double2 h; int n0, n1, n2, c0, c1, c2; };
 __device__ __forceinline__ VertexIn load_vertex(const Dev& d, const Consts& k, int v) {
   VertexIn in;
