@@ -847,7 +847,9 @@ __device__ __forceinline__ void row_pad(const int (&w)[kR], int (&r)[kR], const 
 }
 template <int kR>
 __device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Consts& k, const Cand* __restrict__ list,
-                                                       const unsigned base, const unsigned n, const int lane_in) {
+                                                       const unsigned base, const unsigned n, const int lane_in,
+                                                       const int4* __restrict__ pre = nullptr) {
+  // pre (optional): the 64 bytes of this lane's candidate, fetched by the caller before the list length was known
   const int lane = lane_in & 31;
 #ifdef AVM_TRACE
   const bool trq = (lane_in & 0x100) != 0;
@@ -866,7 +868,9 @@ __device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Const
   if (trq && blockIdx.x == 0 && threadIdx.x == 0) d.ctr->tr2[7] = tqe;
 #endif
   AVM_TR_W0(0, 0);
-  if (have) {
+  if (pre) {
+    if (have) { ca = pre[0]; cb = pre[1]; cc = pre[2]; cd = pre[3]; }
+  } else if (have) {
     const int4* __restrict__ src = reinterpret_cast<const int4*>(list + i);
     ca = __ldcg(src); cb = __ldcg(src + 1); cc = __ldcg(src + 2); cd = __ldcg(src + 3);
   }
@@ -1011,10 +1015,20 @@ __global__ void __launch_bounds__(kT1Block)
 t1_flip_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, const unsigned parity, const bool count_stats) {
   pdl_launch_dependents();
   pdl_wait();
-  const unsigned int n_cand = min(d.ctr->n_cand[parity], list_cap(k, parity));
   const Cand* __restrict__ list = list_base(d, k, parity);
   const int lane = threadIdx.x & 31;
   const unsigned gwarp = (blockIdx.x * kT1Block + threadIdx.x) >> 5, nwarps = (gridDim.x * kT1Block) >> 5;
+  // the first batch of candidate records is fetched while the list length is still in flight (one round trip
+  // less in a kernel that is a chain of round trips); entries beyond the length are ignored
+  int4 pre[4] = {make_int4(0, 0, 0, 0), make_int4(0, 0, 0, 0), make_int4(0, 0, 0, 0), make_int4(0, 0, 0, 0)};
+  {
+    const unsigned i0 = gwarp * 8u + (unsigned)(lane >> 2);
+    if (i0 < list_cap(k, parity)) {
+      const int4* __restrict__ src = reinterpret_cast<const int4*>(list + i0);
+      pre[0] = __ldcg(src); pre[1] = __ldcg(src + 1); pre[2] = __ldcg(src + 2); pre[3] = __ldcg(src + 3);
+    }
+  }
+  const unsigned int n_cand = min(__ldcg(&d.ctr->n_cand[parity]), list_cap(k, parity));
   if (count_stats && gwarp == 0 && lane == 0 && n_cand) atomicAdd((unsigned long long*)&d.ctr->t1_candidates, (unsigned long long)n_cand);
   if (count_stats && parity < 2u && gwarp == 0 && lane == 0) report_t1_load(d, n_cand);     // the step's list: report the T1 load
   unsigned int flips = 0, seen = 0;
@@ -1022,7 +1036,8 @@ t1_flip_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, 
   // constant bank; the row stays in registers): the kernel is a chain of dependent round trips and
   // every reload or local-memory access in it would queue behind the outstanding gathers
   for (unsigned int i = gwarp * 8u; i < n_cand; i += nwarps * 8u) {
-    flips += k.S <= 16 ? t1_flip_quads_impl<16>(d, k, list, i, n_cand, lane) : t1_flip_quads(d, k, list, i, n_cand, lane);
+    flips += k.S <= 16 ? t1_flip_quads_impl<16>(d, k, list, i, n_cand, lane, i == gwarp * 8u ? pre : nullptr)
+                       : t1_flip_quads(d, k, list, i, n_cand, lane);
     seen += min(8u, n_cand - i);
   }
   if (count_stats && lane == 0) {
