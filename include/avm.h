@@ -67,8 +67,9 @@ enum {
    * FUSED: two launches per step, the T1 flips of a step run inside the next force/move launch.
    * UNFUSED: three launches per step, a stand-alone T1 kernel.  PERSISTENT: one cooperative launch
    * per avm_step call (per stretch between re-sorts) advances all its steps, with grid-wide barriers
-   * between the stages (launch-free stepping; the default for systems of at most 512 vertices, which
-   * run as one CTA).  All schedules give the same bits (tests); at most one flag may be given. */
+   * between the stages (launch-free stepping; the default for systems of at most 8192 vertices: one
+   * CTA up to 512 vertices, one thread-block cluster with the hardware cluster barrier beyond).  All
+   * schedules give the same bits (tests); at most one flag may be given. */
   AVM_FLAG_SCHEDULE_FUSED = 4,
   AVM_FLAG_SCHEDULE_UNFUSED = 8,
   AVM_FLAG_SCHEDULE_PERSISTENT = 16,

@@ -365,12 +365,14 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   // bit-identical to the other schedules.  Measured: a system that fits one CTA steps in
   // 2.8 us instead of 4.8 (barriers are __syncthreads); with several CTAs a step is a chain of ~8 dependent L2
   // round trips either way (10.3 vs 9.8 us at configs[1], 22.3 vs 20.1 at configs[2]), so the default uses it
-  // only for systems of at most 512 vertices; AVM_FLAG_SCHEDULE_PERSISTENT selects it for any size.
+  // only for systems of at most 8192 vertices: one CTA up to 512 vertices, one thread-block CLUSTER of up to 16 CTAs
+  // with the hardware cluster barrier beyond (7.7 vs 8.1 us at configs[1]); AVM_FLAG_SCHEDULE_PERSISTENT selects it for
+  // any size (a cooperative grid with an arrival-counter barrier above 8192 vertices).
   s->persistent_grid = 0;
   {
     const bool forced = (params->flags & AVM_FLAG_SCHEDULE_PERSISTENT) != 0;
     const bool other = (params->flags & (AVM_FLAG_SCHEDULE_FUSED | AVM_FLAG_SCHEDULE_UNFUSED)) != 0;
-    if (s->t1_passes == 1 && !other && (forced || V <= 512)) s->persistent_grid = persistent_grid(V, false);
+    if (s->t1_passes == 1 && !other && (forced || V <= 8192)) s->persistent_grid = persistent_grid(V, false);
   }
   s->h_feedback = nullptr;
   s->d_feedback = &s->ctr->feedback_sink;
