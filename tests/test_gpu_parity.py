@@ -340,6 +340,22 @@ def test_full_size_configs_against_oracle(B, k, steps):
     L2 = t.Lx * t.Ly
     apg = g.compute_forces()[1].cpu().numpy()
     assert abs(apg[:, 0].sum() - L2) <= 1e-12 * L2
+    # candidate and winner sets of the state both sides have reached, as sets of (tag_min, tag_max); the oracle's
+    # state is loaded into a fresh simulation so that both decide from identical positions
+    tt = w.Tiling(t.Lx, t.Ly, t.S, so["pos"], so["cell_vertex_num"], so["cell_vertices"], so["vertex_neighbors"],
+                  so["vertex_cell_neighbors"], so["theta"])
+    g.close()
+    g2 = B.from_tiling(tt, **dict(p, step0=steps))
+    cand, win = g2.debug_t1()
+    co, wo = o.debug_t1()
+    cg, wg = {tuple(x) for x in cand.tolist()}, {tuple(x) for x in win.tolist()}
+    cs, ws = {tuple(x) for x in co.tolist()}, {tuple(x) for x in wo.tolist()}
+    fuzzy = near_threshold(so, cg ^ cs, t.Lx, t.Ly, p["l_c"])
+    assert (cg ^ cs) <= fuzzy
+    assert len(cs) > 1000
+    if not fuzzy:
+        assert wg == ws
+    g2.close()
     _TILINGS.pop(k, None)
 
 
