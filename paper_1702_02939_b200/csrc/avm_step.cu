@@ -34,7 +34,7 @@ namespace cg = cooperative_groups;
 #endif
 static constexpr int kVertexBlock = AVM_VERTEX_BLOCK;
 #ifndef AVM_CELL_BLOCK
-#define AVM_CELL_BLOCK 128
+#define AVM_CELL_BLOCK 64
 #endif
 static constexpr int kCellBlock = AVM_CELL_BLOCK;
 static constexpr int kT1Block = 128;
@@ -49,7 +49,7 @@ static constexpr unsigned kFull = 0xffffffffu;
 #define AVM_PDL 1          // chain the step's kernels with programmatic dependent launch
 #endif
 #ifndef AVM_CU_MINB
-#define AVM_CU_MINB 8      // cell pass: resident CTAs per SM asked of the compiler (64 registers; measured best of 7..11)
+#define AVM_CU_MINB 16     // cell pass: resident CTAs per SM asked of the compiler (64 registers; CTAs of 64 threads x 16 per SM: a CTA that holds a T1-marking thread keeps fewer idle warps resident; measured against 128 x 8: -0.3 us steady, -0.8 us in the burst, -2 us at N = 4M)
 #endif
 #ifndef AVM_FM_MINB
 #define AVM_FM_MINB 3      // force_move: minimum resident CTAs per SM asked of the compiler
