@@ -38,7 +38,10 @@ static constexpr int kVertexBlock = AVM_VERTEX_BLOCK;
 #endif
 static constexpr int kCellBlock = AVM_CELL_BLOCK;
 static constexpr int kT1Block = 128;
-static constexpr int kT1Grid = 148 * 2;
+#ifndef AVM_T1_GRID
+#define AVM_T1_GRID (148 * 3)      // CTAs of the T1 kernels (166 registers: three CTAs of 128 per SM; measured against 148 x 2: -0.5 us/step in the burst and at configs[2])
+#endif
+static constexpr int kT1Grid = AVM_T1_GRID;
 static constexpr unsigned kFull = 0xffffffffu;
 
 // tuning knobs (compile-time; the defaults are the measured best, profiles/)
