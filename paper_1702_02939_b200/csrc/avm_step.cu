@@ -150,6 +150,18 @@ __device__ __forceinline__ void move_vertex(const Dev& d, const Consts& k, int v
 
 // the same vertex update with every input read from L2 (after another warp of this launch
 // rewrote the neighbourhood: L1 may hold stale lines)
+// (one-CTA persistent kernel: plain cached loads, see cu_stream)
+__device__ __noinline__ void move_vertex_plain(const Dev& d, const Consts& k, int v) {
+  const double2 h = pos_ld(d.pos + v, k);
+  double2 q[3];
+  CellRec c[3];
+#pragma unroll
+  for (int s = 0; s < 3; ++s) {
+    q[s] = pos_ld(d.pos + d.vn[s * k.Vs + v], k);
+    c[s] = rec_ld_plain(d.rec + d.vc[s * k.Vs + v]);
+  }
+  move_vertex(d, k, v, h, q[0], q[1], q[2], c[0], c[1], c[2]);
+}
 __device__ __noinline__ void move_vertex_coherent(const Dev& d, const Consts& k, int v) {
   const double2 h = pos_ldcg(d.pos + v, k);
   double2 q[3];
@@ -572,8 +584,12 @@ __device__ __noinline__ void t1_report_cell(const Dev& d, const Consts& k, int c
 // kCoh: every load of data another CTA may have written earlier in the same launch goes through
 // the coherent path (the persistent multi-step kernel); false = the per-step kernel, where the
 // streams are read with cache hints and the gathers through the non-coherent path.
-template <bool kCoh, typename T> __device__ __forceinline__ T cu_stream(const T* p) { return kCoh ? __ldcg(p) : ld_stream(p); }
-template <bool kCoh> __device__ __forceinline__ double2 cu_pos(const pos_t* p, const Consts& k) { return kCoh ? pos_ldcg(p, k) : pos_ldg(p, k); }
+// kCoh = 2 (the persistent kernel as ONE CTA): everything was written by this very SM, whose L1 is write-through
+// and coherent with its own stores, so plain cached loads are safe and a round trip costs an L1 hit instead of L2.
+template <int kCoh, typename T> __device__ __forceinline__ T cu_stream(const T* p) { return kCoh == 1 ? __ldcg(p) : kCoh == 2 ? *p : ld_stream(p); }
+template <int kCoh> __device__ __forceinline__ double2 cu_pos(const pos_t* p, const Consts& k) {
+  return kCoh == 1 ? pos_ldcg(p, k) : kCoh == 2 ? pos_ld(p, k) : pos_ldg(p, k);
+}
 // Observables (NEXT-2; slots documented at observables_partial_kernel below).  kObs: the pass also reduces
 // them over the moved tiling it is computing anyway (avm_step_observe): per-thread values, a fixed
 // tree over the CTA in shared memory, one partial per CTA and slot; observables_final_kernel finishes.
@@ -581,7 +597,7 @@ static constexpr int kObs = 9;
 __device__ __forceinline__ double obs_combine(int slot, double a, double b) {
   return slot == 6 ? fmin(a, b) : slot == 7 ? fmax(a, b) : a + b;
 }
-template <bool kStep, bool kPerCell, bool kCoh, bool kObserve = false>
+template <bool kStep, bool kPerCell, int kCoh, bool kObserve = false>
 __device__ __forceinline__ void cell_update_body(const Dev& d, const Consts& k, const unsigned long long step, const unsigned parity,
                                                  const int gid, double* __restrict__ obs_partial = nullptr) {
   if (kStep && gid == 0) { d.ctr->flip_done = 0; d.ctr->next_cand = 0; }   // the previous list is long done
@@ -656,7 +672,7 @@ __device__ __forceinline__ void cell_update_body(const Dev& d, const Consts& k, 
   if (n > 8) {
     for (int q = 2; 4 * q < n; ++q) {
       const int j0 = 4 * q;
-      const int4 qq = kCoh ? __ldcg(d.cv + (size_t)q * k.N + c) : d.cv[(size_t)q * k.N + c];
+      const int4 qq = kCoh == 1 ? __ldcg(d.cv + (size_t)q * k.N + c) : d.cv[(size_t)q * k.N + c];
       const int ee[4] = {qq.x, qq.y, qq.z, qq.w};
       double2 hh[4];
 #pragma unroll
@@ -726,7 +742,7 @@ cell_update_observe_kernel(const __grid_constant__ Dev d, const __grid_constant_
                            const unsigned parity, double* __restrict__ obs_partial) {
   pdl_launch_dependents();
   pdl_wait();
-  cell_update_body<true, kPerCell, false, true>(d, k, step, parity, blockIdx.x * kCellBlock + threadIdx.x, obs_partial);
+  cell_update_body<true, kPerCell, 0, true>(d, k, step, parity, blockIdx.x * kCellBlock + threadIdx.x, obs_partial);
 }
 template <bool kStep, bool kPerCell>
 __global__ void __launch_bounds__(kCellBlock, AVM_CU_MINB)
@@ -734,7 +750,7 @@ cell_update_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts
                    const unsigned parity) {
   pdl_launch_dependents();
   pdl_wait();
-  cell_update_body<kStep, kPerCell, false>(d, k, step, parity, blockIdx.x * kCellBlock + threadIdx.x);
+  cell_update_body<kStep, kPerCell, 0>(d, k, step, parity, blockIdx.x * kCellBlock + threadIdx.x);
 }
 
 // Detection alone (test hooks avm_t1_pass / avm_debug_t1): thread per vertex, edge owned by the
@@ -884,7 +900,7 @@ __device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Const
   const int sx1 = cc.z & 3, sx2 = (cc.z >> 2) & 3;
   const int x1 = cd.x, y1 = cd.y, x2 = cd.z, y2 = cd.w;
   const int cell = t == 0 ? cL : t == 1 ? cR : t == 2 ? cE1 : cE2;     // 0 for idle groups: a valid index
-  const unsigned long long mk = d.minkey[cell];
+  const unsigned long long mk = __ldcg(d.minkey + cell);      // written by L2 atomics: never from L1
   const int nrow = (cc.w >> (8 * t)) & 0xff;            // as counted by the marking thread (a winner's cells are its own)
   const int need = t < 2 ? nrow : nrow + 1;             // entries of the longer of the old and the new row
   const double2 h1 = pos_ld(d.pos + v1, k), h2 = pos_ld(d.pos + v2, k);
@@ -1084,7 +1100,7 @@ struct GridBarrier {
   }
 };
 static constexpr int kClusterBlock = 256;     // CTA size of the one-cluster grid (measured at configs[1]: 7.7 us/step; 512 threads: 8.4)
-template <bool kPerCell>
+template <bool kPerCell, bool kOneCta>
 __global__ void __launch_bounds__(kClusterBlock)
 persistent_steps_kernel(Dev d, const __grid_constant__ Consts k, const unsigned long long step0, const int n_steps, const int one_cluster) {
   GridBarrier grid = {&d.ctr->bar, 0u, one_cluster != 0};
@@ -1102,11 +1118,11 @@ persistent_steps_kernel(Dev d, const __grid_constant__ Consts k, const unsigned 
       const int4 q = __ldcg(reinterpret_cast<const int4*>(d.cand + i) + 1);
       d.minkey[q.x] = ~0ull; d.minkey[q.y] = ~0ull; d.minkey[q.z] = ~0ull; d.minkey[q.w] = ~0ull;
     }
-    for (int v = tid; v < k.V; v += stride) move_vertex_coherent(d, k, v);
+    for (int v = tid; v < k.V; v += stride) { if (kOneCta) move_vertex_plain(d, k, v); else move_vertex_coherent(d, k, v); }
     grid.sync();
     { pos_t* t = d.pos; d.pos = d.pos_next; d.pos_next = t; }
     // ---- rows a4 + a1 + a5 + a6 (marking half)
-    for (int gid = tid; gid < n_round; gid += stride) cell_update_body<true, kPerCell, true>(d, k, step, parity, gid);
+    for (int gid = tid; gid < n_round; gid += stride) cell_update_body<true, kPerCell, kOneCta ? 2 : 1>(d, k, step, parity, gid);
     grid.sync();
     // ---- rows a6 (deciding half) + a7
     const unsigned n_cand = min(__ldcg(&d.ctr->n_cand[parity]), (unsigned)k.cap_a);
@@ -1359,8 +1375,8 @@ int persistent_grid(int V, bool per_cell) {
   cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   if (!coop || sms <= 0) return 0;
-  if (per_cell) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, persistent_steps_kernel<true>, kVertexBlock, 0);
-  else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, persistent_steps_kernel<false>, kVertexBlock, 0);
+  if (per_cell) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, persistent_steps_kernel<true, false>, kVertexBlock, 0);
+  else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, persistent_steps_kernel<false, false>, kVertexBlock, 0);
   if (per_sm < 1) return 0;
   const int want = V <= 512 ? 1 : cdiv(V, kVertexBlock), cap = sms * per_sm;     // tiny systems: one CTA, barriers are __syncthreads
   // up to kClusterVertices vertices the grid is one cluster of at most 16 CTAs (hardware barrier instead of an
@@ -1377,7 +1393,8 @@ int launch_persistent_steps(const Dev& d, const Consts& k, unsigned long long st
   int ns = n_steps;
   int one_cluster = 0;
   void* args[] = {(void*)&dd, (void*)&kk, (void*)&step0, (void*)&ns, (void*)&one_cluster};
-  const void* fn = k.per_cell ? (const void*)persistent_steps_kernel<true> : (const void*)persistent_steps_kernel<false>;
+  const void* fn = grid == 1 ? (k.per_cell ? (const void*)persistent_steps_kernel<true, true> : (const void*)persistent_steps_kernel<false, true>)
+                             : (k.per_cell ? (const void*)persistent_steps_kernel<true, false> : (const void*)persistent_steps_kernel<false, false>);
   if (grid > 1 && grid <= kClusterMax && k.V <= kClusterVertices) {
     // the grid as one thread-block cluster: co-scheduled by construction, barriers in hardware
     one_cluster = 1;
