@@ -186,6 +186,25 @@ __device__ __forceinline__ void report_t1_load(const Dev& d, const unsigned n) {
   }
 }
 
+__device__ __noinline__ void move_two_coherent(const Dev& d, const Consts& k, int va, int vb) {
+  const double2 ha = pos_ldcg(d.pos + va, k), hb = pos_ldcg(d.pos + vb, k);
+  int na[3], nb[3], ca[3], cb[3];
+#pragma unroll
+  for (int s = 0; s < 3; ++s) {
+    na[s] = __ldcg(d.vn + s * k.Vs + va); nb[s] = __ldcg(d.vn + s * k.Vs + vb);
+    ca[s] = __ldcg(d.vc + s * k.Vs + va); cb[s] = __ldcg(d.vc + s * k.Vs + vb);
+  }
+  double2 qa[3], qb[3];
+  CellRec ra[3], rb[3];
+#pragma unroll
+  for (int s = 0; s < 3; ++s) {
+    qa[s] = pos_ldcg(d.pos + na[s], k); qb[s] = pos_ldcg(d.pos + nb[s], k);
+    ra[s] = rec_ldcg(d.rec + ca[s]); rb[s] = rec_ldcg(d.rec + cb[s]);
+  }
+  move_vertex(d, k, va, ha, qa[0], qa[1], qa[2], ra[0], ra[1], ra[2]);
+  move_vertex(d, k, vb, hb, qb[0], qb[1], qb[2], rb[0], rb[1], rb[2]);
+}
+
 __device__ __forceinline__ unsigned int ld_volatile(const unsigned int* p) {
   unsigned int x;
   asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(x) : "l"(p) : "memory");
@@ -1118,7 +1137,14 @@ persistent_steps_kernel(Dev d, const __grid_constant__ Consts k, const unsigned 
       const int4 q = __ldcg(reinterpret_cast<const int4*>(d.cand + i) + 1);
       d.minkey[q.x] = ~0ull; d.minkey[q.y] = ~0ull; d.minkey[q.z] = ~0ull; d.minkey[q.w] = ~0ull;
     }
-    for (int v = tid; v < k.V; v += stride) { if (kOneCta) move_vertex_plain(d, k, v); else move_vertex_coherent(d, k, v); }
+    if (kOneCta) {
+      for (int v = tid; v < k.V; v += stride) move_vertex_plain(d, k, v);
+    } else {
+      // two vertices per trip: both sets of loads are in flight together (a cluster takes 2 vertices per thread at 8192)
+      int v = tid;
+      for (; v + stride < k.V; v += 2 * stride) move_two_coherent(d, k, v, v + stride);
+      if (v < k.V) move_vertex_coherent(d, k, v);
+    }
     grid.sync();
     { pos_t* t = d.pos; d.pos = d.pos_next; d.pos_next = t; }
     // ---- rows a4 + a1 + a5 + a6 (marking half)
