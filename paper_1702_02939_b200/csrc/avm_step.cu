@@ -162,7 +162,12 @@ __device__ __noinline__ void move_vertex_plain(const Dev& d, const Consts& k, in
   }
   move_vertex(d, k, v, h, q[0], q[1], q[2], c[0], c[1], c[2]);
 }
-__device__ __noinline__ void move_vertex_coherent(const Dev& d, const Consts& k, int v) {
+// helpers of the fused launch: inlined (measured -0.2 us/step against calls; the flip itself stays a call there: inlined
+// into the 80-register kernel it costs the sweep 3.7 us)
+#ifndef AVM_FUSED_ATTR
+#define AVM_FUSED_ATTR __forceinline__
+#endif
+__device__ AVM_FUSED_ATTR void move_vertex_coherent(const Dev& d, const Consts& k, int v) {
   const double2 h = pos_ldcg(d.pos + v, k);
   double2 q[3];
   CellRec c[3];
@@ -213,6 +218,13 @@ __device__ __forceinline__ unsigned int ld_volatile(const unsigned int* p) {
 
 __device__ __noinline__ unsigned t1_flip_quads(const Dev& d, const Consts& k, const Cand* __restrict__ list, unsigned base,
                                                unsigned n, const int lane);
+template <int kR>
+__device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Consts& k, const Cand* __restrict__ list,
+                                                       const unsigned base, const unsigned n, const int lane_in,
+                                                       const int4* __restrict__ pre = nullptr);
+#ifndef AVM_FUSED_FLIP_INLINE
+#define AVM_FUSED_FLIP_INLINE 0
+#endif
 
 // The sweep of one thread over vertices first, first + step_v, ...  kSkipDirty: vertices flagged
 // in `dirty` (read-only for this whole launch) are left to the dirty pass below.
@@ -271,7 +283,7 @@ __device__ __forceinline__ void sweep(const Dev& d, const Consts& k, const unsig
 // step wrote it, the cell pass of this step clears it), so the sweep's decision to skip a vertex
 // never changes while flips are in flight.
 // first: a batch already claimed for this warp (by its CTA), or >= prev for none
-__device__ __noinline__ void flipper_flips(const Dev& d, const Consts& k, const unsigned prev, const int lane, const unsigned first) {
+__device__ AVM_FUSED_ATTR void flipper_flips(const Dev& d, const Consts& k, const unsigned prev, const int lane, const unsigned first) {
   unsigned mine = 0, flips = 0;
   unsigned i = first;
 #ifdef AVM_TRACE
@@ -300,7 +312,7 @@ __device__ __noinline__ void flipper_flips(const Dev& d, const Consts& k, const 
 #ifdef AVM_TRACE
     flips += t1_flip_quads(d, k, d.cand, i, prev, lane | 0x100);
 #else
-    flips += t1_flip_quads(d, k, d.cand, i, prev, lane);
+    flips += (AVM_FUSED_FLIP_INLINE && k.S <= 16) ? t1_flip_quads_impl<16>(d, k, d.cand, i, prev, lane) : t1_flip_quads(d, k, d.cand, i, prev, lane);
 #endif
 #ifdef AVM_TRACE
     if (w0) d.ctr->tr2[0] = gtime() + (flips & 0);
@@ -337,7 +349,7 @@ __device__ __noinline__ void flipper_flips(const Dev& d, const Consts& k, const 
 // Lanes = 4 cells x 8 row entries per pass (96 % of the cells need one pass); a vertex that sits
 // in several of the four rows is moved by the lowest lane holding it.  A vertex shared with
 // another candidate's cells is moved twice, with the same inputs and the same result.
-__device__ __noinline__ void mover_unit(const Dev& d, const Consts& k, const unsigned i, const int lane) {
+__device__ AVM_FUSED_ATTR void mover_unit(const Dev& d, const Consts& k, const unsigned i, const int lane) {
   const int t = lane >> 3, j8 = lane & 7;
   const int4 q = __ldcg(reinterpret_cast<const int4*>(d.cand + i) + 1);   // (cL, cR, cE1, cE2)
   const int cell = t == 0 ? q.x : t == 1 ? q.y : t == 2 ? q.z : q.w;
@@ -354,42 +366,6 @@ __device__ __noinline__ void mover_unit(const Dev& d, const Consts& k, const uns
     if (j < n && __ffs(same) - 1 == lane) move_vertex_coherent(d, k, u);
   }
   if (lane < 4) d.minkey[lane == 0 ? q.x : lane == 1 ? q.y : lane == 2 ? q.z : q.w] = ~0ull;
-}
-
-// Moves every flagged vertex of this warp's slice of the bitmap (many-candidate mode).  The set
-// bits of up to 32 words (1024 vertices) are compacted so that all 32 lanes work: an inclusive
-// scan of the population counts, then each lane finds the word and the bit of "its" vertex.
-__device__ __noinline__ void dirty_pass(const Dev& d, const Consts& k, const unsigned int* __restrict__ dirty,
-                                        const unsigned gwarp, const unsigned nwarps, const int lane) {
-  const unsigned per = ((unsigned)k.nw + nwarps - 1u) / nwarps;
-  const unsigned w0 = min(gwarp * per, (unsigned)k.nw), w1 = min(w0 + per, (unsigned)k.nw);
-  for (unsigned base = w0; base < w1; base += 32u) {
-    const unsigned word = base + lane < w1 ? __ldg(dirty + base + lane) : 0u;
-    if (!__any_sync(kFull, word != 0u)) continue;
-    int incl = __popc(word);
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const int y = __shfl_up_sync(kFull, incl, o);
-      if (lane >= o) incl += y;
-    }
-    const int total = __shfl_sync(kFull, incl, 31);
-    for (int k0 = 0; k0 < total; k0 += 32) {
-      const int idx = k0 + lane;
-      int j = 0;                                   // number of words whose inclusive count is <= idx
-#pragma unroll
-      for (int st = 16; st > 0; st >>= 1) {
-        const int probe = __shfl_sync(kFull, incl, j + st - 1);
-        if (probe <= idx) j += st;
-      }
-      j = min(j, 31);
-      const unsigned wj = __shfl_sync(kFull, word, j);
-      const int excl = __shfl_sync(kFull, incl, j) - __popc(wj);
-      if (idx < total) {
-        const int bit = (int)__fns(wj, 0u, idx - excl + 1);
-        move_vertex_coherent(d, k, (int)((base + (unsigned)j) * 32u) + bit);
-      }
-    }
-  }
 }
 
 // minimum keys of candidates [i0, i1) back to idle (row a6), thread per candidate
@@ -484,7 +460,9 @@ force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts 
 // pass of NEXT-1 (no statistics, but the sticky overflow bit is still raised);
 // kMarkSilent = the debug hook (no side effects beyond the list and the minimum keys).
 enum : int { kMarkSilent = 0, kMarkFirstPass = 1, kMarkRepeatedPass = 2 };
-__device__ __noinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va, int vb, unsigned parity, const int mode) {
+// (inlined everywhere: a call from the cell pass, even one that is never taken, costs that pass a stack frame, the
+// ABI's register partition and generic loads of the by-reference parameter structs: measured 2 us per step)
+__device__ __forceinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va, int vb, unsigned parity, const int mode) {
   const bool count_stats = mode == kMarkFirstPass;
   // The marking thread delays the end of the cell pass when it sits in the last wave, so its
   // loads are issued in two batches of independent loads instead of a chain of five.
@@ -575,7 +553,7 @@ __device__ __noinline__ void t1_mark_edge(const Dev& d, const Consts& k, int va,
 // being the closing edge) as possibly short.  Each edge is seen by its two cells in opposite
 // directions: it is reported from the cell that traverses it from the smaller to the larger
 // (current) vertex index.
-__device__ __noinline__ void t1_report_cell(const Dev& d, const Consts& k, int c, int n, unsigned smask, unsigned parity) {
+__device__ __forceinline__ void t1_report_cell(const Dev& d, const Consts& k, int c, int n, unsigned smask, unsigned parity) {
   while (smask) {
     const int j = __ffs(smask);     // edge (j-1) -> (j mod n)
     smask &= smask - 1u;
@@ -886,7 +864,7 @@ __device__ __forceinline__ void row_pad(const int (&w)[kR], int (&r)[kR], const 
 template <int kR>
 __device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Consts& k, const Cand* __restrict__ list,
                                                        const unsigned base, const unsigned n, const int lane_in,
-                                                       const int4* __restrict__ pre = nullptr) {
+                                                       const int4* __restrict__ pre) {
   // pre (optional): the 64 bytes of this lane's candidate, fetched by the caller before the list length was known
   const int lane = lane_in & 31;
 #ifdef AVM_TRACE
