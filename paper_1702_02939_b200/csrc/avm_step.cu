@@ -151,7 +151,11 @@ __device__ __forceinline__ void move_vertex(const Dev& d, const Consts& k, int v
 // the same vertex update with every input read from L2 (after another warp of this launch
 // rewrote the neighbourhood: L1 may hold stale lines)
 // (one-CTA persistent kernel: plain cached loads, see cu_stream)
-__device__ __noinline__ void move_vertex_plain(const Dev& d, const Consts& k, int v) {
+// (inlined into the persistent kernel: cfg0 2.24 -> 2.00 us/step, cfg1 7.5 -> 6.9)
+#ifndef AVM_PERS_ATTR
+#define AVM_PERS_ATTR __forceinline__
+#endif
+__device__ AVM_PERS_ATTR void move_vertex_plain(const Dev& d, const Consts& k, int v) {
   const double2 h = pos_ld(d.pos + v, k);
   double2 q[3];
   CellRec c[3];
@@ -191,7 +195,7 @@ __device__ __forceinline__ void report_t1_load(const Dev& d, const unsigned n) {
   }
 }
 
-__device__ __noinline__ void move_two_coherent(const Dev& d, const Consts& k, int va, int vb) {
+__device__ AVM_PERS_ATTR void move_two_coherent(const Dev& d, const Consts& k, int va, int vb) {
   const double2 ha = pos_ldcg(d.pos + va, k), hb = pos_ldcg(d.pos + vb, k);
   int na[3], nb[3], ca[3], cb[3];
 #pragma unroll
@@ -222,6 +226,9 @@ template <int kR>
 __device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Consts& k, const Cand* __restrict__ list,
                                                        const unsigned base, const unsigned n, const int lane_in,
                                                        const int4* __restrict__ pre = nullptr);
+#ifndef AVM_PERS_FLIP_INLINE
+#define AVM_PERS_FLIP_INLINE 1    // persistent kernel: the flip inlined too (cfg0 2.00 -> 1.95 us/step, cfg1 6.9 -> 6.7)
+#endif
 #ifndef AVM_FUSED_FLIP_INLINE
 #define AVM_FUSED_FLIP_INLINE 0
 #endif
@@ -1134,7 +1141,11 @@ persistent_steps_kernel(Dev d, const __grid_constant__ Consts k, const unsigned 
       if (tid == 0) atomicAdd((unsigned long long*)&d.ctr->t1_candidates, (unsigned long long)n_cand);
       unsigned flips = 0, seen = 0;
       for (unsigned i = gwarp * 8u; i < n_cand; i += nwarps * 8u) {
+#if AVM_PERS_FLIP_INLINE
+        flips += k.S <= 16 ? t1_flip_quads_impl<16>(d, k, d.cand, i, n_cand, lane) : t1_flip_quads(d, k, d.cand, i, n_cand, lane);
+#else
         flips += t1_flip_quads(d, k, d.cand, i, n_cand, lane);
+#endif
         seen += min(8u, n_cand - i);
       }
       if (lane == 0) {
