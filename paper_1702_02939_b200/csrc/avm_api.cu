@@ -361,13 +361,13 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   s->fused_ok = s->t1_passes == 1 && AVM_FUSED_T1 && (V >= (1 << 20) || V <= 2048 || s->fused_forced) &&
                 !(params->flags & AVM_FLAG_SCHEDULE_UNFUSED);
   k.flag_dirty = 0; k.clear_dirty = 0;
-  // Launch-free stepping: one cooperative persistent launch per avm_step call (or per stretch between re-sorts),
-  // bit-identical to the other schedules.  Measured: a system that fits one CTA steps in
-  // 2.8 us instead of 4.8 (barriers are __syncthreads); with several CTAs a step is a chain of ~8 dependent L2
-  // round trips either way (10.3 vs 9.8 us at configs[1], 22.3 vs 20.1 at configs[2]), so the default uses it
-  // only for systems of at most 8192 vertices: one CTA up to 512 vertices, one thread-block CLUSTER of up to 16 CTAs
-  // with the hardware cluster barrier beyond (7.7 vs 8.1 us at configs[1]); AVM_FLAG_SCHEDULE_PERSISTENT selects it for
-  // any size (a cooperative grid with an arrival-counter barrier above 8192 vertices).
+  // Launch-free stepping: ONE launch per avm_step call (or per stretch between re-sorts), bit-identical to the other
+  // schedules.  Default up to 8192 vertices: one CTA up to 512 vertices (barriers are
+  // __syncthreads, cached loads: 1.97 us/step at configs[0] against 4.8 with two launches per step), one thread-block
+  // CLUSTER of up to 16 CTAs with the hardware cluster barrier beyond (8.1 against 9.8 us at configs[1]).  Above that a
+  // step is a chain of ~8 dependent L2 round trips plus barriers either way and one launch per kernel is faster
+  // (15.0 against 20.6 us at configs[2]); AVM_FLAG_SCHEDULE_PERSISTENT still selects it for any size (a cooperative
+  // grid with an arrival-counter barrier).
   s->persistent_grid = 0;
   {
     const bool forced = (params->flags & AVM_FLAG_SCHEDULE_PERSISTENT) != 0;
