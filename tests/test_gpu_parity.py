@@ -829,3 +829,31 @@ def test_observing_geometry_pass_matches_the_oracle(B, k, steps, sort_every):
     # observing costs nothing afterwards: the between-steps observables agree too
     a, b = g.observe(), o.observables()
     assert abs(a["energy"] - b["energy"]) <= 1e-9 * abs(b["energy"]) and abs(a["msd"] - b["msd"]) <= 1e-9 * max(1.0, b["msd"])
+
+
+@pytest.mark.parametrize("N,L", [(300, 17.3), (1500, 38.7), (4000, 63.2)])
+def test_cluster_persistent_default_at_ragged_sizes(B, N, L):
+    """Systems of 513..8192 vertices step by default inside one thread-block cluster (hardware cluster barrier,
+    two vertices per thread and trip).  Sizes that fill the last CTA only partly, per-cell parameters, a re-sort
+    period that cuts the call into stretches: the default must equal one launch per kernel bit for bit and follow
+    the oracle."""
+    t = w.voronoi_tiling(N, L, 31 + N)
+    p = dict(KA=1.0, KP=1.0, A0=1.0, P0=3.9, v0=0.4, Dr=1.0, mu=1.0, dt=0.01, l_c=0.08, seed=5, sort_every=9)
+    rng = np.random.default_rng(N)
+    A0 = 1.0 + 0.2 * rng.standard_normal(N)
+    P0 = 3.9 + 0.1 * rng.standard_normal(N)
+    a = B.from_tiling(t, **p)                       # default: persistent, one cluster
+    c = B.from_tiling(t, schedule="unfused", **p)
+    o = oracle.from_tiling(t, **{k: v for k, v in p.items() if k != "sort_every"})
+    for sim in (a, c, o):
+        sim.set_cell_targets(A0, P0)
+    for n in (1, 17, 40):
+        a.step(n)
+        c.step(n)
+        o.step(n)
+    sa, sc = to_np(a.get_state()), to_np(c.get_state())
+    assert sa["stats"]["kernel_launches"] < sc["stats"]["kernel_launches"] - 100
+    for key in ("pos", "theta", "cell_vertices", "vertex_neighbors", "vertex_cell_neighbors", "cell_vertex_num"):
+        assert np.array_equal(sa[key], sc[key]), key
+    assert sa["stats"]["t1_flips"] == sc["stats"]["t1_flips"] > 20
+    assert_states_match(sa, o.get_state(), t.Lx, t.Ly)
