@@ -119,8 +119,19 @@ lib = _load()
 _LIBS = {"f64": lib}
 
 
+_VARIANTS = {}
+
+
+def register_library(name: str, path: str) -> None:
+    """an alternative build of the same sources and ABI under a name of its own (test builds with timing knobs);
+    `from_tiling(..., precision=name)` then runs on it"""
+    _VARIANTS[name] = _load(path)
+
+
 def library(precision: str = "f64") -> ctypes.CDLL:
     """the C-ABI library for a storage precision: "f64" (default) or "mixed" (libavm_b200_mixed.so, NEXT-3)"""
+    if precision in _VARIANTS:
+        return _VARIANTS[precision]
     if precision not in _LIBS:
         if precision != "mixed":
             raise AvmError(f"unknown precision {precision!r}")

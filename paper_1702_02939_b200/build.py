@@ -45,5 +45,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_variant(path: str, defines) -> str:
+    """the fp64 library with extra -D flags at `path` (test builds: tests/test_gpu_skew.py)"""
+    subprocess.check_call([NVCC] + NVCC_FLAGS + [f"-D{d}" for d in defines] + ["-o", path] + sources())
+    return path
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

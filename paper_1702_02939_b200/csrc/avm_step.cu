@@ -57,6 +57,9 @@ static constexpr unsigned kFull = 0xffffffffu;
 #ifndef AVM_FM_MINB
 #define AVM_FM_MINB 3      // force_move: minimum resident CTAs per SM asked of the compiler
 #endif
+#ifndef AVM_TEST_SKEW
+#define AVM_TEST_SKEW 0     // test builds: hold back the sweepers (1) or the flippers (2) of the fused launch
+#endif
 #ifndef AVM_FM_REGPF
 #define AVM_FM_REGPF 0     // force_move: keep the next vertex's streaming loads in registers (measured: the L2 prefetch does better)
 #endif
@@ -418,6 +421,16 @@ force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts 
       const unsigned wib = threadIdx.x >> 5, nb = gridDim.x;
       const unsigned fid = wib * nb + blockIdx.x;                          // flipper id of this warp, if < prev
       const unsigned full = prev / nb, rest = prev % nb;                   // warps 0..full-1 of every CTA, warp `full` of `rest` CTAs
+#if AVM_TEST_SKEW
+      // Test builds only (tests/test_gpu_skew.py): one side of the launch is held back for tens of microseconds so
+      // that the other finishes first.  1: the sweepers start after the flips and the movers are long done;
+      // 2: the flippers start after the sweep is long over.  Results must not depend on it.
+      if ((AVM_TEST_SKEW == 1) != (fid < prev)) {
+        unsigned long long t0, t1;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+        do { __nanosleep(1000); asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1)); } while (t1 - t0 < (AVM_TEST_SKEW == 1 ? 40000ull : 80000ull));
+      }
+#endif
       if (fid < prev) {
         if (fid * 8u < prev) flipper_flips(d, k, prev, lane, prev);        // the first prev/8 of them claim the flips
         AVM_TR_MAX(1);
