@@ -95,7 +95,7 @@ class ClockSampler:
         except Exception:
             pass
 
-    def start(self, period_s: float = 0.001):
+    def start(self, period_s: float = 0.0005):
         """sample from a background thread while the caller enqueues and waits (ctypes releases the GIL)"""
         import threading
         self._stop = threading.Event()
@@ -411,6 +411,9 @@ def main():
                    "blocked": st1["t1_blocked"] - st0["t1_blocked"], "steps": steps_timed,
                    "error_word": state_after["error"]},
             "clocks": sampler.summary(),
+            # an NVML sample takes about a millisecond, so a 1.5 ms region (--steps 20) holds one; the config's nominal
+            # run in the same process (whole_run below) is sampled the same way and holds hundreds
+            "clocks_nominal_run": whole_run["clocks"] if whole_run else None,
             "roofline": roofline,
             "whole_run": whole_run,
             "second_half": second_half,
