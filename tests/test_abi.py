@@ -43,6 +43,26 @@ def test_params_struct_matches_header(binding, repo_root):
     assert snames == [f[0] for f in binding.AvmStats._fields_]
 
 
+def test_observables_struct_matches_header(binding, repo_root):
+    header = open(os.path.join(repo_root, "include", "avm.h")).read()
+    body = re.search(r"typedef struct avm_observables \{(.*?)\} avm_observables;", header, re.S).group(1)
+    names = []
+    for line in body.splitlines():
+        line = line.split("/*")[0].strip().rstrip(";")
+        if not line:
+            continue
+        typ, rest = line.split(None, 1)
+        names += [(typ, n.strip()) for n in rest.split(",")]
+    want = [("double" if f[1] is ctypes.c_double else "int64_t", f[0]) for f in binding.AvmObservables._fields_]
+    assert names == want
+    # the mixed-precision library is the same ABI
+    mixed = ctypes.CDLL(binding.LIB_MIXED_PATH)
+    for name in binding.ABI_SYMBOLS:
+        assert hasattr(mixed, name), f"{name} not exported by the mixed library"
+    mixed.avm_precision.restype = ctypes.c_char_p
+    assert mixed.avm_precision() == b"mixed"
+
+
 def test_argument_validation_needs_no_gpu(binding):
     b = binding
     good = b.make_params(64, 16, Lx=8.0, Ly=8.0)
