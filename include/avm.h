@@ -104,7 +104,8 @@ enum {
   AVM_EWORKSPACE = -2,    /* workspace too small or misaligned                                   */
   AVM_EINCONSISTENT = -3, /* the topology lists contradict each other or a row is out of range   */
   AVM_ECUDA = -4,         /* a CUDA call failed; avm_last_cuda_error() has the text              */
-  AVM_ENOMEM = -5
+  AVM_ENOMEM = -5,
+  AVM_ETOOLARGE = -6      /* avm_forces_static: more cells than AVM_FORCES_STATIC_MAX_CELLS             */
 };
 
 /* Bytes of device workspace avm_create needs for these parameters (0 on invalid parameters). */
@@ -143,6 +144,45 @@ int avm_step_profile(avm_sim* sim, int64_t n_steps, double* ms_per_kernel);
  * device variant; the host variant returns after the copies have completed. */
 int avm_compute_forces(avm_sim* sim, double* force_xy, double* area_perim);
 int avm_compute_forces_host(avm_sim* sim, double* force_xy, double* area_perim);
+
+/* Geometry and forces of a tiling WITHOUT an avm_sim, a workspace or any allocation — for callers that
+ * are not allowed to allocate: code running inside someone else's memory plan (a plugin or a callback of
+ * a host application that hands out fixed device buffers and forbids cudaMalloc, which would also
+ * synchronise the whole device under the host's feet), real-time loops that must not take the
+ * allocator's locks, and processes whose device memory is fully reserved by another pool.  Such a caller
+ * cannot provide avm_create's workspace either if nobody gave it one.  Same result as avm_create +
+ * avm_compute_forces with the uniform A0, P0, KA, KP of `params` (App. A.1, Eq. A1-A5), to
+ * the last bit in the f64 library.
+ *
+ *   params   : n_cells, n_vertices, max_cell_vertices, Lx, Ly, KA, KP, A0, P0 and device are read; the rest is
+ *              ignored.  The call makes params->device the current device, as avm_create does.
+ *   inputs   : DEVICE pointers, the user-order arrays of the table above (pos_xy, cell_vertex_num,
+ *              cell_vertices, vertex_neighbors, vertex_cell_neighbors), read only, not validated.
+ *   outputs  : DEVICE pointers owned by the caller: force_xy [V][2] = -dE/dh_v, area_perim [N][2] = (A_c, P_c);
+ *              either may be NULL, not both.
+ *   stream   : the two kernels are enqueued on cuda_stream; the call does not synchronise.
+ *
+ * The per-cell (A, P) pairs travel from the geometry kernel to the force kernel through a fixed array
+ * built into the library's device image: 16 bytes x AVM_FORCES_STATIC_MAX_CELLS = 1 MiB of device
+ * memory on every GPU that loads the library, held until the process exits.  Consequences:
+ *   - n_cells > AVM_FORCES_STATIC_MAX_CELLS is refused with AVM_ETOOLARGE (nothing is enqueued); larger
+ *     tilings need avm_compute_forces and a workspace.
+ *   - The first call on each device looks the array's device address up (one cudaGetSymbolAddress, which
+ *     loads the library's kernels on that device if nothing has yet); make that first call before any
+ *     stream capture begins.  Later calls only enqueue the two kernels.
+ *   - No call here uses cudaMalloc, cudaFree, cudaHostAlloc or a library routine that allocates.
+ *   - All calls on a device share the one array, and it keeps what the last call wrote.  Nothing in it
+ *     needs clearing: every entry the force kernel reads was written by the geometry kernel of the same
+ *     call.  But two calls whose kernels can run at the same time on one GPU (different streams, or
+ *     different host threads on different streams) overwrite each other's (A, P) and give wrong forces:
+ *     keep calls on one stream, or order them yourself.
+ * Errors: AVM_EINVAL (NULL input, both outputs NULL, V != 2N, bad stride or box, device outside 0..63),
+ * AVM_ETOOLARGE, AVM_ECUDA. */
+#define AVM_FORCES_STATIC_MAX_CELLS 65536
+int avm_forces_static(const avm_params* params, const double* pos_xy, const int32_t* cell_vertex_num,
+                      const int32_t* cell_vertices, const int32_t* vertex_neighbors,
+                      const int32_t* vertex_cell_neighbors, double* force_xy, double* area_perim,
+                      void* cuda_stream);
 
 /* Total energy of the current state, Eq. 1 / A1, summed on the device in a
  * fixed order (deterministic).  energy is a HOST pointer; synchronises the stream. */

@@ -23,6 +23,7 @@ LIB_MIXED_PATH = os.path.join(_HERE, "libavm_b200_mixed.so")
 # every symbol include/avm.h declares (tests check that the library exports all of them)
 ABI_SYMBOLS = [
     "avm_workspace_bytes", "avm_create", "avm_create_host", "avm_step", "avm_step_profile", "avm_compute_forces",
+    "avm_forces_static",
     "avm_compute_forces_host", "avm_energy", "avm_observe", "avm_step_observe", "avm_spv_geometry", "avm_spv_forces", "avm_spv_step", "avm_spv_test_triangulation", "avm_set_cell_targets", "avm_set_cell_moduli", "avm_msd_reset", "avm_get_state", "avm_get_state_host", "avm_debug_t1",
     "avm_t1_pass", "avm_set_positions", "avm_resort", "avm_philox_words", "avm_hilbert_index",
     "avm_hilbert_index_host", "avm_destroy", "avm_strerror", "avm_last_cuda_error", "avm_precision",
@@ -86,6 +87,7 @@ def _load(path: str = LIB_PATH) -> ctypes.CDLL:
     lib.avm_step_profile.argtypes = [p, i64, p]
     lib.avm_compute_forces.argtypes = [p, p, p]
     lib.avm_compute_forces_host.argtypes = [p, p, p]
+    lib.avm_forces_static.argtypes = [PP, p, p, p, p, p, p, p, p]
     lib.avm_energy.argtypes = [p, ctypes.POINTER(ctypes.c_double)]
     lib.avm_observe.argtypes = [p, ctypes.POINTER(AvmObservables)]
     lib.avm_step_observe.argtypes = [p, i64, ctypes.POINTER(AvmObservables)]
@@ -166,6 +168,23 @@ def make_params(N: int, S: int, *, Lx, Ly, KA=1.0, KP=1.0, A0=1.0, P0=3.8, v0=0.
 
 def _dptr(t) -> Optional[int]:
     return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+AVM_FORCES_STATIC_MAX_CELLS = 65536
+
+
+def forces_static(params: AvmParams, pos, cell_vertex_num, cell_vertices, vertex_neighbors, vertex_cell_neighbors,
+                  force_out, area_perim_out, precision: str = "f64") -> None:
+    """``avm_forces_static``: geometry and forces of a tiling given as CUDA tensors in user order, written into the
+    caller's ``force_out`` [V,2] / ``area_perim_out`` [N,2] (either may be None), on the current stream.  Needs no
+    AvmSim and no workspace, and the library allocates nothing: the per-cell (A, P) pairs pass through a 1 MiB array
+    built into the library.  Raises AvmError (code -6) beyond AVM_FORCES_STATIC_MAX_CELLS cells.  Calls that can
+    overlap on the GPU share that array and must be ordered by the caller (see include/avm.h)."""
+    import torch
+    stream = torch.cuda.current_stream(torch.device("cuda", params.device))
+    _check(library(precision).avm_forces_static(
+        ctypes.byref(params), _dptr(pos), _dptr(cell_vertex_num), _dptr(cell_vertices), _dptr(vertex_neighbors),
+        _dptr(vertex_cell_neighbors), _dptr(force_out), _dptr(area_perim_out), ctypes.c_void_p(stream.cuda_stream)))
 
 
 def _hptr(a: Optional[np.ndarray]):

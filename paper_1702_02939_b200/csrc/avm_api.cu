@@ -846,6 +846,7 @@ const char* avm_strerror(int code) {
     case AVM_EINCONSISTENT: return "topology lists are out of range or inconsistent with each other";
     case AVM_ECUDA: return "CUDA error (see avm_last_cuda_error)";
     case AVM_ENOMEM: return "out of host memory";
+    case AVM_ETOOLARGE: return "more cells than avm_forces_static's fixed scratch array holds (AVM_FORCES_STATIC_MAX_CELLS)";
     default: return "unknown error";
   }
 }
@@ -855,3 +856,8 @@ const char* avm_last_cuda_error(void) { return g_cuda_error.c_str(); }
 const char* avm_precision(void) { return AVM_MIXED ? "mixed" : "f64"; }
 
 }  // extern "C"
+
+// for the entry points that live in other files (avm_forces_static.cu)
+namespace avm {
+void note_cuda_error(const char* call, cudaError_t e) { g_cuda_error = std::string(call) + ": " + cudaGetErrorString(e); }
+}
