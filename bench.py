@@ -299,6 +299,8 @@ def main():
     simp.close()
     del simp
     per_launch_ms = {k: v / max(1, prof_steps) for k, v in prof.items()}
+    # fewer than two launches per step = the library stepped launch-free (its default up to 8192 vertices)
+    timed_persistent = (st1["kernel_launches"] - st0["kernel_launches"]) < 2 * args.steps
     dom = max(kbytes, key=lambda k: per_launch_ms[k])
     ach = kbytes[dom] / (per_launch_ms[dom] * 1e-3) / 1e9
     cap = ncu_capture(dom, cfg["name"] + ("_steady" if args.warmup >= 300 else "")) if args.precision == "f64" else None
@@ -311,7 +313,11 @@ def main():
                 "ncu": {k: cap[k] for k in cap if k not in ("kernel", "workload")} if cap else None,
                 "peak_source": peak_src,
                 "timing": f"CUDA events on the library's stream around every launch of steps {args.warmup}..{args.warmup + prof_steps - 1} "
-                          "of a second, identical run (same schedule decisions as the timed region; the events serialise the launches)",
+                          "of a second, identical run; the events serialise the launches; " + (
+                              "LAUNCHED schedule (one launch per kernel): the timed region ran the launch-free persistent kernel, "
+                              "which avm_step_profile cannot bracket, so these per-kernel times describe a different schedule"
+                              if timed_persistent else "same schedule decisions as the timed region"),
+                "timed_region_schedule": "persistent (launch-free)" if timed_persistent else "one launch per kernel",
                 "bytes_per_launch": kbytes[dom], "ms_per_launch": per_launch_ms[dom],
                 "kernels_ms_per_launch": per_launch_ms,
                 "kernels_frac_of_measured_peak": {k: kbytes[k] / (per_launch_ms[k] * 1e-3) / 1e9 / peak for k in kbytes if per_launch_ms[k] > 0},

@@ -85,7 +85,9 @@ enum {
 /* Counters since creation.  error is a sticky bit set: 1 = a non-finite position was produced,
  * 2 = a flip was suppressed because a cell row would exceed S, 4 = the lists given to avm_create
  * are out of range or inconsistent (avm_create then fails with AVM_EINCONSISTENT), 8 = a T1
- * candidate list overflowed its capacity (cannot happen for a valid tiling). */
+ * candidate list overflowed its capacity (cannot happen for a valid tiling), 16 = the driver refused
+ * the launch-free persistent kernel (e.g. the GPU is shared and the grid cannot be co-resident) and the
+ * run went on with one launch per kernel: same results, more launches. */
 typedef struct avm_stats {
   int64_t step;             /* current step counter (step0 + steps taken)                       */
   int64_t t1_short;         /* edges found shorter than l_c                                      */
@@ -130,8 +132,10 @@ int avm_create_host(const avm_params* params, const double* pos_xy, const int32_
  * Conditions arising inside a step set avm_stats.error; they do not stop the run. */
 int avm_step(avm_sim* sim, int64_t n_steps);
 
-/* Same steps and same schedule as avm_step, but every kernel of the step is bracketed by CUDA
- * events on the stream and the call synchronises after each step: ms_per_kernel (HOST pointer,
+/* Same steps as avm_step, one launch per kernel (with avm_step's choice between two and three launches
+ * per step; never the launch-free persistent kernel, which has no kernel boundaries: for systems that
+ * avm_step advances launch-free the times describe the launched schedule instead).  Every kernel of the
+ * step is bracketed by CUDA events on the stream and the call synchronises after each step: ms_per_kernel (HOST pointer,
  * [AVM_K_COUNT]) receives the summed device time of each kernel class over the n_steps.  In the
  * default two-launch schedule the T1 flips of a step run inside the next force/move launch, so
  * AVM_K_T1_FLIP only holds the stand-alone T1 kernel that completes the last step.  Measurement
@@ -249,7 +253,8 @@ int avm_get_state_host(avm_sim* sim, double* pos_xy, int32_t* cell_vertex_num, i
  * paper, :96-100) is out of scope: these calls never change the lists.  All pointers DEVICE unless stated.
  *
  * avm_spv_geometry: Voronoi vertex of every triangle = circumcentre of its three cells,
- *   stored as the simulation's vertex positions (as avm_set_positions would) and, if non-NULL, in
+ *   stored as the simulation's vertex positions (as avm_set_positions would: the mean-square displacement
+ *   of avm_observe restarts from them, which also holds after avm_spv_forces / avm_spv_step) and, if non-NULL, in
  *   voronoi_xy [V][2]; area_perim [N][2] (may be NULL) = (A_c, P_c) of the resulting cells.  Asynchronous.
  * avm_spv_forces (Eq. A6-A7): force_xy [N][2] = -dE/dr_i with E of Eq. 1; force_sets
  *   [N][S][2] (may be NULL) = the contribution of each Voronoi vertex of the row of cell i ("force

@@ -51,7 +51,7 @@ struct BufferSet {
 
 struct Layout {
   size_t pos[2], vn[2], vc[2], cv[2], cvn[2], theta[2], rec[2], par[2], vtag[2], ctag[2];
-  size_t img, msd_ref;
+  size_t img, msd_ref, img_stamp;
   size_t minkey, cand, ctr, dirty, estamp, ap, epart, key[2], val[2], hist, newidx_v, newidx_c, order_v, order_c;
   size_t total;
 };
@@ -67,7 +67,7 @@ Layout make_layout(const avm_params& p) {
     L.vn[i] = take(12 * Vs); L.vc[i] = take(12 * Vs); L.cv[i] = take(4 * N * S); L.cvn[i] = take(4 * N);
     L.theta[i] = take(8 * N); L.rec[i] = take(32 * N); L.par[i] = take(32 * N); L.vtag[i] = take(4 * V); L.ctag[i] = take(4 * N);
   }
-  L.img = take(8 * V); L.msd_ref = take(16 * V);
+  L.img = take(8 * V); L.msd_ref = take(16 * V); L.img_stamp = take(8 * V);
   L.minkey = take(8 * N);
   L.cand = take(sizeof(Cand) * (t1_passes_of(p) > 1 ? 5 : 3) * N);   // the step's list (3N = every edge) + two lists of N for repeated passes
   L.ctr = take(sizeof(Counters));
@@ -111,6 +111,7 @@ struct avm_sim {
   unsigned int* d_feedback;   // device view of h_feedback (or a word of the counters)
   int2* img;                  // MSD: image counts, user order
   double2* msd_ref;           // MSD: unwrapped reference positions, user order
+  unsigned long long* img_stamp;   // MSD: step + 1 of the latest image-count update by a post-flip mover, user order
   bool tgt_custom, mod_custom;   // per-cell targets / moduli in force (Eq. 1); either one switches Consts::per_cell on
   unsigned int stamp;    // id of the latest repeated T1 pass (estamp entries equal to it were tested in that pass)
   int t1_passes;         // T1 passes per step (1 = north_star's rule; > 1 = repeat until none, NEXT-1)
@@ -124,6 +125,7 @@ struct avm_sim {
   double* epart;
   SortScratch sc;
   int cur_pos, cur_set;
+  long long host_error;   // sticky bits raised by the host side (16: a persistent launch was refused), OR-ed into avm_stats.error
   unsigned long long step;
   long long n_sorts, launches;
 
@@ -134,7 +136,7 @@ struct avm_sim {
     d.vn = b.vn; d.vc = b.vc; d.cv = b.cv; d.cvn = b.cvn; d.theta = b.theta; d.rec = b.rec; d.par = b.par;
     d.vtag = b.vtag; d.ctag = b.ctag;
     d.minkey = minkey; d.cand = cand; d.ctr = ctr; d.dirty = dirty; d.estamp = estamp;
-    d.feedback = d_feedback; d.img = img; d.msd_ref = msd_ref;
+    d.feedback = d_feedback; d.img = img; d.msd_ref = msd_ref; d.img_stamp = img_stamp;
     return d;
   }
   Dev dev_alt() const {   // the other buffer set, target of a re-sort / staging area
@@ -336,7 +338,7 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
     b.vtag = (int*)(w + L.vtag[i]); b.ctag = (int*)(w + L.ctag[i]);
     s->sc.key[i] = (unsigned int*)(w + L.key[i]); s->sc.val[i] = (int*)(w + L.val[i]);
   }
-  s->img = (int2*)(w + L.img); s->msd_ref = (double2*)(w + L.msd_ref);
+  s->img = (int2*)(w + L.img); s->msd_ref = (double2*)(w + L.msd_ref); s->img_stamp = (unsigned long long*)(w + L.img_stamp);
   s->tgt_custom = s->mod_custom = false;
   s->minkey = (unsigned long long*)(w + L.minkey);
   s->cand = (Cand*)(w + L.cand);
@@ -351,7 +353,7 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   s->sc.order_v = (int*)(w + L.order_v); s->sc.order_c = (int*)(w + L.order_c);
   s->cur_pos = 0; s->cur_set = 0;
   s->step = params->step0;
-  s->n_sorts = 0; s->launches = 0;
+  s->n_sorts = 0; s->launches = 0; s->host_error = 0;
   // Two-launch schedule (flips inside the next force/move launch) pays when the sweep is longer
   // than the flippers' chain of dependent loads (~15 us): from about a million vertices; and for
   // tiny systems, which flip rarely and are bound by the number of launches.  In between the plain
@@ -411,6 +413,7 @@ int create_common(const avm_params* params, const double* pos_xy, const int32_t*
   AVM_CUDA_F(cudaMemsetAsync(s->ctr, 0, sizeof(Counters), st));
   AVM_CUDA_F(cudaMemsetAsync(s->dirty, 0, 4 * 2 * (size_t)k.nw, st));
   AVM_CUDA_F(cudaMemsetAsync(s->estamp, 0, 12 * (size_t)k.Vs, st));
+  AVM_CUDA_F(cudaMemsetAsync(s->img_stamp, 0, 8 * (size_t)V, st));     // 0 = never (a stamp is step + 1 >= 1)
   const Dev d = s->dev();
   import_kernel<<<cdiv(V, 256), 256, 0, st>>>(d, k, (const double*)s->pos[1], stage.vn, stage.vc, (const int*)stage.cv);
   validate_kernel<<<cdiv(V, 256), 256, 0, st>>>(d, k);
@@ -467,7 +470,7 @@ int get_state_common(avm_sim* s, double* pos_xy, int32_t* cvn, int32_t* cv, int3
     if (rc) return rc;
     stats->step = (int64_t)s->step;
     stats->t1_short = c.t1_short; stats->t1_candidates = c.t1_candidates; stats->t1_flips = c.t1_flips;
-    stats->t1_blocked = c.t1_blocked; stats->overflow_rejects = c.overflow_rejects; stats->error = c.error;
+    stats->t1_blocked = c.t1_blocked; stats->overflow_rejects = c.overflow_rejects; stats->error = c.error | s->host_error;
     stats->n_sorts = s->n_sorts; stats->kernel_launches = s->launches;
   } else if (host_outputs) {
     AVM_CUDA(cudaStreamSynchronize(st));
@@ -529,7 +532,7 @@ int avm_step(avm_sim* s, int64_t n_steps) {
       }
       const int grid = s->k.per_cell ? persistent_grid(s->k.V, true) : s->persistent_grid;
       const int n = grid > 0 ? launch_persistent_steps(s->dev(), s->k, s->step, (int)chunk, grid, s->stream) : -1;
-      if (n < 0) { s->persistent_grid = 0; break; }    // refused: go on with one launch per kernel
+      if (n < 0) { s->persistent_grid = 0; s->host_error |= 16; break; }    // refused: go on with one launch per kernel, and say so (avm_stats.error)
       s->launches += n;
       if (chunk & 1) s->cur_pos = 1 - s->cur_pos;
       s->step += (unsigned long long)chunk;
@@ -579,7 +582,9 @@ int avm_step_profile(avm_sim* s, int64_t n_steps, double* ms_per_kernel) {
   cudaEvent_t ev[AVM_K_COUNT + 1];
   for (int i = 0; i <= AVM_K_COUNT; ++i) AVM_CUDA(cudaEventCreate(&ev[i]));
   for (int i = 0; i < AVM_K_COUNT; ++i) ms_per_kernel[i] = 0.0;
-  // same schedule decisions as avm_step; the events serialise the launches
+  // One launch per kernel, with avm_step's choice between two and three launches per step; the events serialise
+  // the launches.  The launch-free persistent kernel (avm_step's default up to 8192 vertices) has no kernel
+  // boundaries to bracket and is never taken here, so for such systems these times describe the launched schedule.
   bool pending = false;
   for (int64_t i = 0; i < n_steps; ++i) {
     const bool leave = leave_flips_pending(s, i == n_steps - 1);

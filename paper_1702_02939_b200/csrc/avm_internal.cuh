@@ -127,6 +127,8 @@ struct Dev {
   CellPar* par;       // [N] (A0_i, P0_i, K_A,i, K_P,i), internal order; read only when Consts::per_cell (NEXT-4)
   int2* img;          // [V] USER order: how many box lengths each vertex has left through the boundary (NEXT-2, MSD)
   double2* msd_ref;   // [V] USER order: unwrapped positions at the reference time of the mean-square displacement
+  unsigned long long* img_stamp; // [V] USER order: step + 1 of the latest image-count update made by a post-flip mover of the
+                                 // two-launch schedule (those may move a vertex more than once per step; the count is applied once)
   unsigned int* estamp; // [3*Vs] per directed half-edge (slot plane, owner vertex): id of the repeated pass that tested it last
   Counters* ctr;
   unsigned int* feedback; // mapped HOST word: every force/move launch reports the candidate count of the previous step

@@ -55,10 +55,12 @@ __global__ void spv_voronoi_kernel(const Dev d, const Consts k, const double* __
   double2 h = make_double2(wrap_box(o.r0.x + o.u.x, k.Lx), wrap_box(o.r0.y + o.u.y, k.Ly));
   if (!(isfinite(h.x) && isfinite(h.y))) { atomicOr((unsigned long long*)&d.ctr->error, 1ull); h = o.r0; }   // degenerate triangle
   pos_st(d.pos + v, h, k);
-  if (voronoi_user) {
-    const int t = d.vtag[v];
-    voronoi_user[2 * t] = h.x; voronoi_user[2 * t + 1] = h.y;
-  }
+  const int t = d.vtag[v];
+  // as avm_set_positions: the positions were replaced, not moved, so the unwrapped positions and the reference of the
+  // mean-square displacement restart from them (stale image counts would pair with unrelated positions)
+  d.msd_ref[t] = pos_ld(d.pos + v, k);
+  d.img[t] = make_int2(0, 0);
+  if (voronoi_user) { voronoi_user[2 * t] = h.x; voronoi_user[2 * t + 1] = h.y; }
 }
 
 // App. A.1: g_v = dE/dh_v = -(vertex force) from the cached (2 K_A (A - A0), 2 K_P (P - P0)) of the three cells

@@ -115,9 +115,17 @@ __device__ __forceinline__ VertexIn load_vertex(const Dev& d, const Consts& k, i
 
 // Eq. 4: dh/dt = mu F + (v0/3) sum of the three unit directors (R5), directors of the start of
 // the step (R7); explicit Euler; wrap into the box (R13).
+// kMover: the caller is a post-flip mover of the two-launch schedule (mover_unit).  Those move a vertex once per
+// candidate whose cells hold it, with the same inputs and the same result, so everything here is idempotent except
+// the image count of the mean-square displacement: the first mover to exchange this step's stamp applies it, the
+// others find the stamp and leave the count alone.  Every other caller moves each vertex exactly once per step.
+__device__ __forceinline__ bool img_claim(const Dev& d, int tag, unsigned long long step) {
+  return atomicExch(d.img_stamp + tag, step + 1ull) != step + 1ull;
+}
+template <bool kMover = false>
 __device__ __forceinline__ void move_vertex(const Dev& d, const Consts& k, int v, const double2 h, const double2 q0,
                                             const double2 q1, const double2 q2, const CellRec& c0, const CellRec& c1,
-                                            const CellRec& c2) {
+                                            const CellRec& c2, const unsigned long long step = 0ull) {
   const double2 f = vertex_force(h, q0, q1, q2, c0, c1, c2, k);
   const double vx = __fma_rn(k.mu, f.x, __dmul_rn(k.v0_3, __dadd_rn(__dadd_rn(c0.nx, c1.nx), c2.nx)));
   const double vy = __fma_rn(k.mu, f.y, __dmul_rn(k.v0_3, __dadd_rn(__dadd_rn(c0.ny, c1.ny), c2.ny)));
@@ -134,8 +142,11 @@ __device__ __forceinline__ void move_vertex(const Dev& d, const Consts& k, int v
   if (pk.y == 0u && y > k.hLy) ++iy;
   d.pos_next[v] = pk;
   if (ix | iy) {
-    int2* im = d.img + d.vtag[v];
-    int2 c = *im; c.x += ix; c.y += iy; *im = c;
+    const int tag = d.vtag[v];
+    if (!kMover || img_claim(d, tag, step)) {
+      int2* im = d.img + tag;
+      int2 c = *im; c.x += ix; c.y += iy; *im = c;
+    }
   }
 #else
   if ((hi_word(x) >= hi_word(k.Lx)) | (hi_word(y) >= hi_word(k.Ly))) {
@@ -143,8 +154,11 @@ __device__ __forceinline__ void move_vertex(const Dev& d, const Consts& k, int v
     x = wrap_box_count(x, k.Lx, ix); y = wrap_box_count(y, k.Ly, iy);
     if (!(isfinite(x) && isfinite(y))) atomicOr((unsigned long long*)&d.ctr->error, 1ull);
     if (ix | iy) {                      // the vertex left through the boundary: keep its unwrapped position (MSD)
-      int2* im = d.img + d.vtag[v];
-      int2 c = *im; c.x += ix; c.y += iy; *im = c;
+      const int tag = d.vtag[v];
+      if (!kMover || img_claim(d, tag, step)) {
+        int2* im = d.img + tag;
+        int2 c = *im; c.x += ix; c.y += iy; *im = c;
+      }
     }
   }
   d.pos_next[v] = make_double2(x, y);
@@ -174,7 +188,8 @@ __device__ AVM_PERS_ATTR void move_vertex_plain(const Dev& d, const Consts& k, i
 #ifndef AVM_FUSED_ATTR
 #define AVM_FUSED_ATTR __forceinline__
 #endif
-__device__ AVM_FUSED_ATTR void move_vertex_coherent(const Dev& d, const Consts& k, int v) {
+template <bool kMover = false>
+__device__ AVM_FUSED_ATTR void move_vertex_coherent(const Dev& d, const Consts& k, int v, const unsigned long long step = 0ull) {
   const double2 h = pos_ldcg(d.pos + v, k);
   double2 q[3];
   CellRec c[3];
@@ -183,7 +198,7 @@ __device__ AVM_FUSED_ATTR void move_vertex_coherent(const Dev& d, const Consts& 
     q[s] = pos_ldcg(d.pos + __ldcg(d.vn + s * k.Vs + v), k);
     c[s] = rec_ldcg(d.rec + __ldcg(d.vc + s * k.Vs + v));
   }
-  move_vertex(d, k, v, h, q[0], q[1], q[2], c[0], c[1], c[2]);
+  move_vertex<kMover>(d, k, v, h, q[0], q[1], q[2], c[0], c[1], c[2], step);
 }
 
 // The host chooses the schedule of later steps from the T1 load (avm_api.cu: leave_flips_pending), which it
@@ -288,7 +303,8 @@ __device__ __forceinline__ void sweep(const Dev& d, const Consts& k, const unsig
 // A few "flipper" warps do nothing else, so with few candidates all of this runs in the shadow of
 // the sweep; with many candidates every warp also claims what is left once its share of the
 // sweep is done.  Work is claimed, so a candidate always belongs to a warp that is running: the
-// wait can never depend on a CTA that has not been scheduled (no co-residency assumption).
+// wait can never depend on a CTA that has not been scheduled (no co-residency assumption; in the
+// few-candidate mode the waiting flipper warps claim what is still unclaimed after ~4 us).
 // The bitmap of flagged vertices is read-only for the whole launch (the cell pass of the previous
 // step wrote it, the cell pass of this step clears it), so the sweep's decision to skip a vertex
 // never changes while flips are in flight.
@@ -358,8 +374,9 @@ __device__ AVM_FUSED_ATTR void flipper_flips(const Dev& d, const Consts& k, cons
 // to idle (row a6).  Units are assigned statically: nothing ever waits for a unit.
 // Lanes = 4 cells x 8 row entries per pass (96 % of the cells need one pass); a vertex that sits
 // in several of the four rows is moved by the lowest lane holding it.  A vertex shared with
-// another candidate's cells is moved twice, with the same inputs and the same result.
-__device__ AVM_FUSED_ATTR void mover_unit(const Dev& d, const Consts& k, const unsigned i, const int lane) {
+// another candidate's cells (or met again in a later pass of a long row) is moved twice, with the same inputs
+// and the same result; its image count is applied once (img_claim).
+__device__ AVM_FUSED_ATTR void mover_unit(const Dev& d, const Consts& k, const unsigned i, const int lane, const unsigned long long step) {
   const int t = lane >> 3, j8 = lane & 7;
   const int4 q = __ldcg(reinterpret_cast<const int4*>(d.cand + i) + 1);   // (cL, cR, cE1, cE2)
   const int cell = t == 0 ? q.x : t == 1 ? q.y : t == 2 ? q.z : q.w;
@@ -373,7 +390,7 @@ __device__ AVM_FUSED_ATTR void mover_unit(const Dev& d, const Consts& k, const u
     if (j0 > 0 && j < n) u = __ldcg(reinterpret_cast<const int*>(d.cv + (size_t)(j >> 2) * k.N + cell) + (j & 3));
     const int uu = j < n ? u : -1 - lane;                                   // inactive lanes match nobody
     const unsigned same = __match_any_sync(kFull, uu);
-    if (j < n && __ffs(same) - 1 == lane) move_vertex_coherent(d, k, u);
+    if (j < n && __ffs(same) - 1 == lane) move_vertex_coherent<true>(d, k, u, step);
   }
   if (lane < 4) d.minkey[lane == 0 ? q.x : lane == 1 ? q.y : lane == 2 ? q.z : q.w] = ~0ull;
 }
@@ -398,7 +415,8 @@ __device__ __forceinline__ void release_minkeys(const Dev& d, const unsigned i0,
 #endif
 template <bool kFused>
 __global__ void __launch_bounds__(kVertexBlock, AVM_FM_MINB)
-force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, const unsigned parity) {
+force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts k, const unsigned long long step) {
+  const unsigned parity = (unsigned)(step & 1ull);
   pdl_launch_dependents();
   pdl_wait();
   const int tid = blockIdx.x * kVertexBlock + threadIdx.x;
@@ -421,10 +439,12 @@ force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts 
       const unsigned wib = threadIdx.x >> 5, nb = gridDim.x;
       const unsigned fid = wib * nb + blockIdx.x;                          // flipper id of this warp, if < prev
       const unsigned full = prev / nb, rest = prev % nb;                   // warps 0..full-1 of every CTA, warp `full` of `rest` CTAs
-#if AVM_TEST_SKEW
+#if AVM_TEST_SKEW == 1 || AVM_TEST_SKEW == 2
       // Test builds only (tests/test_gpu_skew.py): one side of the launch is held back for tens of microseconds so
       // that the other finishes first.  1: the sweepers start after the flips and the movers are long done;
       // 2: the flippers start after the sweep is long over.  Results must not depend on it.
+      // (3, below: every other mover starts 30 us after the rest, so that a vertex two movers share is moved at two
+      // clearly different times.)
       if ((AVM_TEST_SKEW == 1) != (fid < prev)) {
         unsigned long long t0, t1;
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
@@ -432,12 +452,27 @@ force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts 
       }
 #endif
       if (fid < prev) {
-        if (fid * 8u < prev) flipper_flips(d, k, prev, lane, prev);        // the first prev/8 of them claim the flips
+        // The first prev/8 of them claim the flips at once.  The others wait for the decisions, and a waiting warp that
+        // has polled for ~4 us tries to claim too: a batch still unclaimed by then belongs to a warp that is not
+        // running (a CTA not yet resident: a shared GPU, MPS), so the wait never depends on co-residency.
+        bool claim = fid * 8u < prev;
+        for (unsigned polls = 0;;) {
+          if (claim) { flipper_flips(d, k, prev, lane, prev); claim = false; }
+          if (ld_volatile(&d.ctr->flip_done) >= prev) break;
+          __nanosleep(64);
+          if (++polls == 64u) { polls = 0; claim = true; }
+        }
         AVM_TR_MAX(1);
-        while (ld_volatile(&d.ctr->flip_done) < prev) __nanosleep(64);
         __threadfence();
         AVM_TR_MAX(3);
-        mover_unit(d, k, fid, lane);
+#if AVM_TEST_SKEW == 3
+        if (fid & 1u) {
+          unsigned long long t0, t1;
+          asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+          do { __nanosleep(1000); asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1)); } while (t1 - t0 < 30000ull);
+        }
+#endif
+        mover_unit(d, k, fid, lane, step);
         AVM_TR_MAX(4);
       } else {
         const unsigned before = blockIdx.x * full + min(blockIdx.x, rest) + min(wib, full) + (wib > full && blockIdx.x < rest ? 1u : 0u);
@@ -1116,7 +1151,10 @@ struct GridBarrier {
     __syncthreads();
   }
 };
-static constexpr int kClusterBlock = 256;     // CTA size of the one-cluster grid (measured at configs[1]: 7.7 us/step; 512 threads: 8.4)
+// CTA size of the persistent kernel in all its forms (one CTA, one cluster, cooperative grid): its launch bounds, the
+// occupancy query that sizes the cooperative grid and both launches use this one constant, whatever AVM_VERTEX_BLOCK
+// is.  Measured at configs[1] as one cluster: 256 threads 7.7 us/step, 512 threads 8.4.
+static constexpr int kClusterBlock = 256;
 template <bool kPerCell, bool kOneCta>
 __global__ void __launch_bounds__(kClusterBlock)
 persistent_steps_kernel(Dev d, const __grid_constant__ Consts k, const unsigned long long step0, const int n_steps, const int one_cluster) {
@@ -1345,8 +1383,8 @@ int launch_step(const Dev& d, const Consts& k, unsigned long long step, cudaStre
   const unsigned parity = (unsigned)(step & 1ull);
   if (ev) cudaEventRecord(ev[0], s);
   const bool pdl = AVM_PDL && ev == nullptr;   // events between the kernels would break the chain anyway
-  if (consume_pending) launch_chained(force_move_kernel<true>, k.fm_grid, kVertexBlock, s, pdl, d, k, parity);
-  else launch_chained(force_move_kernel<false>, k.fm_grid, kVertexBlock, s, pdl, d, k, parity);
+  if (consume_pending) launch_chained(force_move_kernel<true>, k.fm_grid, kVertexBlock, s, pdl, d, k, step);
+  else launch_chained(force_move_kernel<false>, k.fm_grid, kVertexBlock, s, pdl, d, k, step);
   if (ev) cudaEventRecord(ev[1], s);
   Dev m = d;                      // from here on the moved positions are "the" positions
   m.pos = d.pos_next; m.pos_next = d.pos;
@@ -1403,10 +1441,10 @@ int persistent_grid(int V, bool per_cell) {
   cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   if (!coop || sms <= 0) return 0;
-  if (per_cell) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, persistent_steps_kernel<true, false>, kVertexBlock, 0);
-  else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, persistent_steps_kernel<false, false>, kVertexBlock, 0);
+  if (per_cell) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, persistent_steps_kernel<true, false>, kClusterBlock, 0);
+  else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, persistent_steps_kernel<false, false>, kClusterBlock, 0);
   if (per_sm < 1) return 0;
-  const int want = V <= 512 ? 1 : cdiv(V, kVertexBlock), cap = sms * per_sm;     // tiny systems: one CTA, barriers are __syncthreads
+  const int want = V <= 512 ? 1 : cdiv(V, kClusterBlock), cap = sms * per_sm;     // tiny systems: one CTA, barriers are __syncthreads
   // up to kClusterVertices vertices the grid is one cluster of at most 16 CTAs (hardware barrier instead of an
   // arrival counter in L2); every thread then takes several vertices
   if (V > 512 && V <= kClusterVertices) { const int wc = cdiv(V, kClusterBlock); return wc < kClusterMax ? wc : kClusterMax; }
@@ -1438,7 +1476,7 @@ int launch_persistent_steps(const Dev& d, const Consts& k, unsigned long long st
     one_cluster = 0;                       // refused (cluster size not schedulable): the cooperative grid below
   }
   cudaMemsetAsync(&d.ctr->bar, 0, sizeof(unsigned int), s);
-  if (cudaLaunchCooperativeKernel(fn, dim3((unsigned)grid), dim3(kVertexBlock), args, 0, s) != cudaSuccess) {
+  if (cudaLaunchCooperativeKernel(fn, dim3((unsigned)grid), dim3(kClusterBlock), args, 0, s) != cudaSuccess) {
     cudaGetLastError();
     return -1;
   }

@@ -123,6 +123,24 @@ def test_trajectory_parity_larger_configs(B, k, steps, chunk):
     assert g.stats()["t1_flips"] > 50
 
 
+@pytest.mark.parametrize("sched", ["fused", "unfused", "persistent"])
+@pytest.mark.parametrize("k,steps,chunk", [(0, 100, 5), (1, 40, 10)])
+def test_trajectory_parity_with_mobility_and_moduli_other_than_one(B, k, steps, chunk, sched):
+    """every other dynamic test runs mu = K_A = K_P = A0 = 1, where a dropped or misplaced factor in the
+    move (Eq. 4) or in the force prefactors (Eq. A1-A3) would go unnoticed.  Same bar as
+    the headline trajectory test, through the T1 burst, in every schedule."""
+    t = tiling(k)
+    p = dict(w.config_params(k), mu=0.6, KA=1.7, KP=0.6, A0=1.2)
+    g = B.from_tiling(t, schedule=sched, **p)
+    o = oracle.from_tiling(t, **p)
+    for s in range(0, steps, chunk):
+        g.step(chunk)
+        o.step(chunk)
+        assert_states_match(to_np(g.get_state()), o.get_state(), t.Lx, t.Ly)
+    st = g.stats()
+    assert st["t1_flips"] >= 20 and st["error"] == 0
+
+
 def near_threshold(state, pairs, Lx, Ly, l_c, band=1e-9):
     pos = state["pos"]
     out = set()
@@ -777,6 +795,37 @@ def test_mean_square_displacement_matches_the_oracle(B, sched):
     g = B.from_tiling(hx, KA=0.0, KP=0.0, v0=0.8, Dr=0.0, dt=0.01, l_c=0.0, schedule=sched)
     g.step(1500)
     assert abs(g.observe()["msd"] - 144.0) < 1e-9 * 144.0
+
+
+@pytest.mark.parametrize("seed", [4, 1])
+def test_image_counts_are_applied_once_when_movers_overlap(B, seed):
+    """in the two-launch schedule the post-flip movers run once per T1 candidate, so a vertex of a cell
+    that two candidates touch (or met again in a later pass over a long row) is moved more than once in a step.
+    The move is idempotent, the image count of the mean-square displacement is an increment: it must be applied
+    once.  The tiling translates rigidly (no forces, one common director) by a fifth of the box per step, so a
+    third of the vertices cross the boundary in every step and the MSD is (n v0 dt)^2 up to the end points that T1s
+    reposition; a vertex counted twice adds 64^2 / 8192 = 0.5.  (The library that incremented per mover gave
+    4101.8 and 4102.6 instead of 4096.0 on these two tilings.)  The steps must come in ONE call: the last step of
+    a call always completes with the stand-alone T1 kernel.  Exact equality with the three-launch schedule, and
+    the oracle's unwrapped positions."""
+    t = w.voronoi_tiling(4096, 64.0, seed)
+    t.theta[:] = 0.6
+    p = dict(KA=0.0, KP=0.0, A0=1.0, P0=3.8, v0=128.0, Dr=0.0, mu=1.0, dt=0.1, l_c=0.008, seed=11)
+    f = B.from_tiling(t, schedule="fused", **p)
+    u = B.from_tiling(t, schedule="unfused", **p)
+    o = oracle.from_tiling(t, **p)
+    for n in (5, 10):
+        f.step(5)
+        u.step(5)
+        o.step(5)
+        a = f.observe()["msd"]
+        assert a == u.observe()["msd"], (n, a, u.observe()["msd"])
+        assert abs(a - o.msd()) <= 1e-9 * o.msd()
+        assert abs(a - (12.8 * n) ** 2) < 1e-3
+    sf, su = f.stats(), u.stats()
+    assert sf["kernel_launches"] < su["kernel_launches"] - 6                    # it really ran two launches per step
+    assert 20 < sf["t1_candidates"] <= 85 and sf["t1_blocked"] > 0               # one warp per candidate, with shared cells
+    assert np.array_equal(to_np(f.get_state())["pos"], to_np(u.get_state())["pos"])
 
 
 @pytest.mark.parametrize("k,steps,sort_every", [(0, 150, 0), (1, 60, 7), (2, 20, 6)])

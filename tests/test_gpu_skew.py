@@ -19,7 +19,7 @@ def B(tmp_path_factory):
     from paper_1702_02939_b200 import build, binding
     build.build()
     d = tmp_path_factory.mktemp("skew")
-    for n in (1, 2):
+    for n in (1, 2, 3):
         binding.register_library(f"skew{n}", build.build_variant(str(d / f"libavm_skew{n}.so"), [f"AVM_TEST_SKEW={n}"]))
     return binding
 
@@ -51,3 +51,24 @@ def test_fused_schedule_does_not_depend_on_who_finishes_first(B, skew):
     for key in ("t1_short", "t1_candidates", "t1_flips", "t1_blocked", "error"):
         assert sg["stats"][key] == sr["stats"][key], key
     assert sr["stats"]["t1_flips"] > 1000
+
+
+def test_image_counts_are_applied_once_when_movers_run_at_different_times(B):
+    """ADVICE r2, under skew (see tests/test_gpu_parity.py::test_image_counts_are_applied_once_when_movers_overlap
+    for the scenario: a rigidly translating tiling whose MSD is (n v0 dt)^2).  Movers of different candidates
+    normally start within nanoseconds of each other, and a lost update can hide a second increment of a shared
+    vertex's image count; the third test build starts every other mover 30 us late, so every shared vertex is
+    moved at two clearly different times.  (Without the once-only claim this build gave 4108.2 instead of 4096.0.)"""
+    t = w.voronoi_tiling(4096, 64.0, 4)
+    t.theta[:] = 0.6
+    p = dict(KA=0.0, KP=0.0, A0=1.0, P0=3.8, v0=128.0, Dr=0.0, mu=1.0, dt=0.1, l_c=0.008, seed=11)
+    ref = B.from_tiling(t, schedule="unfused", **p)
+    g = B.from_tiling(t, schedule="fused", precision="skew3", **p)
+    ref.step(5)
+    g.step(5)
+    m = ref.observe()["msd"]
+    assert g.observe()["msd"] == m and abs(m - 64.0 ** 2) < 1e-3
+    st = g.stats()
+    assert st["kernel_launches"] < ref.stats()["kernel_launches"] - 3
+    assert 20 < st["t1_candidates"] <= 85 and st["t1_blocked"] > 0     # the one-warp-per-candidate mode, with shared cells
+    assert np.array_equal(to_np(g.get_state())["pos"], to_np(ref.get_state())["pos"])

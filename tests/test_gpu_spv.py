@@ -42,6 +42,13 @@ def test_spv_geometry_and_forces_match_the_oracle(B, N, L, seed, sort):
     assert np.abs(ap.cpu().numpy() - apo).max() <= 1e-10 * np.abs(apo).max()
     # the Voronoi vertices are now the simulation's vertex positions
     assert np.abs(h.min_image(g.get_state()["pos"].cpu().numpy() - ho, L)).max() <= 1e-10 * L
+    # ... replaced, not moved: the mean-square displacement restarts from them, whatever was counted before
+    if N == 64:
+        g2 = B.from_tiling(t, sort_at_create=sort, **dict(p, v0=3.0, dt=0.02))
+        g2.step(200)
+        assert g2.observe()["msd"] > 1.0
+        g2.spv_geometry(r)
+        assert g2.observe()["msd"] == 0.0
     F, fs = g.spv_forces(r)
     Fo = o.forces()
     rms = np.sqrt((Fo ** 2).sum(1).mean())
@@ -54,11 +61,13 @@ def test_spv_geometry_and_forces_match_the_oracle(B, N, L, seed, sort):
         assert np.abs(fs.cpu().numpy().sum(axis=1) - F.cpu().numpy()).max() <= 1e-12 * scale
 
 
-def test_spv_steps_match_the_oracle(B):
+@pytest.mark.parametrize("mu,KA,KP", [(1.0, 1.0, 1.0), (0.37, 1.7, 0.6)])
+def test_spv_steps_match_the_oracle(B, mu, KA, KP):
     """ten steps of Eq. 3 on the fixed triangulation: positions, directors (Philox keyed on the same seed, step,
-    cell), the simulation's saved Voronoi vertices, and the circumcircle verdict after every call"""
+    cell), the simulation's saved Voronoi vertices, and the circumcircle verdict after every call; also with a
+    mobility and moduli other than 1 (the oracle's mu is pinned by tests/test_oracle_spv.py)"""
     t = w.voronoi_tiling(1024, 32.0, 3)
-    p = dict(KA=1.0, KP=1.0, A0=1.0, P0=3.8, v0=0.2, Dr=1.0, mu=1.0, dt=2e-5, l_c=0.0, seed=11)
+    p = dict(KA=KA, KP=KP, A0=1.0, P0=3.8, v0=0.2, Dr=1.0, mu=mu, dt=2e-5, l_c=0.0, seed=11)
     g = B.from_tiling(t, sort_at_create=True, **p)
     o = spv.SpvOracle(t, t.points, **p)
     r = dev(t.points)

@@ -116,6 +116,34 @@ def test_eq3_pure_self_propulsion_and_director_noise():
     assert np.abs(d2 - 0.01 * 0.3 * np.stack([np.cos(th1), np.sin(th1)], axis=1)).max() < 1e-14
 
 
+def test_eq3_mobility_scales_the_force_term():
+    """Eq. 3: dr_i/dt = mu F_i + v0 n_i.  A passive step (v0 = 0) with mu = 0.37 displaces every cell
+    by dt mu F(r0) (F from the force routine that central differences of E pin above), and, independently of that
+    routine, the energy drops at the rate mu |F|^2: (E0 - E1) / (dt sum |F|^2) -> mu for a small step, with |F|^2
+    taken from central differences of E.  Fails when the step drops mu or applies it to the propulsion term."""
+    mu, dt = 0.37, 1e-7
+    t = w.voronoi_tiling(64, 8.0, 4)
+    o = spv.SpvOracle(t, t.points, KA=1.0, KP=1.0, A0=1.0, P0=3.6, v0=0.0, mu=mu, dt=dt)
+    r0, F0, e0 = o.r.copy(), o.forces(), o.energy()
+    o.step(1)
+    d = h.min_image(o.r - r0, 8.0)
+    assert np.abs(d - dt * mu * F0).max() < 1e-14
+    # |F|^2 from central differences of the energy, not from forces()
+    eps, g2 = 1e-6, 0.0
+    for i in range(t.N):
+        for a in range(2):
+            rp, rm = r0.copy(), r0.copy()
+            rp[i, a] += eps
+            rm[i, a] -= eps
+            g2 += ((o.energy(rp) - o.energy(rm)) / (2 * eps)) ** 2
+    assert abs((e0 - o.energy()) / (dt * g2) - mu) < 2e-3 * mu
+    # the propulsion term does not carry mu: active step, no forces
+    a = spv.SpvOracle(t, t.points, KA=0.0, KP=0.0, v0=0.3, Dr=0.0, mu=mu, dt=0.01)
+    th = a.theta.copy()
+    a.step(1)
+    assert np.abs(h.min_image(a.r - t.points, 8.0) - 0.01 * 0.3 * np.stack([np.cos(th), np.sin(th)], axis=1)).max() < 1e-14
+
+
 def test_passive_spv_descends_the_energy():
     t = w.voronoi_tiling(64, 8.0, 4)
     o = spv.SpvOracle(t, t.points, KA=1.0, KP=1.0, A0=1.0, P0=3.6, v0=0.0, dt=2e-5)   # a Poisson-Voronoi start is stiff (max |F| ~ 90): small dt
