@@ -141,6 +141,28 @@ def test_trajectory_parity_with_mobility_and_moduli_other_than_one(B, k, steps, 
     assert st["t1_flips"] >= 20 and st["error"] == 0
 
 
+@pytest.mark.parametrize("sched", ["fused", "unfused", "persistent"])
+def test_an_edge_whose_end_cells_coincide_does_not_flip_on_gpu(B, sched):
+    """GPU twin of tests/test_oracle_t1.py::test_an_edge_whose_end_cells_coincide_does_not_flip (R10, "the four cells
+    are distinct"): the tiling of tests/horseshoe.py passes avm_create's validation, its one short edge is counted and
+    is no candidate, neither in the test hooks nor in the cell pass of a real step (nothing moves: dt = 0)."""
+    from tests import horseshoe as hs
+    t, edge = hs.build()
+    g = B.from_tiling(t, schedule=sched, **hs.PARAMS)
+    o = oracle.from_tiling(t, **hs.PARAMS)
+    cand, win = g.debug_t1()
+    assert len(cand) == 0 and len(win) == 0
+    g.t1_pass()
+    o.t1_pass()
+    assert_states_match(to_np(g.get_state()), o.get_state(), t.Lx, t.Ly, pos_tol=0.0)
+    g.step(3)
+    o.step(3)
+    sg = to_np(g.get_state())
+    assert_states_match(sg, o.get_state(), t.Lx, t.Ly, pos_tol=0.0)
+    assert sg["stats"]["t1_short"] == 4 and sg["stats"]["t1_candidates"] == 0 and sg["stats"]["t1_flips"] == 0
+    assert np.array_equal(sg["cell_vertices"], t.cell_vertices)
+
+
 def near_threshold(state, pairs, Lx, Ly, l_c, band=1e-9):
     pos = state["pos"]
     out = set()

@@ -394,3 +394,33 @@ def test_repeated_passes_count_the_first_pass_and_raise_overflow_on_any_pass():
     one.step(1)
     st = one.get_state()["stats"]
     assert st["error"] == 2 and st["overflow_rejects"] == 1 and st["t1_short"] == 3 and st["t1_flips"] == 1
+
+
+def test_an_edge_whose_end_cells_coincide_does_not_flip():
+    """R10, "the four cells are distinct" (a reading: the paper is silent).  In a valid tiling E1, E2 never equal L
+    or R (a vertex has three distinct cells) and L != R for cells narrower than half the box, so the clause is
+    about E1 == E2: one cell touching both ends of an edge it does not contain.  tests/horseshoe.py reaches such a
+    tiling from the 4 x 4 hexagonal torus by T1s and this test first checks it with the independent list checker.
+    The edge is the only short one and passes every other clause (L, R have more than three vertices, E has room):
+    it is counted as short, is no candidate, and the pass changes nothing.  Fails when the clause is deleted."""
+    from tests import horseshoe as hs
+    t, (v1, v2, cL, cR, cE) = hs.build()
+    h.check_topology(t.cell_vertex_num, t.cell_vertices, t.vertex_neighbors, t.vertex_cell_neighbors)
+    assert len({cL, cR, cE}) == 3
+    rows = [set(t.cell_vertices[c, :t.cell_vertex_num[c]].tolist()) for c in (cL, cR, cE)]
+    assert {v1, v2} <= rows[0] and {v1, v2} <= rows[1] and {v1, v2} <= rows[2]      # E holds both ends ...
+    row = t.cell_vertices[cE, :t.cell_vertex_num[cE]].tolist()
+    i1, n = row.index(v1), len(row)
+    assert row[(i1 + 1) % n] != v2 and row[(i1 - 1) % n] != v2                       # ... but not the edge
+    d = h.min_image(t.pos[v2] - t.pos[v1], np.array([t.Lx, t.Ly]))
+    assert np.hypot(*d) < hs.PARAMS["l_c"]
+    o = oracle.from_tiling(t, **hs.PARAMS)
+    before = o.get_state()
+    cand, win = o.debug_t1()
+    assert len(cand) == 0 and len(win) == 0
+    o.t1_pass()
+    after = o.get_state()
+    for key in ("cell_vertex_num", "cell_vertices", "vertex_neighbors", "vertex_cell_neighbors", "pos"):
+        assert np.array_equal(before[key], after[key]), key
+    st = after["stats"]
+    assert st["t1_short"] == 1 and st["t1_candidates"] == 0 and st["t1_flips"] == 0 and st["error"] == 0
