@@ -204,6 +204,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (kernel experiments only)")
     ap.add_argument("--no-nominal-run", action="store_true", help="skip the whole_run / second_half records")
+    ap.add_argument("--no-cfg4", action="store_true",
+                    help="skip the cfg4 sub-record (N = 4,194,304: the config's own 500-step run, added to the default cfg3 line)")
     ap.add_argument("--profile-steps", type=int, default=0,
                     help="steps of the per-kernel event pass (default: the timed region itself, at most 200 steps)")
     ap.add_argument("--t1-passes", type=int, default=1,
@@ -264,14 +266,32 @@ def main():
         barrier()
         return max_over_ranks(e0.elapsed_time(e1), dist, "cuda"), sampler
 
-    def region_record(ms, n, first_step, st0, st1, sampler):
+    def region_record(ms, n, first_step, st0, st1, sampler, n_vertices=None):
         per = ms / n
+        nv = V if n_vertices is None else n_vertices
+        scale = nv / V                                    # both byte models are per vertex
         return {"steps": f"{first_step}..{first_step + n - 1}", "ms_per_step": per,
-                "value": aggregate_value(V, n, ms, world), "unit": UNIT, "timesteps_per_s": n / (ms * 1e-3),
+                "value": aggregate_value(nv, n, ms, world), "unit": UNIT, "timesteps_per_s": n / (ms * 1e-3),
                 "t1_flips_per_step": (st1["t1_flips"] - st0["t1_flips"]) / n,
-                "bandwidth": {"bytes_model_this_repo_128B_per_vertex": bandwidth_fractions(step_bytes, per, peak),
-                              "bytes_model_survey_134B_per_vertex": bandwidth_fractions(survey_step_bytes, per, peak)},
+                "bandwidth": {"bytes_model_this_repo_128B_per_vertex": bandwidth_fractions(step_bytes * scale, per, peak),
+                              "bytes_model_survey_134B_per_vertex": bandwidth_fractions(survey_step_bytes * scale, per, peak)},
                 "clocks": sampler.summary()}
+
+    def nominal_run(tq, pq, nominal):
+        """the config's own run from its initial state, timed in two halves (re-sorts included)"""
+        simn = B.from_tiling(tq, **pq)
+        s0 = simn.stats()
+        h1 = nominal // 2
+        ms1, smp1 = timed_steps(simn, h1)
+        s1 = simn.stats()
+        ms2, smp2 = timed_steps(simn, nominal - h1)
+        s2 = simn.stats()
+        smp_all = ClockSampler(local_rank)
+        smp_all.sm, smp_all.reasons, smp_all.sm_max = smp1.sm + smp2.sm, smp1.reasons | smp2.reasons, smp1.sm_max
+        whole = region_record(ms1 + ms2, nominal, 0, s0, s2, smp_all, tq.V)
+        whole["includes_resorts"] = s2["n_sorts"] - s0["n_sorts"]
+        second = region_record(ms2, nominal - h1, h1, s1, s2, smp2, tq.V)
+        return simn, whole, second
 
     # ---------------- device-resident run: inputs already in HBM when the clock starts -----------
     sim = B.from_tiling(t, **p)
@@ -331,20 +351,36 @@ def main():
     whole_run = second_half = None
     if not args.no_nominal_run:
         nominal = cfg["steps"] if cfg["steps"] <= 2000 else 2000     # cfg1/cfg2 name 10^4 steps: the first 2000 are timed
-        simn = B.from_tiling(t, **p)
-        s0 = simn.stats()
-        h1 = nominal // 2
-        ms1, smp1 = timed_steps(simn, h1)
-        s1 = simn.stats()
-        ms2, smp2 = timed_steps(simn, nominal - h1)
-        s2 = simn.stats()
-        smp_all = ClockSampler(local_rank)
-        smp_all.sm, smp_all.reasons, smp_all.sm_max = smp1.sm + smp2.sm, smp1.reasons | smp2.reasons, smp1.sm_max
-        whole_run = region_record(ms1 + ms2, nominal, 0, s0, s2, smp_all)
-        whole_run["includes_resorts"] = s2["n_sorts"] - s0["n_sorts"]
-        second_half = region_record(ms2, nominal - h1, h1, s1, s2, smp2)
+        simn, whole_run, second_half = nominal_run(t, p, nominal)
         simn.close()
         del simn
+
+    # ---------------- cfg4 (N = 4,194,304, T1-heavy, re-sort every 100 steps) beside the default cfg3 line -------
+    # The largest single-GPU config has no line of its own in a default run: its own 500-step run in two
+    # halves, then the per-kernel event pass over the next 40 steps of the same simulation.  GPU only, no oracle leg.
+    cfg4 = None
+    if args.config == 3 and world == 1 and args.precision == "f64" and args.t1_passes == 1 and not (args.no_cfg4 or args.no_nominal_run):
+        c4 = w.CONFIGS[4]
+        t4 = w.config_tiling(4)
+        p4 = dict(w.config_params(4), device=local_rank, schedule=args.schedule, precision=args.precision)
+        sim4, whole4, second4 = nominal_run(t4, p4, c4["steps"])
+        smp4 = ClockSampler(local_rank)
+        torch.cuda.synchronize()
+        smp4.start()
+        prof4 = sim4.step_profile(40)
+        torch.cuda.synchronize()
+        smp4.stop()
+        err4 = sim4.stats()["error"]
+        sim4.close()
+        del sim4
+        kb4 = {"force_move": BYTES_FORCE_MOVE_PER_VERTEX * t4.V, "cell_update": BYTES_CELL_UPDATE_PER_CELL * t4.N}
+        per4 = {k: v / 40 for k, v in prof4.items()}
+        cfg4 = {"workload": workload_string(c4, t4.N, t4.V), "whole_run": whole4, "second_half": second4,
+                "kernels_ms_per_launch": per4,
+                "kernels_frac_of_measured_peak": {k: kb4[k] / (per4[k] * 1e-3) / 1e9 / peak for k in kb4 if per4[k] > 0},
+                "kernels_timing": f"CUDA events around every launch of steps {c4['steps']}..{c4['steps'] + 39} of the same simulation (serialised launches)",
+                "clocks_during_profile_pass": smp4.summary(), "error_word": err4}
+        del t4
 
     # ---------------- end to end through the host-pointer entry points --------------------------
     # One job = avm_create_host (H2D of the whole state from pinned memory) + K steps +
@@ -425,6 +461,7 @@ def main():
             "second_half": second_half,
             "e2e": e2e,
             "cpu_baseline": cpu,
+            "cfg4": cfg4,
         }
         print(json.dumps(line))
     if dist is not None:
