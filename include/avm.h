@@ -20,7 +20,10 @@
  *     or pinned) host memory.  The *_host twins take host pointers and do the copies themselves.
  *   - The library never allocates or frees device memory: the caller passes one workspace of
  *     avm_workspace_bytes() bytes (256-byte aligned) that must outlive the avm_sim.  The avm_sim
- *     object itself owns only host-side bookkeeping.
+ *     object itself owns only host-side bookkeeping: a heap object and, when the kernel schedule is
+ *     chosen per step (the default from a million vertices), one 64-byte block of mapped pinned host
+ *     memory (cudaHostAlloc) through which the kernels report the T1 load; avm_destroy frees both.
+ *     avm_forces_static (below) allocates nothing at all.
  *   - All work is enqueued on the CUDA stream given at creation.  avm_step never synchronises the
  *     host (the AVM loop has no host<->device traffic).
  *   - Every user-visible array is in USER ORDER (the order given to avm_create), whatever the

@@ -556,26 +556,6 @@ int avm_step(avm_sim* s, int64_t n_steps) {
   return AVM_OK;
 }
 
-#ifdef AVM_TRACE
-// variant builds only: mean phase times (us) of the fused force/move launch since the last call
-extern "C" int avm_trace_read(avm_sim* s, double* out8) {
-  Counters c;
-  int rc = read_counters(s, &c);
-  if (rc) return rc;
-  for (int i = 1; i < 8; ++i) out8[i] = c.tr_acc[0] ? 1e-3 * (double)c.tr_acc[i] / (double)c.tr_acc[0] : 0.0;
-  out8[0] = (double)c.tr_acc[0];
-  // stamps of warp 0's first batch in the latest launch, relative to its entry into flipper_flips
-  fprintf(stderr, "w0 quads (us from entry): cand %.2f phase2 %.2f writes %.2f refresh %.2f rec %.2f | flipper_flips (us from entry): precheck %.2f claim %.2f quads %.2f loop_end %.2f fence %.2f signalled %.2f second_call_duration %.2f\n",
-          1e-3 * c.tr2[1], 1e-3 * c.tr2[2], 1e-3 * c.tr2[3], 1e-3 * c.tr2[4], 1e-3 * c.tr2[5],
-          1e-3 * c.tr2[9], 1e-3 * c.tr2[10], 1e-3 * c.tr2[11], 1e-3 * c.tr2[12], 1e-3 * c.tr2[13], 1e-3 * c.tr2[14], 1e-3 * c.tr2[15]);
-  fprintf(stderr, "   call: before_call->callee_entry %.2f, callee_entry->callee_end %.2f, callee_end->after_call %.2f\n", 1e-3 * (double)(long long)(c.tr2[7] - c.tr2[6]), 1e-3 * (double)(long long)(c.tr2[8] - c.tr2[7]), 1e-3 * (double)(long long)(c.tr2[0] - c.tr2[8]));
-  fprintf(stderr, "   per-lane phase2 / end (us): ");
-  for (int l = 0; l < 32; ++l) fprintf(stderr, "%.1f/%.1f ", 1e-3 * c.tr2[16 + l], 1e-3 * c.tr2[48 + l]);
-  fprintf(stderr, "\n");
-  cudaMemsetAsync(s->ctr->tr_acc, 0, sizeof(c.tr_acc), s->stream);
-  return AVM_OK;
-}
-#endif
 
 int avm_step_profile(avm_sim* s, int64_t n_steps, double* ms_per_kernel) {
   if (!s || n_steps < 0 || !ms_per_kernel) return AVM_EINVAL;

@@ -68,9 +68,6 @@ struct Counters {
   long long t1_short, t1_candidates, t1_flips, t1_blocked, overflow_rejects, error;
   double obs[16];  // observables of the latest avm_energy / avm_observe call (slots: avm_step.cu)
   unsigned long long spv[2];   // SPV circumcircle test (avm_spv.cu): failed tests of the latest step, first failing step of the call
-  // phase trace of the fused force/move launch (variant builds with -DAVM_TRACE only): tr = this launch's
-  // min start / max phase-end times (ns, %globaltimer), tr_acc = sums of (phase end - start) over launches
-  unsigned long long tr[8], tr_acc[8], tr2[80];
 };
 
 // Up to this many T1 candidates a step leaves its flips to the next force/move launch (two launches per

@@ -72,14 +72,6 @@ static constexpr unsigned kFull = 0xffffffffu;
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
 
-#ifdef AVM_TRACE
-__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
-#define AVM_TR_MAX(slot) do { if (lane == 0) atomicMax(&d.ctr->tr[slot], gtime()); } while (0)
-#define AVM_TR_W0(slot, dep) do { if (trq && blockIdx.x == 0 && threadIdx.x == 0) { if (slot == 0) tq0 = gtime(); else d.ctr->tr2[slot] = gtime() + ((dep) & 0) - tq0; } } while (0)
-#else
-#define AVM_TR_MAX(slot) do { } while (0)
-#define AVM_TR_W0(slot, dep) do { } while (0)
-#endif
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 // ---- cache-hinted loads -------------------------------------------------------------------------
@@ -312,50 +304,20 @@ __device__ __forceinline__ void sweep(const Dev& d, const Consts& k, const unsig
 __device__ AVM_FUSED_ATTR void flipper_flips(const Dev& d, const Consts& k, const unsigned prev, const int lane, const unsigned first) {
   unsigned mine = 0, flips = 0;
   unsigned i = first;
-#ifdef AVM_TRACE
-  const bool w0 = blockIdx.x == 0 && threadIdx.x == 0;
-  unsigned long long ts[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-  ts[0] = gtime();
-#endif
   for (;;) {
     if (i >= prev) {
       const unsigned nc = ld_volatile(&d.ctr->next_cand);
-#ifdef AVM_TRACE
-      if (!ts[1]) ts[1] = gtime() + (nc & 0);
-#endif
       if (nc >= prev) break;        // nothing left: no atomic
       if (lane == 0) i = atomicAdd(&d.ctr->next_cand, 8u);
       i = __shfl_sync(kFull, i, 0);
-#ifdef AVM_TRACE
-      if (!ts[2]) ts[2] = gtime() + (i & 0);
-#endif
       if (i >= prev) break;
     }
-#ifdef AVM_TRACE
-    const unsigned long long tb = gtime();
-    if (w0) d.ctr->tr2[6] = tb;
-#endif
-#ifdef AVM_TRACE
-    flips += t1_flip_quads(d, k, d.cand, i, prev, lane | 0x100);
-#else
     flips += (AVM_FUSED_FLIP_INLINE && k.S <= 16) ? t1_flip_quads_impl<16>(d, k, d.cand, i, prev, lane) : t1_flip_quads(d, k, d.cand, i, prev, lane);
-#endif
-#ifdef AVM_TRACE
-    if (w0) d.ctr->tr2[0] = gtime() + (flips & 0);
-    if (!ts[3]) ts[3] = gtime() + (flips & 0);
-    else if (!ts[7]) ts[7] = ts[0] + gtime() + (flips & 0) - tb;      // duration of the second call
-#endif
     mine += min(8u, prev - i);
     i = prev;
   }
-#ifdef AVM_TRACE
-  ts[4] = gtime();
-#endif
   if (mine) {
     __threadfence();
-#ifdef AVM_TRACE
-    ts[5] = gtime();
-#endif
     __syncwarp();
     if (lane == 0) {
       if (flips) atomicAdd((unsigned long long*)&d.ctr->t1_flips, (unsigned long long)flips);
@@ -363,10 +325,6 @@ __device__ AVM_FUSED_ATTR void flipper_flips(const Dev& d, const Consts& k, cons
       atomicAdd(&d.ctr->flip_done, mine);
     }
   }
-#ifdef AVM_TRACE
-  ts[6] = gtime();
-  if (w0 && mine) for (int j = 1; j < 8; ++j) d.ctr->tr2[8 + j] = ts[j] > ts[0] ? ts[j] - ts[0] : 0;
-#endif
 }
 
 // One unit of post-flip work = one candidate (few-candidate mode): every vertex of the (post-flip)
@@ -428,9 +386,6 @@ force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts 
   if (kFused) {
     if (prev == 0u) { sweep<false>(d, k, nullptr, tid, stride, lane); return; }
     if (tid == 0) atomicAdd((unsigned long long*)&d.ctr->t1_candidates, (unsigned long long)prev);
-#ifdef AVM_TRACE
-    if (lane == 0) atomicMin(&d.ctr->tr[0], gtime());
-#endif
     const unsigned int* __restrict__ dirty = d.dirty + (size_t)(parity ^ 1u) * (size_t)k.nw;
     if (prev <= AVM_LIGHT_MAX && 3u * prev <= nwarps) {      // (a small grid must keep most of its warps for the sweep)
       // few candidates: one dedicated warp per candidate (warp 0 of the first CTAs, then warp 1, ...:
@@ -462,9 +417,7 @@ force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts 
           __nanosleep(64);
           if (++polls == 64u) { polls = 0; claim = true; }
         }
-        AVM_TR_MAX(1);
         __threadfence();
-        AVM_TR_MAX(3);
 #if AVM_TEST_SKEW == 3
         if (fid & 1u) {
           unsigned long long t0, t1;
@@ -473,11 +426,9 @@ force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts 
         }
 #endif
         mover_unit(d, k, fid, lane, step);
-        AVM_TR_MAX(4);
       } else {
         const unsigned before = blockIdx.x * full + min(blockIdx.x, rest) + min(wib, full) + (wib > full && blockIdx.x < rest ? 1u : 0u);
         sweep<true>(d, k, dirty, (int)((gwarp - before) * 32u) + lane, (int)((nwarps - prev) * 32u), lane);
-        AVM_TR_MAX(2);
       }
     } else {
       // many candidates (the burst after a random start, T1-heavy regimes): the flips come first,
@@ -488,13 +439,10 @@ force_move_kernel(const __grid_constant__ Dev d, const __grid_constant__ Consts 
       if (threadIdx.x == 0) s_first = atomicAdd(&d.ctr->next_cand, 8u * (kVertexBlock / 32));   // one claim per CTA
       __syncthreads();
       flipper_flips(d, k, prev, lane, s_first + 8u * (threadIdx.x >> 5));
-      AVM_TR_MAX(1);
       while (ld_volatile(&d.ctr->flip_done) < prev) __nanosleep(32);
       __threadfence();
-      AVM_TR_MAX(3);
       release_minkeys(d, 0u, prev, (unsigned)stride, (unsigned)tid);       // every decision has been taken (row a6)
       sweep<false>(d, k, nullptr, tid, stride, lane);
-      AVM_TR_MAX(2);
     }
   } else {
     // the previous step's T1 candidates are done: clear their cells' minimum keys (row a6)
@@ -653,14 +601,6 @@ template <bool kStep, bool kPerCell, int kCoh, bool kObserve = false>
 __device__ __forceinline__ void cell_update_body(const Dev& d, const Consts& k, const unsigned long long step, const unsigned parity,
                                                  const int gid, double* __restrict__ obs_partial = nullptr) {
   if (kStep && gid == 0) { d.ctr->flip_done = 0; d.ctr->next_cand = 0; }   // the previous list is long done
-#ifdef AVM_TRACE
-  if (kStep && gid == 0) {
-    const unsigned long long t0 = d.ctr->tr[0];
-    if (t0 != ~0ull) { for (int i = 1; i < 8; ++i) if (d.ctr->tr[i] > t0) d.ctr->tr_acc[i] += d.ctr->tr[i] - t0; d.ctr->tr_acc[0] += 1; }
-    d.ctr->tr[0] = ~0ull;
-    for (int i = 1; i < 8; ++i) d.ctr->tr[i] = 0;
-  }
-#endif
   // the bitmap the force/move launch of this step swept with is spent: clear it for the next step's cell pass
   if (kStep && k.clear_dirty && gid < k.nw) d.dirty[(size_t)(parity ^ 1u) * (size_t)k.nw + gid] = 0u;
   const bool valid = gid < k.N;
@@ -922,9 +862,6 @@ __device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Const
                                                        const int4* __restrict__ pre) {
   // pre (optional): the 64 bytes of this lane's candidate, fetched by the caller before the list length was known
   const int lane = lane_in & 31;
-#ifdef AVM_TRACE
-  const bool trq = (lane_in & 0x100) != 0;
-#endif
   const int t = lane & 3;
   const unsigned i = base + (unsigned)(lane >> 2);
   const bool have = i < n;
@@ -932,20 +869,12 @@ __device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Const
   // one another (the marking thread decoded the neighbourhood), so the decision costs no extra
   // round trip: phase 1 = the candidate, phase 2 = keys, rows and the two end points
   int4 ca = make_int4(0, 0, 0, 0), cb = ca, cc = ca, cd = ca;
-#ifdef AVM_TRACE
-  unsigned long long tq0 = 0;
-  const unsigned long long tqe = gtime();
-  if (trq && blockIdx.x == 0 && threadIdx.x < 32) d.ctr->tr2[16 + threadIdx.x] = 0, d.ctr->tr2[48 + threadIdx.x] = 0;
-  if (trq && blockIdx.x == 0 && threadIdx.x == 0) d.ctr->tr2[7] = tqe;
-#endif
-  AVM_TR_W0(0, 0);
   if (pre) {
     if (have) { ca = pre[0]; cb = pre[1]; cc = pre[2]; cd = pre[3]; }
   } else if (have) {
     const int4* __restrict__ src = reinterpret_cast<const int4*>(list + i);
     ca = __ldcg(src); cb = __ldcg(src + 1); cc = __ldcg(src + 2); cd = __ldcg(src + 3);
   }
-  AVM_TR_W0(1, ca.x + cb.x + cc.x + cd.x);
   const int v1 = ca.x, v2 = ca.y, k1 = ca.z, k2 = ca.w;
   const int cL = cb.x, cR = cb.y, cE1 = cb.z, cE2 = cb.w;
   const unsigned long long key = ((unsigned long long)(unsigned)cc.y << 32) | (unsigned)cc.x;
@@ -968,10 +897,6 @@ __device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Const
   const unsigned agree = __ballot_sync(kFull, have && mk == key);
   const unsigned wins = __ballot_sync(kFull, ((agree >> (lane & ~3)) & 0xfu) == 0xfu);
   const unsigned nflips = (unsigned)__popc(wins & 0x11111111u);
-  AVM_TR_W0(2, (int)wins + r[0] + r[4] + r[8] + r[12] + nrow + (int)h1.x + (int)h2.x);
-#ifdef AVM_TRACE
-  if (trq && blockIdx.x == 0 && threadIdx.x < 32) d.ctr->tr2[16 + threadIdx.x] = gtime() - tqe + (((int)wins + r[0] + r[4] + r[8] + r[12] + nrow + (int)h1.x + (int)h2.x) & 0);
-#endif
   if (!((wins >> lane) & 1u)) return nflips;
   // ---- geometry: rigid counter-clockwise quarter turn about the midpoint, new length 1.5 l_c (R9);
   // every lane of the group evaluates it (same bits) because each needs both new positions below
@@ -1033,7 +958,6 @@ __device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Const
   for (int q = 0; q < kR / 4; ++q)
     if (4 * q < k.S && (q < 2 || 4 * q < need)) d.cv[(size_t)q * k.N + cell] = make_int4(r[4 * q], r[4 * q + 1], r[4 * q + 2], r[4 * q + 3]);
   d.cvn[cell] = nnew;
-  AVM_TR_W0(3, nnew);
   // ---- refresh the cached geometry of my cell (directors unchanged): the same serial sum as the
   // per-step pass (geom_edge), so that a resumed run reproduces these records bit for bit.  Positions
   // are fetched eight at a time with unconditional, mutually independent loads (entries beyond the
@@ -1065,16 +989,10 @@ __device__ __forceinline__ unsigned t1_flip_quads_impl(const Dev& d, const Const
     }
   }
   geom_edge(rxp, ryp, 0.0, 0.0, acc, per);      // the closing edge back to entry 0
-  AVM_TR_W0(4, (int)acc);
   double ra, rp;
   if (k.per_cell) rec_from_geometry(d.par[cell], __dmul_rn(0.5, acc), per, ra, rp);
   else { ra = k.KA2 * (__dmul_rn(0.5, acc) - k.A0); rp = k.KP2 * (per - k.P0); }
   rec_st_ap(d.rec + cell, ra, rp);
-  AVM_TR_W0(5, 0);
-#ifdef AVM_TRACE
-  if (trq && blockIdx.x == 0 && threadIdx.x < 32) d.ctr->tr2[48 + threadIdx.x] = gtime() - tqe;
-  if (trq && blockIdx.x == 0 && threadIdx.x == 0) d.ctr->tr2[8] = gtime();
-#endif
   return nflips;
 }
 __device__ __noinline__ unsigned t1_flip_quads(const Dev& d, const Consts& k, const Cand* __restrict__ list, const unsigned base,
